@@ -1,0 +1,258 @@
+"""Pins for the oracle's fields: summation density (eq.3), Tait EOS (eq.6, Listing 4),
+momentum (eq.8-9, Listing 4) with artificial viscosity (R9) and
+continuity (eq.7).  Each pin is something the paper or the mathematics fixes, chosen so that a
+dropped term, a wrong sign or index, or a transposed operand fails at least one of them."""
+import numpy as np
+import pytest
+
+from conftest import golden_path
+
+
+def _golden():
+    for line in open(golden_path("lattice_sums.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        dim, kernel, hdx, rho, count = line.split()
+        yield int(dim), kernel, float(hdx), float(rho), int(count)
+
+
+# ------------------------------------------------------------------------------------ density
+@pytest.mark.parametrize("dim,kernel,hdx,rho_ref,count", list(_golden()))
+def test_lattice_density_uniform_and_equal_to_lattice_sum(O, WL, dim, kernel, hdx, rho_ref, count):
+    n = (32, 32) if dim == 2 else (16, 16, 16)
+    wl = WL.lattice(n, dim, hdx, kernel)
+    st = O.State(wl)
+    st.arrays[0]["h"][:] = hdx / n[0]                    # the exact real h, not its float32 rounding
+    st.arrays[0]["m"][:] = (1.0 / n[0]) ** dim
+    for method in ("cell", "brute"):
+        rho, ab, pairs = O.density(wl, st, 0, [0], pred32=False, method=method)
+        assert np.ptp(rho) < 1e-13 * rho.mean()          # uniform on an unjittered periodic lattice
+        assert rho.mean() == pytest.approx(rho_ref, rel=2e-12)
+        assert pairs == count * wl.n_total
+        assert np.array_equal(rho, ab)
+
+
+def test_two_particle_density_by_hand(O, WL):
+    """rho_0 = m_0 W(0,h_00) + m_1 W(r,h_01) with the cubic spline written out here (2-D, q<1 and 1<q<2)."""
+    wl = WL.random_box(n=2, dim=2, periodic=False, seed=1, kernel="cubic")
+    st = O.State(wl)
+    A = st.arrays[0]
+    sig = 10.0 / (7.0 * np.pi)
+    for r, branch in ((0.06, 0), (0.15, 1)):
+        A["x"][:] = [0.3, 0.3 + r]; A["y"][:] = [0.4, 0.4]; A["h"][:] = [0.1, 0.1]; A["m"][:] = [2.0, 3.0]
+        q = r / 0.1
+        f = 1 - 1.5 * q * q + 0.75 * q ** 3 if branch == 0 else 0.25 * (2 - q) ** 3
+        rho, _, pairs = O.density(wl, st, 0, [0], pred32=False, method="brute")
+        assert pairs == 4
+        assert rho[0] == pytest.approx(2.0 * sig / 0.01 + 3.0 * sig / 0.01 * f, rel=1e-14)
+        assert rho[1] == pytest.approx(3.0 * sig / 0.01 + 2.0 * sig / 0.01 * f, rel=1e-14)
+    # variable h: the pair uses h_ij = (h_i+h_j)/2 (R3), the self term h_i
+    A["x"][:] = [0.3, 0.42]; A["h"][:] = [0.1, 0.14]
+    q = 0.12 / 0.12
+    f = 0.25 * (2 - q) ** 3
+    rho, _, _ = O.density(wl, st, 0, [0], pred32=False, method="brute")
+    assert rho[0] == pytest.approx(2.0 * sig / 0.1 ** 2 + 3.0 * sig / 0.12 ** 2 * f, rel=1e-13)
+
+
+def test_density_sources_are_additive(O, WL):
+    wl = WL.random_box(n=1200, dim=3, periodic=True, seed=3, two_arrays=True, variable_h=True)
+    st = O.State(wl)
+    a, _, _ = O.density(wl, st, 0, [0])
+    b, _, _ = O.density(wl, st, 0, [1])
+    ab, _, _ = O.density(wl, st, 0, [0, 1])
+    assert np.allclose(a + b, ab, rtol=1e-14, atol=0)
+
+
+# ------------------------------------------------------------------------------------ EOS
+def test_tait_eos(O, WL):
+    wl = WL.dam_break_2d()
+    rho0, c0 = wl.rho0, wl.c0
+    assert O.eos(wl, np.array([rho0]))[0] == 0.0                                  # p(rho0) = 0
+    e = 1e-6 * rho0
+    dp = (O.eos(wl, np.array([rho0 + e]))[0] - O.eos(wl, np.array([rho0 - e]))[0]) / (2 * e)
+    assert dp == pytest.approx(c0 * c0, rel=1e-9)                                 # dp/drho = c0^2
+    B = rho0 * c0 * c0 / 7.0                                                      # Listing 4
+    assert O.eos(wl, np.array([2 * rho0]))[0] == pytest.approx(B * 127.0, rel=1e-14)   # gamma = 7 (L124)
+    assert O.eos(wl, np.array([0.5 * rho0]))[0] == pytest.approx(B * (2.0 ** -7 - 1.0), rel=1e-14)
+
+
+# ------------------------------------------------------------------------------------ momentum
+def _prepared(O, WL, **kw):
+    wl = WL.random_box(**kw)
+    st = O.State(wl)
+    for d in range(len(st.arrays)):
+        st.arrays[d]["p"] = O.eos(wl, st.arrays[d]["rho"])
+    return wl, st
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_momentum_conservation(O, WL, dim):
+    """Symmetric pair terms => sum_i m_i a_i = 0 to round-off (periodic, no gravity, variable h, any rho,p,v)."""
+    wl, st = _prepared(O, WL, n=1500, dim=dim, periodic=True, seed=31, variable_h=True, kernel="wendland_c2")
+    o = O.accel(wl, st, 0, [0], pred32=False)
+    m = st.arrays[0]["m"]
+    scale = (m * o["abs_a"]).sum()
+    for k in ("au", "av", "aw")[:dim]:
+        assert abs((m * o[k]).sum()) < 1e-13 * scale
+    assert np.abs(o["au"]).max() > 1e-3                   # not trivially zero
+    if dim == 2:
+        assert not o["aw"].any()
+
+
+def test_two_particle_acceleration_by_hand(O, WL):
+    """One approaching pair, 2-D cubic, written out from eq.9 + R9."""
+    wl, st = _prepared(O, WL, n=2, dim=2, periodic=False, seed=1, kernel="cubic")
+    A = st.arrays[0]
+    A["x"][:] = [0.30, 0.42]; A["y"][:] = [0.40, 0.45]; A["h"][:] = [0.1, 0.1]; A["m"][:] = [2.0, 3.0]
+    A["rho"][:] = [1.1, 0.9]; A["p"][:] = [0.7, -0.2]
+    A["u"][:] = [1.0, -1.0]; A["v"][:] = [0.2, 0.0]
+    o = O.accel(wl, st, 0, [0], pred32=False, method="brute")
+    d = np.array([-0.12, -0.05]); r = np.hypot(*d); h = 0.1; q = r / h
+    assert 1 < q < 2
+    dw = 10 / (7 * np.pi) / h ** 3 * (-0.75 * (2 - q) ** 2)
+    grad0 = dw * d / r                                     # grad_0 W_01
+    v01 = np.array([2.0, 0.2]); vr = v01 @ d
+    assert vr < 0
+    mu = h * vr / (r * r + wl.eps * h * h)
+    Pi = -wl.alpha * wl.c0 * mu / 1.0
+    tmp = 0.7 / 1.1 ** 2 + (-0.2) / 0.9 ** 2 + Pi
+    a0 = -3.0 * tmp * grad0
+    a1 = -2.0 * tmp * (-grad0)
+    assert o["au"][0] == pytest.approx(a0[0], rel=1e-13) and o["av"][0] == pytest.approx(a0[1], rel=1e-13)
+    assert o["au"][1] == pytest.approx(a1[0], rel=1e-13) and o["av"][1] == pytest.approx(a1[1], rel=1e-13)
+    assert o["arho"][0] == pytest.approx(3.0 * (v01 @ grad0), rel=1e-13)             # eq.7
+    assert o["arho"][1] == pytest.approx(2.0 * ((-v01) @ (-grad0)), rel=1e-13)
+    # receding pair: Pi = 0 -> pure eq.9
+    A["u"][:] = [-1.0, 1.0]
+    o = O.accel(wl, st, 0, [0], pred32=False, method="brute")
+    a0 = -3.0 * (0.7 / 1.1 ** 2 - 0.2 / 0.9 ** 2) * grad0
+    assert o["au"][0] == pytest.approx(a0[0], rel=1e-13)
+
+
+def test_gravity_is_the_initial_value(O, WL):
+    """Listing 4: the accumulator starts at the body force; an isolated particle gets exactly g."""
+    wl, st = _prepared(O, WL, n=2, dim=2, periodic=False, seed=1, g=(0.0, -9.81, 0.0))
+    A = st.arrays[0]
+    A["x"][:] = [0.1, 0.9]; A["y"][:] = [0.1, 0.9]; A["h"][:] = 0.01
+    o = O.accel(wl, st, 0, [0])
+    assert (o["au"] == 0.0).all() and (o["av"] == -9.81).all() and o["n_pairs"] == 2
+
+
+def test_galilean_invariance_and_alpha_zero(O, WL):
+    wl, st = _prepared(O, WL, n=1000, dim=3, periodic=True, seed=33)
+    o1 = O.accel(wl, st, 0, [0])
+    st2 = st.copy()
+    for k, c in zip("uvw", (3.0, -2.0, 0.5)):
+        st2.arrays[0][k] += c
+    o2 = O.accel(wl, st2, 0, [0])
+    for k in ("au", "av", "aw", "arho"):
+        assert np.allclose(o1[k], o2[k], rtol=0, atol=1e-12 * np.abs(o1[k]).max())
+    # alpha = 0 -> no dependence on velocity at all (pure eq.9)
+    o3 = O.accel(wl, st, 0, [0], alpha=0.0)
+    st3 = st.copy(); st3.arrays[0]["u"] *= -7.0
+    o4 = O.accel(wl, st3, 0, [0], alpha=0.0)
+    assert np.array_equal(o3["au"], o4["au"]) and not np.allclose(o3["au"], o1["au"])
+
+
+def test_rotation_covariance_2d(O, WL):
+    """Rotate the whole state by 90 degrees about the box centre: accelerations rotate with it."""
+    wl, st = _prepared(O, WL, n=900, dim=2, periodic=True, seed=34, variable_h=True, kernel="quintic")
+    o1 = O.accel(wl, st, 0, [0], pred32=False)
+    st2 = st.copy(); A, B = st.arrays[0], st2.arrays[0]
+    B["x"], B["y"] = 1.0 - A["y"], A["x"].copy()
+    B["x"] = np.where(B["x"] >= 1.0, B["x"] - 1.0, B["x"])
+    B["u"], B["v"] = -A["v"], A["u"].copy()
+    o2 = O.accel(wl, st2, 0, [0], pred32=False)
+    s = np.abs(o1["au"]).max()
+    assert np.allclose(o2["au"], -o1["av"], rtol=0, atol=1e-11 * s)
+    assert np.allclose(o2["av"], o1["au"], rtol=0, atol=1e-11 * s)
+    assert np.allclose(o2["arho"], o1["arho"], rtol=0, atol=1e-11 * np.abs(o1["arho"]).max())
+
+
+def test_uniform_pressure_on_lattice_gives_zero(O, WL):
+    wl = WL.lattice((32, 32), 2, 1.3, "cubic")
+    st = O.State(wl)
+    st.arrays[0]["p"][:] = 5.0
+    o = O.accel(wl, st, 0, [0])
+    assert np.abs(o["au"]).max() < 1e-12 * o["abs_a"].max() and np.abs(o["av"]).max() < 1e-12 * o["abs_a"].max()
+
+
+@pytest.mark.parametrize("kernel,hdx", [("cubic", 1.3), ("quintic", 1.0), ("wendland_c2", 1.3)])
+def test_pressure_gradient_continuum_limit(O, WL, kernel, hdx):
+    """eq.5/eq.9: a_p -> -(1/rho) grad p.  p = sin(2 pi x) cos(2 pi y) on a 64^2 lattice, rho = 1."""
+    wl = WL.lattice((64, 64), 2, hdx, kernel)
+    st = O.State(wl); A = st.arrays[0]
+    x, y = A["x"], A["y"]
+    A["p"] = np.sin(2 * np.pi * x) * np.cos(2 * np.pi * y)
+    o = O.accel(wl, st, 0, [0], alpha=0.0)
+    ex = -2 * np.pi * np.cos(2 * np.pi * x) * np.cos(2 * np.pi * y)
+    ey = 2 * np.pi * np.sin(2 * np.pi * x) * np.sin(2 * np.pi * y)
+    e64 = np.abs(o["au"] - ex).max()
+    assert e64 < 0.04 * 2 * np.pi
+    assert np.abs(o["av"] - ey).max() < 0.04 * 2 * np.pi
+    assert np.corrcoef(o["au"], ex)[0, 1] > 0.9999          # right sign, right component
+    # (at fixed h/dx the lattice-sum error of the SPH gradient does not vanish under refinement, so
+    #  no convergence ratio is asserted; 4 % bounds smoothing + discretisation error for these h/dx)
+    assert np.abs(o["au"]).max() == pytest.approx(2 * np.pi, rel=0.04)
+
+
+def test_continuity_continuum_limit_and_uniform_flow(O, WL):
+    """eq.4/eq.7: arho -> -rho div(v);  uniform velocity => arho = 0 exactly."""
+    wl = WL.lattice((64, 64), 2, 1.3, "cubic")
+    st = O.State(wl); A = st.arrays[0]
+    A["u"][:] = 0.3; A["v"][:] = -1.1
+    assert not O.accel(wl, st, 0, [0])["arho"].any()
+    x, y = A["x"], A["y"]
+    A["u"] = np.sin(2 * np.pi * x); A["v"] = np.cos(2 * np.pi * y) * 0.5
+    o = O.accel(wl, st, 0, [0])
+    div = 2 * np.pi * np.cos(2 * np.pi * x) - np.pi * np.sin(2 * np.pi * y)
+    assert np.abs(o["arho"] + 1.0 * div).max() < 0.03 * 3 * np.pi
+    assert np.corrcoef(o["arho"], -div)[0, 1] > 0.9999
+
+
+def test_viscosity_dissipates(O, WL):
+    """Pi_ij >= 0 only for approaching pairs => sum_i m_i u_i . a_visc,i <= 0 (total, by pair symmetry)."""
+    wl, st = _prepared(O, WL, n=2000, dim=3, periodic=True, seed=35)
+    o = O.accel(wl, st, 0, [0])
+    m = st.arrays[0]["m"]
+    assert (m * o["visc_power"]).sum() < 0.0
+
+
+def test_taylor_green_decay_rate_bracket(O, WL):
+    """C1 state: the artificial viscosity acts like nu = alpha h c0 / 8 on all pairs in
+    2-D (continuum limit of Pi); acting on approaching pairs only it gives about half of that.  So
+    nu_eff = -(dE/dt)/(16 pi^2 E)... measured from one evaluation as -sum m u.a_visc / (8 pi^2 * 2 KE)
+    must lie in [alpha h c0/16 * 0.8, alpha h c0/8 * 1.2], i.e. the kinetic energy decays like
+    exp(2 b t) with b = -8 pi^2 nu (L657 with nu = 1/Re)."""
+    wl = WL.taylor_green_2d()
+    st = O.State(wl)
+    O.evaluate(wl, st, "summation")
+    A = st.arrays[0]
+    o = O.accel(wl, st, 0, [0])
+    m = A["m"]
+    ke = 0.5 * (m * (A["u"] ** 2 + A["v"] ** 2)).sum()
+    power = (m * o["visc_power"]).sum()                       # dKE/dt from viscosity
+    nu_eff = -power / (16 * np.pi ** 2 * ke)                  # dKE/dt = 2 b KE = -16 pi^2 nu KE
+    h = float(A["h"][0])
+    full = wl.alpha * h * wl.c0 / 8.0
+    assert 0.8 * full / 2 < nu_eff < 1.2 * full
+    assert ke == pytest.approx(0.25, rel=2e-2)                # <u^2+v^2>/2 = 1/4 for U = 1
+
+
+def test_fluid_solid_tables(O, WL):
+    """Listing 3 (L363-378): continuity fluid<-{fluid,solid}, solid<-{fluid}; momentum fluid<-{fluid,solid}."""
+    wl = WL.dam_break_2d(dx=0.05)
+    assert wl.accel_sources == [[0, 1], []] and wl.arho_sources == [[0, 1], [0]]
+    st = O.State(wl)
+    st.arrays[0]["v"][:] = -1.0                                # fluid falling onto the fixed floor
+    O.evaluate(wl, st, "continuity")
+    F, S = st.arrays
+    assert (F["p"] == 0).all() and (S["p"] == 0).all()        # rho = rho0 everywhere -> p = 0
+    assert not S["au"].any() and not S["av"].any()
+    floor = (S["y"] > -0.05) & (S["x"] > 0.2) & (S["x"] < 0.8)
+    assert floor.any() and (S["arho"][floor] > 0).all()       # approaching fluid compresses the floor layer
+    far = S["x"] > 2.0
+    assert not S["arho"][far].any()                            # solids with no fluid neighbour: nothing
+    near_floor = F["y"] < 0.1
+    assert (F["arho"][near_floor] > 0).all()
+    assert (F["av"][near_floor] > -9.81).all()                 # viscous push back from the wall

@@ -1,0 +1,105 @@
+"""Pins for the oracle's predictor-corrector step (eqs. 12-14; R10/R11).
+Closed forms and invariants: constant acceleration is integrated exactly; the kick-drift-kick form is
+time reversible and second order; fixed arrays do not move; the periodic wrap keeps x in [lo,hi)."""
+import numpy as np
+import pytest
+
+
+def test_free_fall_is_an_exact_parabola(O, WL):
+    """No neighbours + gravity: eqs. 12-14 give x0 + u0 t + g t^2/2 for ANY dt (KDK is exact for constant a)."""
+    wl = WL.random_box(n=3, dim=2, periodic=False, seed=1, g=(0.0, -9.81, 0.0))
+    st = O.State(wl); A = st.arrays[0]
+    A["x"][:] = [0.1, 0.5, 0.9]; A["y"][:] = [0.9, 0.5, 0.1]; A["h"][:] = 1e-3
+    A["u"][:] = [1.0, 0.0, -1.0]; A["v"][:] = [0.0, 2.0, 0.5]
+    x0, y0, u0, v0 = (A[k].copy() for k in "xyuv")
+    dt, n = 0.013, 7
+    for _ in range(n):
+        O.pc_step(wl, st, dt, "summation")
+    t = n * dt
+    assert np.allclose(A["x"], x0 + u0 * t, rtol=0, atol=1e-14)
+    assert np.allclose(A["y"], y0 + v0 * t - 0.5 * 9.81 * t * t, rtol=0, atol=1e-13)
+    assert np.allclose(A["v"], v0 - 9.81 * t, rtol=0, atol=1e-13)
+    assert np.array_equal(A["u"], u0)
+
+
+def test_single_step_is_eqs_12_to_14(O, WL):
+    """One step from a state with known a^n: recompute eqs. 12-14 by hand around the oracle's own F."""
+    wl = WL.random_box(n=400, dim=2, periodic=True, seed=41, variable_h=True)
+    st = O.State(wl)
+    O.evaluate(wl, st, "summation")
+    s0 = st.copy(); A0 = s0.arrays[0]
+    dt = wl.dt
+    O.pc_step(wl, st, dt, "summation")
+    A1 = st.arrays[0]
+    uh = A0["u"] + 0.5 * dt * A0["au"]                        # (12)
+    x1 = A0["x"] + dt * uh                                    # (13)
+    x1 = np.where(x1 >= 1.0, x1 - 1.0, np.where(x1 < 0.0, x1 + 1.0, x1))
+    assert np.array_equal(A1["x"], x1)
+    assert np.allclose(A1["u"], uh + 0.5 * dt * A1["au"], rtol=0, atol=1e-15)   # (14) with a^{n+1}
+    assert (A1["x"] >= 0).all() and (A1["x"] < 1.0).all()
+    # a^{n+1} was evaluated at (x^{n+1}, u^{n+1/2}) (R10)
+    chk = s0.copy(); C = chk.arrays[0]
+    C["x"] = x1; C["y"] = A1["y"]; C["u"] = uh; C["v"] = A0["v"] + 0.5 * dt * A0["av"]
+    O.evaluate(wl, chk, "summation")
+    assert np.allclose(chk.arrays[0]["au"], A1["au"], rtol=0, atol=1e-12 * np.abs(A1["au"]).max())
+
+
+def test_time_reversibility(O, WL):
+    """KDK with alpha = 0 in summation mode: a step dt followed by a step -dt returns to the start."""
+    wl = WL.random_box(n=500, dim=2, periodic=True, seed=42)
+    wl.alpha = 0.0
+    st = O.State(wl)
+    A = st.arrays[0]
+    A["u"] *= 0.05; A["v"] *= 0.05
+    s0 = st.copy()
+    dt = wl.dt
+    for _ in range(3):
+        O.pc_step(wl, st, dt, "summation")
+    moved = np.abs(st.arrays[0]["x"] - s0.arrays[0]["x"]).max()
+    for _ in range(3):
+        O.pc_step(wl, st, -dt, "summation")
+    for k in "xyuv":
+        assert np.abs(st.arrays[0][k] - s0.arrays[0][k]).max() < 1e-9 * max(1.0, moved / dt)
+    assert moved > 1e-6
+
+
+def test_second_order_convergence(O, WL):
+    """Halving dt divides the error against a fine reference by about 4 (2nd-order scheme, L146)."""
+    wl = WL.lattice((16, 16), 2, 1.3, "cubic")
+    wl.alpha = 0.0
+    base = O.State(wl); A = base.arrays[0]
+    A["u"] = 0.2 * np.sin(2 * np.pi * A["y"]); A["v"] = 0.2 * np.sin(2 * np.pi * A["x"])
+    T = 16 * wl.dt
+
+    def run(nsteps):
+        st = base.copy()
+        for _ in range(nsteps):
+            O.pc_step(wl, st, T / nsteps, "summation")
+        return np.concatenate([st.arrays[0]["u"], st.arrays[0]["v"]])
+    ref = run(128)
+    e1 = np.abs(run(8) - ref).max()
+    e2 = np.abs(run(16) - ref).max()
+    assert 3.0 < e1 / e2 < 5.5
+
+
+def test_fixed_arrays_and_continuity_mode(O, WL):
+    """L142: the tank particles are fixed, but the continuity equation is solved on them and p set by the EOS."""
+    wl = WL.dam_break_2d(dx=0.05)
+    st = O.State(wl)
+    S0 = {k: st.arrays[1][k].copy() for k in "xyuv"}
+    for _ in range(5):
+        O.pc_step(wl, st, wl.dt, "continuity")
+    F, S = st.arrays
+    for k in "xyuv":
+        assert np.array_equal(S[k], S0[k])
+    assert (F["v"] < 0).all()                                 # everything is falling
+    assert F["v"].min() == pytest.approx(-9.81 * 5 * wl.dt, rel=0.3)
+    assert S["rho"].max() > wl.rho0 and (S["p"][S["rho"] > wl.rho0] > 0).all()
+    assert np.abs(F["rho"] / wl.rho0 - 1).max() < 0.02        # weakly compressible
+
+
+def test_no_move_option(O, WL):
+    wl = WL.random_box(n=300, dim=3, periodic=True, seed=43, variable_h=True)
+    st = O.State(wl); x0 = st.arrays[0]["x"].copy(); u0 = st.arrays[0]["u"].copy()
+    O.pc_step(wl, st, wl.dt, "summation", move=False)
+    assert np.array_equal(st.arrays[0]["x"], x0) and not np.array_equal(st.arrays[0]["u"], u0)
