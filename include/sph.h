@@ -1,0 +1,180 @@
+/* sph.h -- C ABI of the B200-native SPH hot path of arXiv 1909.04504 (PySPH).
+ *
+ * One library, libsph_b200.so, hand-written CUDA for sm_100a.  Every step of the path runs in its
+ * kernels; there is NO CPU fallback: each call fails with SPH_ERR_CUDA if no device is usable.
+ *
+ * Problem statement (PAPER.md, cited as L<line>):
+ *   - particles live in NAMED ARRAYS of per-particle properties x,y,z,u,v,w,h,m,rho,p, one 1-D
+ *     contiguous array per property (L205, L316);
+ *   - an equation acts on ONE destination array from a LIST of source arrays (L382, L423-425);
+ *   - neighbours of i are the particles within the kernel support k*h (L106, L158), found with a
+ *     uniform cell grid sorted by cell key, rebuilt whenever particles move (L158-170, L443);
+ *   - groups are barriers: the EOS of ALL arrays completes before the momentum equation (L337).
+ *
+ * Conventions
+ *   real type      float (the paper's GPU runs are single precision, L733).
+ *   pointers       every particle buffer is CALLER-OWNED.  `mem` says where it lives: SPH_MEM_DEVICE
+ *                  (device pointers on the context's device) or SPH_MEM_HOST (host pointers; the library
+ *                  copies through its own staging buffers with cudaMemcpyAsync on the context stream --
+ *                  pinned memory makes those copies asynchronous).  The library never frees or
+ *                  reallocates caller memory.  Arrays must be contiguous; z,w may be NULL when dim == 2.
+ *   ownership      sph_ctx is opaque and LIBRARY-OWNED; it holds all workspace (cell tables, the
+ *                  cell-sorted mirror of the particle state), allocated once in sph_create from
+ *                  `capacity`.  No call allocates device memory after sph_create.
+ *   asynchrony     all work is enqueued on the stream given to sph_create.  Calls marked [sync]
+ *                  synchronise that stream before returning; the others do not.
+ *   errors         every call returns 0 (SPH_OK) or a negative sph_error.  Argument errors are detected
+ *                  on the host before any work is enqueued.  Device-side conditions (a particle outside a
+ *                  non-periodic domain, a non-finite result) set a device flag that the next [sync] call
+ *                  reports.  sph_last_error(ctx) gives a message.  n == 0 arrays are legal.
+ *   order          results are returned in the CALLER's particle order (the internal state is cell-sorted).
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPH_MAX_ARRAYS 4
+#define SPH_ABI_VERSION 1
+
+typedef struct sph_ctx sph_ctx;
+
+enum sph_error {
+    SPH_OK = 0,
+    SPH_ERR_NULL = -1,          /* a required pointer is NULL                                  */
+    SPH_ERR_BAD_ARG = -2,       /* invalid value (dim, kernel, mask, periodic axis with < 3 cells ...) */
+    SPH_ERR_CAPACITY = -3,      /* n exceeds the capacity given to sph_create, or output too small */
+    SPH_ERR_STALE_NNPS = -4,    /* call needs a neighbour structure and none has been built      */
+    SPH_ERR_OUT_OF_DOMAIN = -5, /* [sync] particles left a non-periodic domain box               */
+    SPH_ERR_NONFINITE = -6,     /* [sync] NaN/Inf produced by a pair loop                        */
+    SPH_ERR_CUDA = -7           /* CUDA runtime error (message in sph_last_error)                */
+};
+
+enum sph_kernel {               /* smoothing kernels, R1 (the paper prints none: L209, L435) */
+    SPH_KERNEL_CUBIC = 0,       /* cubic spline,   support 2h */
+    SPH_KERNEL_QUINTIC = 1,     /* quintic spline, support 3h */
+    SPH_KERNEL_WENDLAND_C2 = 2  /* Wendland C2,    support 2h */
+};
+
+enum sph_density_mode {
+    SPH_DENSITY_SUMMATION = 0,  /* rho from eq.3 (L112) every evaluation                          */
+    SPH_DENSITY_CONTINUITY = 1  /* rho integrated from eq.7 (L126), as the paper's dam break (L142, L369-374) */
+};
+
+enum sph_mem { SPH_MEM_DEVICE = 0, SPH_MEM_HOST = 1 };
+enum sph_array_flags { SPH_ARRAY_DYNAMIC = 0, SPH_ARRAY_FIXED = 1 /* x,u never updated (tank walls, L142) */ };
+
+typedef struct sph_domain {     /* create_domain / update_domain (L443-445) */
+    int dim;                    /* 2 or 3 */
+    double lo[3], hi[3];        /* box; on a non-periodic axis it must enclose all particles */
+    int periodic[3];            /* per axis; a periodic axis needs (hi-lo) >= 3 * k * h_max */
+} sph_domain;
+
+typedef struct sph_params {
+    int kernel;                 /* enum sph_kernel */
+    double rho0, c0, gamma;     /* Tait EOS, eq.6 (L122): p = (rho0 c0^2/gamma)[(rho/rho0)^gamma - 1] */
+    double alpha, eps;          /* artificial viscosity (R9): Pi = -alpha c0 mu/rhobar, mu = h vr/(r^2+eps h^2) */
+    double g[3];                /* body force = initial value of the accumulator (Listing 4) */
+    int move;                   /* 1: sph_pc_step applies eq.13 (default); 0: positions frozen (config C5) */
+} sph_params;
+
+typedef struct sph_array {      /* one named particle array (L316) */
+    int64_t n;
+    int flags;                  /* enum sph_array_flags */
+    int mem;                    /* enum sph_mem: where the pointers below live */
+    float *x, *y, *z;           /* positions      (z NULL allowed when dim == 2) */
+    float *u, *v, *w;           /* velocities     (w NULL allowed when dim == 2; all NULL -> 0) */
+    float *h;                   /* smoothing length; sets the search radius (L316) */
+    float *m;                   /* mass           (NULL -> 0: array only queries, never a source of mass) */
+    float *rho;                 /* density        (NULL -> rho0) */
+    float *p;                   /* pressure       (NULL -> EOS(rho)) */
+} sph_array;
+
+typedef struct sph_stats {
+    int32_t n_cells[3];         /* grid dimensions */
+    double cell_size[3];
+    int64_t n_particles;        /* all arrays */
+    int64_t pairs_density;      /* (i,j) pairs passing the predicate in the last density pass(es), self pairs included */
+    int64_t pairs_accel;        /* same for the last acceleration pass(es) */
+    int64_t candidates;         /* predicate evaluations in the last pair pass */
+    int64_t kernel_launches;    /* CUDA kernels launched by this context since sph_create */
+    int64_t steps_done;         /* predictor-corrector steps since the last sph_nnps_build */
+    int32_t variable_h;         /* 1 if h_min != h_max at the last build */
+    float h_max;
+} sph_stats;
+
+/* ---- lifetime ------------------------------------------------------------------------------- */
+
+/* Creates a context for `n_arrays` (1..SPH_MAX_ARRAYS) particle arrays of at most capacity[a] particles.
+ * cuda_stream: a cudaStream_t (e.g. torch.cuda.Stream.cuda_stream), NULL = the legacy default stream.
+ * Allocates all workspace (about 120 B per particle of capacity + the cell tables).  [sync] */
+int sph_create(sph_ctx** out, const sph_params* params, const sph_domain* domain,
+               int n_arrays, const int64_t* capacity, void* cuda_stream);
+int sph_destroy(sph_ctx* ctx);                                                           /* [sync] */
+
+/* Dest/source tables used by sph_pc_step (Listing 3; L528-534).  Each is an array of n_arrays
+ * bitmasks over source arrays (bit b = array b); NULL keeps the default:
+ *   density (summation mode): every array <- all arrays;
+ *   accel:   dynamic arrays <- all arrays, fixed arrays <- none;
+ *   arho (continuity mode):   dynamic <- all arrays, fixed <- dynamic arrays only. */
+int sph_set_tables(sph_ctx* ctx, const uint32_t* density_src, const uint32_t* accel_src, const uint32_t* arho_src);
+
+/* ---- the four calls of the path --------------------------------------------------------------- */
+
+/* sph_nnps_build(pos, h, domain, periodic) -- Sec.2.2 (L158-170): loads the caller's arrays (positions and
+ * h define the search; u,v,w,m,rho,p are carried along into cell order), computes h_max, sizes the cell
+ * grid (cell >= k*h_max, L158-160), computes cell keys, counting-sorts all arrays into ONE grid (key =
+ * cell * n_arrays + array), builds cell-start offsets and gathers every property into cell order.
+ * Replaces any previous state of the context.  [sync] (reads h_max back to size the grid) */
+int sph_nnps_build(sph_ctx* ctx, int n_arrays, const sph_array* arrays);
+
+/* Summation density, eq.3 (L112): rho_i = sum_{b in source_mask} sum_{j in N_b(i)} m_j W(r_ij, h_ij) for
+ * every particle i of array `dest`, self pair included; then the EOS (eq.6) on that array.  Updates the
+ * context's rho/p of `dest` and, if non-NULL, writes rho_out / p_out (n_dest floats, caller order, `mem`). */
+int sph_summation_density(sph_ctx* ctx, int dest, uint32_t source_mask, float* rho_out, float* p_out, int mem);
+
+/* WCSPH acceleration, eq.8-9 (L128-132) + artificial viscosity + optional continuity RHS eq.7 (L126):
+ *   a_i = g - sum_b sum_j m_j (p_i/rho_i^2 + p_j/rho_j^2 + Pi_ij) grad_i W_ij,   arho_i = sum m_j v_ij . grad_i W_ij
+ * from the context's current rho,p (as loaded by sph_nnps_build or computed by sph_summation_density).
+ * ax,ay,az (az may be NULL when dim == 2) and arho (NULL: not computed) receive n_dest floats, caller order. */
+int sph_wcsph_accel(sph_ctx* ctx, int dest, uint32_t source_mask,
+                    float* ax, float* ay, float* az, float* arho, int mem);
+
+/* n_steps predictor-corrector steps, eqs. 12-14 (L148-152), R10/R11, on the context's state:
+ *   [a^0 = F(x^0,u^0) on the first call after a build]
+ *   u += dt/2 a ; x += dt u (+ periodic wrap, L443) ; NNPS rebuilt (L443) ; [rho = eq.3] ; EOS ; a = F ; u += dt/2 a
+ * density_mode selects eq.3 or the integrated eq.7 (rho stepped like u, on every array).
+ * Fixed arrays keep x,u.  No host synchronisation inside. */
+int sph_pc_step(sph_ctx* ctx, double dt, int n_steps, int density_mode);
+
+/* ---- state out, verification, diagnostics ------------------------------------------------------ */
+
+/* Writes the context's current state of array `array` into the non-NULL pointers of *out
+ * (x,y,z,u,v,w,rho,p; h and m never change) in the caller's original particle order.  out->n must equal
+ * the array's size.  Asynchronous for SPH_MEM_DEVICE; [sync] for SPH_MEM_HOST. */
+int sph_sync_state(sph_ctx* ctx, int array, const sph_array* out);
+
+/* Last accelerations of array `array` (ax,ay,az,arho; any may be NULL), caller order. */
+int sph_get_accel(sph_ctx* ctx, int array, float* ax, float* ay, float* az, float* arho, int mem);
+
+/* Neighbour lists N_src(i) of every particle i of array `dest` as CSR in ORIGINAL indices of array `src`,
+ * each row sorted ascending: offsets[n_dest+1], indices[total].  Pass indices == NULL (or too small a cap)
+ * to get *total only.  Used for the bit-exact set parity.  Host pointers when mem == SPH_MEM_HOST.  [sync] */
+int sph_nnps_get_neighbors(sph_ctx* ctx, int dest, int src, int64_t* offsets, int32_t* indices,
+                           int64_t cap, int64_t* total, int mem);
+
+int sph_get_stats(sph_ctx* ctx, sph_stats* out);                                         /* [sync] */
+int sph_synchronize(sph_ctx* ctx);   /* [sync] waits for the stream and reports pending device-side errors */
+
+const char* sph_strerror(int code);
+const char* sph_last_error(const sph_ctx* ctx);
+int sph_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

@@ -1,0 +1,127 @@
+// WCSPH acceleration, eq.8-9 (L128-132; Listing 4):
+//     a_i = g - sum_j m_j (p_i/rho_i^2 + p_j/rho_j^2 + Pi_ij) grad_i W_ij
+// with Monaghan artificial viscosity Pi_ij (R9; the paper only names "the classic scheme", L185)
+// and, in the same pair loop ("no inter-dependencies and may be computed together", L337), the continuity
+// right-hand side eq.7 (L126; Listing 4):   arho_i = sum_j m_j (v_i - v_j) . grad_i W_ij.
+// Gravity is the initial value of the accumulator (Listing 4).
+#include "sph_pair.cuh"
+
+template <int KERNEL, int DIM, bool VARH, bool PER, bool ARHO>
+struct AccelPolicy : QueuePolicy<AccelPolicy<KERNEL, DIM, VARH, PER, ARHO>> {
+    const float4* posh; const float4* velm; const float2* rp;
+    float4 pi, vi; float rho_i, pr_i;
+    float ax, ay, az, ar;
+    float Lx, Ly, Lz, iLx, iLy, iLz;
+    float sigma, h_c, hinv_c, fac_c, visc, eps;
+
+    __device__ __forceinline__ void body(uint32_t j) {
+        const float4 pj = __ldg(posh + j);
+        const float4 vj = __ldg(velm + j);
+        const float2 rj = __ldg(rp + j);
+        const float dx = min_image<PER>(pi.x - pj.x, Lx, iLx);
+        const float dy = min_image<PER>(pi.y - pj.y, Ly, iLy);
+        float dz = 0.0f;
+        float r2 = fmaf(dy, dy, dx * dx);
+        if (DIM == 3) { dz = min_image<PER>(pi.z - pj.z, Lz, iLz); r2 = fmaf(dz, dz, r2); }
+        const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;       // grad W := 0 at r = 0 (R18): rinv = 0
+        const float r = r2 * rinv;
+        float hij, hinv, fac;
+        if (VARH) {
+            hij = 0.5f * (pi.w + pj.w);
+            hinv = rcp_approx(hij);
+            fac = sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
+        } else { hij = h_c; hinv = hinv_c; fac = fac_c; }
+        float f, df;
+        kernel_profile<KERNEL, DIM>(r * hinv, f, df);
+        const float gc = fac * hinv * df * rinv;                        // grad_i W_ij = gc * (dx,dy,dz)
+        const float vx = vi.x - vj.x, vy = vi.y - vj.y;
+        float vr = fmaf(vy, dy, vx * dx);
+        if (DIM == 3) vr = fmaf(vi.z - vj.z, dz, vr);
+        // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
+        const float den = fmaf(eps * hij, hij, r2) * (rho_i + rj.x);
+        const float Pi = vr < 0.0f ? visc * hij * vr * rcp_approx(den) : 0.0f;
+        const float s = -vj.w * gc * (pr_i + rj.y + Pi);
+        ax = fmaf(s, dx, ax); ay = fmaf(s, dy, ay);
+        if (DIM == 3) az = fmaf(s, dz, az);
+        if (ARHO) ar = fmaf(vj.w * gc, vr, ar);
+    }
+};
+
+// ARHO_ONLY launches serve ContinuityEquation(dest=solid, sources=[fluid]) (Listing 3): the same
+// loop, only arho is stored.
+template <int KERNEL, int DIM, bool VARH, bool MERGED, bool PER, bool ARHO>
+__global__ void __launch_bounds__(PAIR_BLOCK)
+k_accel(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
+        int arho_only, unsigned long long* __restrict__ counters) {
+    extern __shared__ uint32_t smem_q[];
+    const int i = blockIdx.x * PAIR_BLOCK + threadIdx.x;
+    const bool in = i < n;
+    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1), vi = make_float4(0, 0, 0, 0);
+    float2 ri = make_float2(1, 0);
+    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; vi = S.velm[i]; ri = S.rp[i]; }
+    const uint32_t my_mask = in ? pc.src_mask[meta >> SPH_META_IDX_BITS] : 0u;
+    const bool active = my_mask != 0u;
+    if (!__any_sync(SPH_FULL_MASK, active)) return;
+
+    AccelPolicy<KERNEL, DIM, VARH, PER, ARHO> pol;
+    pol.init(smem_q);
+    pol.posh = S.posh; pol.velm = S.velm; pol.rp = S.rp;
+    pol.pi = pi; pol.vi = vi; pol.rho_i = ri.x; pol.pr_i = ri.y;
+    pol.ax = pc.g[0]; pol.ay = pc.g[1]; pol.az = pc.g[2]; pol.ar = 0.0f;
+    pol.Lx = g.L[0]; pol.Ly = g.L[1]; pol.Lz = g.L[2];
+    pol.iLx = 1.0f / g.L[0]; pol.iLy = 1.0f / g.L[1]; pol.iLz = 1.0f / g.L[2];
+    pol.sigma = pc.sigma; pol.h_c = pc.h_const; pol.hinv_c = pc.hinv_const; pol.fac_c = pc.fac_const;
+    pol.visc = pc.visc; pol.eps = pc.eps;
+
+    walk_candidates<DIM, VARH, MERGED>(g, pc, S.posh, cell_start, active, pi, ci, my_mask, pol);
+    pol.flush();
+
+    if (active) {
+        float4 a = S.acc[i];
+        if (arho_only) a.w = pol.ar;
+        else a = make_float4(pol.ax, pol.ay, DIM == 3 ? pol.az : 0.0f, ARHO ? pol.ar : a.w);
+        S.acc[i] = a;
+        if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
+    }
+    const unsigned long long h = warp_sum_u64(pol.hits), t = warp_sum_u64(pol.tests);
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); atomicAdd(&counters[CNT_CANDIDATES], t); }
+}
+
+template <int KERNEL, int DIM>
+static int launch_accel_kd(sph_ctx* c, bool merged, bool want_arho, bool arho_only) {
+    const int n = (int)c->n_total;
+    if (n == 0) return SPH_OK;
+    const int grid = (n + PAIR_BLOCK - 1) / PAIR_BLOCK;
+    const size_t smem = (size_t)PAIR_QCAP * PAIR_BLOCK * sizeof(uint32_t);
+    const bool per = c->grid.per[0] || c->grid.per[1] || c->grid.per[2];
+    const bool varh = c->variable_h;
+    SortedState& S = c->S[c->cur];
+    const int ao = arho_only ? 1 : 0;
+#define LA(VARH, MERGED, PER, ARHO) do { \
+        auto kern = k_accel<KERNEL, DIM, VARH, MERGED, PER, ARHO>; \
+        SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        SPH_LAUNCH(c, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, ao, c->counters); } while (0)
+#define LA2(VARH, MERGED, PER) do { if (want_arho) LA(VARH, MERGED, PER, true); else LA(VARH, MERGED, PER, false); } while (0)
+#define LA3(VARH, MERGED) do { if (per) LA2(VARH, MERGED, true); else LA2(VARH, MERGED, false); } while (0)
+    if (varh) { if (merged) LA3(true, true); else LA3(true, false); }
+    else      { if (merged) LA3(false, true); else LA3(false, false); }
+#undef LA3
+#undef LA2
+#undef LA
+    return SPH_OK;
+}
+
+int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, bool arho_only) {
+    bool merged = true;
+    for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
+        c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
+        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) merged = false;
+    }
+    const int k = c->prm.kernel, d = c->grid.dim;
+#define KD(K, D) if (k == K && d == D) return launch_accel_kd<K, D>(c, merged, want_arho || arho_only, arho_only)
+    KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
+    KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
+    KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);
+#undef KD
+    return sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
+}

@@ -1,0 +1,385 @@
+// C ABI of libsph_b200.so (include/sph.h): argument checking, workspace, and the order of kernels.
+// Every step of the path runs in the kernels of sph_nnps.cu / sph_density.cu / sph_accel.cu; this file only
+// marshals arguments and enqueues launches.  There is no CPU fallback.
+#include "sph_ctx.cuh"
+#include <math.h>
+#include <string.h>
+#include <new>
+
+static const int N_STAGE_FIELDS = 10;
+
+
+extern "C" const char* sph_strerror(int code) {
+    switch (code) {
+        case SPH_OK: return "ok";
+        case SPH_ERR_NULL: return "null pointer";
+        case SPH_ERR_BAD_ARG: return "bad argument";
+        case SPH_ERR_CAPACITY: return "capacity exceeded";
+        case SPH_ERR_STALE_NNPS: return "no neighbour structure: call sph_nnps_build first";
+        case SPH_ERR_OUT_OF_DOMAIN: return "particles outside a non-periodic domain";
+        case SPH_ERR_NONFINITE: return "non-finite value produced";
+        case SPH_ERR_CUDA: return "CUDA error";
+    }
+    return "unknown error";
+}
+extern "C" const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context"; }
+extern "C" int sph_abi_version(void) { return SPH_ABI_VERSION; }
+
+static void default_tables(sph_ctx* c) {
+    uint32_t all = (1u << c->na) - 1u, dyn = 0;
+    for (int a = 0; a < c->na; ++a) if (!c->fixed[a]) dyn |= 1u << a;
+    for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
+        const bool live = a < c->na;
+        c->tbl_density[a] = live ? all : 0u;
+        c->tbl_accel[a] = (live && !c->fixed[a]) ? all : 0u;
+        c->tbl_arho[a] = live ? (c->fixed[a] ? dyn : all) : 0u;     // Listing 3
+    }
+}
+
+static void set_consts(sph_ctx* c) {
+    const sph_params& P = c->prm;
+    PairConsts& pc = c->pc;
+    memset(&pc, 0, sizeof(pc));
+    pc.kh = (float)(0.5 * kernel_support(P.kernel));
+    pc.sigma = (float)kernel_sigma(P.kernel, c->dom.dim);
+    pc.rho0 = (float)P.rho0;
+    pc.B = (float)(P.rho0 * P.c0 * P.c0 / P.gamma);
+    pc.gamma = (float)P.gamma;
+    pc.gamma_is_7 = (P.gamma == 7.0);
+    pc.visc = (float)(-2.0 * P.alpha * P.c0);
+    pc.eps = (float)P.eps;
+    for (int k = 0; k < 3; ++k) pc.g[k] = (float)P.g[k];
+    pc.all_mask = (1u << c->na) - 1u;
+    pc.h_const = 1.0f; pc.hinv_const = 1.0f; pc.fac_const = 1.0f;
+}
+
+extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_domain* domain,
+                          int n_arrays, const int64_t* capacity, void* cuda_stream) {
+    if (!out || !params || !domain || !capacity) return SPH_ERR_NULL;
+    *out = nullptr;
+    if (n_arrays < 1 || n_arrays > SPH_MAX_ARRAYS) return SPH_ERR_BAD_ARG;
+    if (domain->dim != 2 && domain->dim != 3) return SPH_ERR_BAD_ARG;
+    if (params->kernel < 0 || params->kernel > SPH_KERNEL_WENDLAND_C2) return SPH_ERR_BAD_ARG;
+    if (!(params->rho0 > 0) || !(params->c0 > 0) || !(params->gamma > 0)) return SPH_ERR_BAD_ARG;
+    for (int k = 0; k < domain->dim; ++k) if (!(domain->hi[k] > domain->lo[k])) return SPH_ERR_BAD_ARG;
+    int64_t tot = 0;
+    for (int a = 0; a < n_arrays; ++a) {
+        if (capacity[a] < 0 || capacity[a] > (int64_t)SPH_META_IDX_MASK) return SPH_ERR_BAD_ARG;
+        tot += capacity[a];
+    }
+    if (tot > (int64_t)0x7fffff00) return SPH_ERR_BAD_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return SPH_ERR_CUDA;   // no CPU fallback
+
+    sph_ctx* c = new (std::nothrow) sph_ctx;
+    if (!c) return SPH_ERR_CUDA;
+    memset(c, 0, sizeof(*c));
+    c->stream = (cudaStream_t)cuda_stream;
+    c->prm = *params; c->dom = *domain; c->na = n_arrays;
+    if (domain->dim == 2) { c->dom.lo[2] = 0; c->dom.hi[2] = 1; c->dom.periodic[2] = 0; }
+    for (int a = 0; a < n_arrays; ++a) c->cap[a] = capacity[a];
+    c->cap_total = tot;
+    default_tables(c);
+    set_consts(c);
+    *out = c;                                  // so the caller can read sph_last_error / destroy on failure
+    SPH_CUDA_OK(c, cudaGetDevice(&c->device));
+    SPH_CUDA_OK(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
+
+    const size_t N = (size_t)tot + 1;
+    c->max_keys = 4 * tot + 65536; if (c->max_keys > ((int64_t)1 << 26)) c->max_keys = (int64_t)1 << 26;
+    for (int b = 0; b < 2; ++b) {
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].posh, N * sizeof(float4)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].velm, N * sizeof(float4)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].rp, N * sizeof(float2)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].meta, N * sizeof(uint32_t)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].cell, N * sizeof(uint32_t)));
+    }
+    SPH_CUDA_OK(c, cudaMalloc(&c->S[0].acc, N * sizeof(float4)));
+    c->S[1].acc = c->S[0].acc;
+    SPH_CUDA_OK(c, cudaMalloc(&c->key, (N + 1) * sizeof(uint32_t)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->rank, (N + 1) * sizeof(uint32_t)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->cell_count, (size_t)(c->max_keys + 2) * sizeof(uint32_t)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->cell_start, (size_t)(c->max_keys + 2) * sizeof(uint32_t)));
+    const size_t scan_n = (size_t)(c->max_keys > tot ? c->max_keys : tot) + 2;
+    SPH_CUDA_OK(c, cudaMalloc(&c->block_sums, (scan_n / 2048 + 4) * sizeof(uint32_t)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(float)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->counters, CNT_COUNT * sizeof(unsigned long long)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 2 * sizeof(float)));
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->S[0].acc, 0, N * sizeof(float4), c->stream));
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+extern "C" int sph_destroy(sph_ctx* c) {
+    if (!c) return SPH_ERR_NULL;
+    cudaStreamSynchronize(c->stream);
+    for (int b = 0; b < 2; ++b) {
+        cudaFree(c->S[b].posh); cudaFree(c->S[b].velm); cudaFree(c->S[b].rp); cudaFree(c->S[b].meta); cudaFree(c->S[b].cell);
+    }
+    cudaFree(c->S[0].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
+    cudaFree(c->block_sums); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
+    delete c;
+    return SPH_OK;
+}
+
+extern "C" int sph_set_tables(sph_ctx* c, const uint32_t* density_src, const uint32_t* accel_src, const uint32_t* arho_src) {
+    if (!c) return SPH_ERR_NULL;
+    const uint32_t all = (1u << c->na) - 1u;
+    const uint32_t* in[3] = { density_src, accel_src, arho_src };
+    uint32_t* dst[3] = { c->tbl_density, c->tbl_accel, c->tbl_arho };
+    for (int t = 0; t < 3; ++t) if (in[t]) for (int a = 0; a < c->na; ++a) if (in[t][a] & ~all) return sph_fail(c, SPH_ERR_BAD_ARG, "source mask names a non-existent array");
+    for (int t = 0; t < 3; ++t) if (in[t]) for (int a = 0; a < c->na; ++a) dst[t][a] = in[t][a];
+    c->tables_user = true;
+    return SPH_OK;
+}
+
+// cell >= k*h_max (L158-160) with a margin that absorbs the float rounding of the cell coordinate.
+static int size_grid(sph_ctx* c) {
+    GridDesc& g = c->grid;
+    memset(&g, 0, sizeof(g));
+    g.dim = c->dom.dim; g.na = c->na;
+    const double cutoff = kernel_support(c->prm.kernel) * (double)c->h_max;
+    if (!(cutoff > 0.0)) return sph_fail(c, SPH_ERR_BAD_ARG, "h_max must be positive");
+    double scale = 1.0;
+    for (int iter = 0; iter < 64; ++iter) {
+        int64_t total = 1; bool ok = true;
+        for (int k = 0; k < 3; ++k) {
+            g.per[k] = (k < g.dim) ? (c->dom.periodic[k] != 0) : 0;
+            const double L = (k < g.dim) ? c->dom.hi[k] - c->dom.lo[k] : 1.0;
+            int n = 1;
+            if (k < g.dim) {
+                double est = L / (cutoff * scale);
+                double margin = 1.0e-3 + 4.0e-7 * est;
+                double nd = floor(L / (cutoff * scale * (1.0 + margin)));
+                if (nd > 1.0e6) nd = 1.0e6;
+                n = nd < 1.0 ? 1 : (int)nd;
+                if (g.per[k] && n < 3) {
+                    if (scale > 1.0) ok = false;      // cannot coarsen further
+                    else return sph_fail(c, SPH_ERR_BAD_ARG, "a periodic axis needs at least 3 cells of size k*h_max");
+                }
+            }
+            g.nc[k] = n;
+            g.lo[k] = (float)c->dom.lo[k]; g.hi[k] = (float)c->dom.hi[k];
+            g.L[k] = (float)(c->dom.hi[k] - c->dom.lo[k]);
+            g.inv_cell[k] = (float)(n / L);
+            total *= n;
+        }
+        if (!ok) return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
+        if (total * c->na <= c->max_keys) { c->n_keys = total * c->na; return SPH_OK; }
+        scale *= 1.26;
+    }
+    return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
+}
+
+static float* stage_field(sph_ctx* c, int field, int array) { return c->staging + ((size_t)field * (c->cap_total + 1) + c->base[array]); }
+
+extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays) {
+    if (!c || !arrays) return SPH_ERR_NULL;
+    if (n_arrays != c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "n_arrays differs from sph_create");
+    c->built = false; c->have_accel = false;
+    int64_t tot = 0;
+    for (int a = 0; a < c->na; ++a) {
+        const sph_array& A = arrays[a];
+        if (A.n < 0) return sph_fail(c, SPH_ERR_BAD_ARG, "negative n");
+        if (A.n > c->cap[a]) return sph_fail(c, SPH_ERR_CAPACITY, "array larger than its capacity");
+        if (A.n > 0 && (!A.x || !A.y || !A.h || (c->dom.dim == 3 && !A.z))) return sph_fail(c, SPH_ERR_NULL, "x, y, (z), h are required");
+        if (A.mem != SPH_MEM_DEVICE && A.mem != SPH_MEM_HOST) return sph_fail(c, SPH_ERR_BAD_ARG, "bad mem");
+        c->n[a] = A.n; c->base[a] = tot; c->fixed[a] = (A.flags & SPH_ARRAY_FIXED) ? 1 : 0;
+        tot += A.n;
+    }
+    c->base[c->na] = tot; c->n_total = tot;
+    if (!c->tables_user) default_tables(c);
+
+    PackArgs P; memset(&P, 0, sizeof(P));
+    P.na = c->na;
+    for (int a = 0; a <= c->na; ++a) P.base[a] = c->base[a];
+    for (int a = 0; a < c->na; ++a) {
+        const sph_array& A = arrays[a];
+        const float* src[N_STAGE_FIELDS] = { A.x, A.y, A.z, A.u, A.v, A.w, A.h, A.m, A.rho, A.p };
+        const float* use[N_STAGE_FIELDS];
+        for (int f = 0; f < N_STAGE_FIELDS; ++f) {
+            use[f] = src[f];
+            if (A.mem == SPH_MEM_HOST && src[f] && A.n > 0) {
+                float* d = stage_field(c, f, a);
+                SPH_CUDA_OK(c, cudaMemcpyAsync(d, src[f], (size_t)A.n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+                use[f] = d;
+            }
+        }
+        P.a[a] = PackSrc{ use[0], use[1], use[2], use[3], use[4], use[5], use[6], use[7], use[8], use[9] };
+    }
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
+    c->cur = 0;
+    int rc = nnps_pack(c, P); if (rc) return rc;
+    int hmm[2] = { 0, 0 };
+    SPH_CUDA_OK(c, cudaMemcpyAsync(hmm, c->hminmax, sizeof(hmm), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    if (tot == 0) { c->h_min = c->h_max = 1.0f; }
+    else { memcpy(&c->h_min, &hmm[0], 4); memcpy(&c->h_max, &hmm[1], 4); }
+    if (!(c->h_max > 0.0f) || !isfinite(c->h_max)) return sph_fail(c, SPH_ERR_BAD_ARG, "smoothing lengths must be positive and finite");
+    c->variable_h = (c->h_min != c->h_max);
+    c->pc.h_const = c->h_max;
+    c->pc.hinv_const = (float)(1.0 / (double)c->h_max);
+    c->pc.fac_const = (float)(kernel_sigma(c->prm.kernel, c->dom.dim) / pow((double)c->h_max, c->dom.dim));
+    rc = size_grid(c); if (rc) return rc;
+    rc = nnps_key_hist(c); if (rc) return rc;
+    rc = nnps_sort_from_keys(c); if (rc) return rc;
+    c->built = true; c->steps_done = 0;
+    return SPH_OK;
+}
+
+// caller-order output of up to 12 fields of one array, to device pointers or through the staging buffer to host
+static int emit(sph_ctx* c, int array, OutPtrs O, int mem) {
+    float** f = (float**)&O;
+    const int NF = sizeof(OutPtrs) / sizeof(float*);
+    const size_t n = (size_t)c->n[array];
+    if (mem == SPH_MEM_DEVICE) return nnps_gather_out(c, array, O);
+    float* host[NF]; int used = 0;
+    for (int k = 0; k < NF; ++k) { host[k] = f[k]; if (f[k]) { if (used >= N_STAGE_FIELDS) return sph_fail(c, SPH_ERR_BAD_ARG, "too many host outputs in one call"); f[k] = c->staging + (size_t)used * (c->cap_total + 1); ++used; } }
+    int rc = nnps_gather_out(c, array, O); if (rc) return rc;
+    for (int k = 0; k < NF; ++k) if (host[k] && n) SPH_CUDA_OK(c, cudaMemcpyAsync(host[k], f[k], n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+static int zero_counter(sph_ctx* c, int which) {
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->counters + which, 0, sizeof(unsigned long long), c->stream));
+    return SPH_OK;
+}
+
+extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask, float* rho_out, float* p_out, int mem) {
+    if (!c) return SPH_ERR_NULL;
+    if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
+    if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
+    uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
+    masks[dest] = source_mask;
+    int rc = zero_counter(c, CNT_PAIRS_DENSITY); if (rc) return rc;
+    rc = zero_counter(c, CNT_CANDIDATES); if (rc) return rc;
+    rc = launch_density(c, masks); if (rc) return rc;
+    if (rho_out || p_out) { OutPtrs O; memset(&O, 0, sizeof(O)); O.rho = rho_out; O.p = p_out; return emit(c, dest, O, mem); }
+    return SPH_OK;
+}
+
+extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float* ax, float* ay, float* az, float* arho, int mem) {
+    if (!c) return SPH_ERR_NULL;
+    if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
+    if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
+    uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
+    masks[dest] = source_mask;
+    int rc = zero_counter(c, CNT_PAIRS_ACCEL); if (rc) return rc;
+    rc = zero_counter(c, CNT_CANDIDATES); if (rc) return rc;
+    rc = launch_accel(c, masks, arho != nullptr, false); if (rc) return rc;
+    if (ax || ay || az || arho) { OutPtrs O; memset(&O, 0, sizeof(O)); O.ax = ax; O.ay = ay; O.az = az; O.arho = arho; return emit(c, dest, O, mem); }
+    return SPH_OK;
+}
+
+// One evaluation F(x,u,rho) in group order (Listing 3): [density ->] EOS on all arrays | barrier |
+// continuity + momentum.  Destinations that share a source mask share a launch.
+static int evaluate(sph_ctx* c, bool continuity) {
+    int rc;
+    rc = zero_counter(c, CNT_PAIRS_DENSITY); if (rc) return rc;
+    rc = zero_counter(c, CNT_PAIRS_ACCEL); if (rc) return rc;
+    rc = zero_counter(c, CNT_CANDIDATES); if (rc) return rc;
+    auto grouped = [&](const uint32_t* tbl, const bool* take, auto&& fn) -> int {
+        bool done[SPH_MAX_ARRAYS] = { false, false, false, false };
+        for (int a = 0; a < c->na; ++a) {
+            if (done[a] || !take[a] || !tbl[a]) continue;
+            uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
+            for (int b = a; b < c->na; ++b) if (!done[b] && take[b] && tbl[b] == tbl[a]) { masks[b] = tbl[b]; done[b] = true; }
+            int r = fn(masks); if (r) return r;
+        }
+        return SPH_OK;
+    };
+    bool all[SPH_MAX_ARRAYS] = { true, true, true, true };
+    if (!continuity) { rc = grouped(c->tbl_density, all, [&](const uint32_t* m) { return launch_density(c, m); }); if (rc) return rc; }
+    bool fused[SPH_MAX_ARRAYS], plain[SPH_MAX_ARRAYS], only[SPH_MAX_ARRAYS];
+    for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
+        const bool acc = a < c->na && c->tbl_accel[a] != 0;
+        const bool same = acc && continuity && c->tbl_arho[a] == c->tbl_accel[a];
+        fused[a] = same; plain[a] = acc && !same;
+        only[a] = a < c->na && continuity && c->tbl_arho[a] != 0 && !same;
+    }
+    rc = grouped(c->tbl_accel, fused, [&](const uint32_t* m) { return launch_accel(c, m, true, false); }); if (rc) return rc;
+    rc = grouped(c->tbl_accel, plain, [&](const uint32_t* m) { return launch_accel(c, m, false, false); }); if (rc) return rc;
+    rc = grouped(c->tbl_arho, only, [&](const uint32_t* m) { return launch_accel(c, m, true, true); }); if (rc) return rc;
+    return SPH_OK;
+}
+
+extern "C" int sph_pc_step(sph_ctx* c, double dt, int n_steps, int density_mode) {
+    if (!c) return SPH_ERR_NULL;
+    if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
+    if (n_steps < 0 || (density_mode != SPH_DENSITY_SUMMATION && density_mode != SPH_DENSITY_CONTINUITY) || !isfinite(dt))
+        return sph_fail(c, SPH_ERR_BAD_ARG, "bad n_steps / density_mode / dt");
+    const bool cont = density_mode == SPH_DENSITY_CONTINUITY;
+    int rc;
+    if (!c->have_accel) { rc = evaluate(c, cont); if (rc) return rc; c->have_accel = true; }   // a^0 = F(x^0, u^0)
+    for (int s = 0; s < n_steps; ++s) {
+        rc = nnps_update_key_hist(c, (float)dt, s > 0, true, cont, true); if (rc) return rc;    // (14 of step s-1) + 12 + 13 + key
+        rc = nnps_sort_from_keys(c); if (rc) return rc;                                         // NNPS rebuilt every step (L443)
+        rc = evaluate(c, cont); if (rc) return rc;
+        c->steps_done++;
+    }
+    if (n_steps > 0) { rc = nnps_update_key_hist(c, (float)dt, true, false, cont, false); if (rc) return rc; }   // eq.14
+    return SPH_OK;
+}
+
+extern "C" int sph_sync_state(sph_ctx* c, int array, const sph_array* out) {
+    if (!c || !out) return SPH_ERR_NULL;
+    if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
+    if (array < 0 || array >= c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "bad array");
+    if (out->n != c->n[array]) return sph_fail(c, SPH_ERR_CAPACITY, "out->n differs from the array size");
+    OutPtrs O; memset(&O, 0, sizeof(O));
+    O.x = out->x; O.y = out->y; O.z = out->z; O.u = out->u; O.v = out->v; O.w = out->w; O.rho = out->rho; O.p = out->p;
+    return emit(c, array, O, out->mem);
+}
+
+extern "C" int sph_get_accel(sph_ctx* c, int array, float* ax, float* ay, float* az, float* arho, int mem) {
+    if (!c) return SPH_ERR_NULL;
+    if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
+    if (array < 0 || array >= c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "bad array");
+    OutPtrs O; memset(&O, 0, sizeof(O)); O.ax = ax; O.ay = ay; O.az = az; O.arho = arho;
+    return emit(c, array, O, mem);
+}
+
+extern "C" int sph_nnps_get_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32_t* indices,
+                                      int64_t cap, int64_t* total, int mem) {
+    if (!c || !offsets || !total) return SPH_ERR_NULL;
+    if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
+    if (dest < 0 || dest >= c->na || src < 0 || src >= c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / src");
+    return nnps_export_neighbors(c, dest, src, offsets, indices, cap, total, mem);
+}
+
+static int read_counters(sph_ctx* c, unsigned long long* h) {
+    SPH_CUDA_OK(c, cudaMemcpyAsync(h, c->counters, CNT_COUNT * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+extern "C" int sph_synchronize(sph_ctx* c) {
+    if (!c) return SPH_ERR_NULL;
+    unsigned long long h[CNT_COUNT];
+    int rc = read_counters(c, h); if (rc) return rc;
+    if (h[CNT_OUT_OF_DOMAIN]) { snprintf(c->err, sizeof(c->err), "%llu particle updates fell outside the non-periodic domain box", h[CNT_OUT_OF_DOMAIN]); return SPH_ERR_OUT_OF_DOMAIN; }
+    if (h[CNT_NONFINITE]) { snprintf(c->err, sizeof(c->err), "%llu non-finite results", h[CNT_NONFINITE]); return SPH_ERR_NONFINITE; }
+    return SPH_OK;
+}
+
+extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
+    if (!c || !out) return SPH_ERR_NULL;
+    unsigned long long h[CNT_COUNT];
+    int rc = read_counters(c, h); if (rc) return rc;
+    memset(out, 0, sizeof(*out));
+    for (int k = 0; k < 3; ++k) {
+        out->n_cells[k] = c->grid.nc[k];
+        out->cell_size[k] = c->grid.nc[k] ? (c->dom.hi[k] - c->dom.lo[k]) / c->grid.nc[k] : 0.0;
+    }
+    out->n_particles = c->n_total;
+    out->pairs_density = (int64_t)h[CNT_PAIRS_DENSITY];
+    out->pairs_accel = (int64_t)h[CNT_PAIRS_ACCEL];
+    out->candidates = (int64_t)h[CNT_CANDIDATES];
+    out->kernel_launches = c->launches;
+    out->steps_done = c->steps_done;
+    out->variable_h = c->variable_h ? 1 : 0;
+    out->h_max = c->h_max;
+    return SPH_OK;
+}

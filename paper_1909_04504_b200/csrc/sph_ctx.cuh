@@ -1,0 +1,71 @@
+// The opaque context behind sph_ctx* (library-owned; see include/sph.h "ownership").
+#pragma once
+#include "sph_internal.cuh"
+#include <stdio.h>
+
+enum { CNT_OUT_OF_DOMAIN = 0, CNT_NONFINITE = 1, CNT_PAIRS_DENSITY = 2, CNT_PAIRS_ACCEL = 3,
+       CNT_CANDIDATES = 4, CNT_OVERFLOW = 5, CNT_COUNT = 8 };
+
+struct sph_ctx {
+    cudaStream_t stream;
+    int device, sm_count;
+    sph_params prm;
+    sph_domain dom;
+    int na;
+    int64_t cap[SPH_MAX_ARRAYS], cap_total;
+    int64_t n[SPH_MAX_ARRAYS], base[SPH_MAX_ARRAYS + 1], n_total;   // base = offsets in concatenated caller order
+    int fixed[SPH_MAX_ARRAYS];
+    uint32_t tbl_density[SPH_MAX_ARRAYS], tbl_accel[SPH_MAX_ARRAYS], tbl_arho[SPH_MAX_ARRAYS];
+    bool tables_user;
+
+    GridDesc grid;
+    PairConsts pc;
+    bool built, have_accel, variable_h;
+    float h_min, h_max;
+    int64_t n_keys, max_keys;
+
+    SortedState S[2];          // posh, velm, rp, meta, cell are double-buffered (permute A -> B); acc is shared
+    int cur;
+    uint32_t *key, *rank;      // per particle, pre-sort order
+    uint32_t *cell_count, *cell_start, *block_sums;
+    float* staging;            // host<->device staging for SPH_MEM_HOST (10 floats per particle of capacity)
+    float* out_tmp;            // device scratch for caller-order outputs (4 floats per particle of capacity)
+    unsigned long long* counters;     // device, CNT_COUNT entries
+    float* hminmax;            // device, 2 floats (as ordered ints)
+
+    int64_t launches, steps_done;
+    int64_t last_pairs_density, last_pairs_accel;
+    char err[512];
+};
+
+#define SPH_CUDA_OK(ctx, expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { \
+    snprintf((ctx)->err, sizeof((ctx)->err), "%s: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    return SPH_ERR_CUDA; } } while (0)
+
+static inline int sph_fail(sph_ctx* c, int code, const char* msg) {
+    if (c) snprintf(c->err, sizeof(c->err), "%s", msg);
+    return code;
+}
+
+// launch accounting: every kernel of the library goes through this macro
+#define SPH_LAUNCH(ctx, kernel, grid, block, smem, ...) do { \
+    kernel<<<(grid), (block), (smem), (ctx)->stream>>>(__VA_ARGS__); (ctx)->launches++; \
+    cudaError_t e__ = cudaPeekAtLastError(); if (e__ != cudaSuccess) { \
+        snprintf((ctx)->err, sizeof((ctx)->err), "launch %s: %s", #kernel, cudaGetErrorString(e__)); \
+        return SPH_ERR_CUDA; } } while (0)
+
+struct PackSrc { const float *x, *y, *z, *u, *v, *w, *h, *m, *rho, *p; };
+struct PackArgs { PackSrc a[SPH_MAX_ARRAYS]; long long base[SPH_MAX_ARRAYS + 1]; int na; };
+struct OutPtrs { float *x, *y, *z, *u, *v, *w, *rho, *p, *ax, *ay, *az, *arho; };
+
+// sph_nnps.cu
+int nnps_pack(sph_ctx* c, const PackArgs& A);        // caller SoA -> float4 groups (unsorted) + h_min/h_max
+int nnps_key_hist(sph_ctx* c);                       // key + rank + histogram from S[cur]
+int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey);
+int nnps_sort_from_keys(sph_ctx* c);                 // scan + scatter (key/rank/cell_count filled); swaps buffers
+int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O);
+int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32_t* indices, int64_t cap,
+                          int64_t* total, int mem);
+// sph_density.cu / sph_accel.cu: one launch serves every dest array whose mask is non-zero
+int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest);
+int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, bool arho_only);

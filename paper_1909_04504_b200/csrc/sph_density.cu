@@ -1,0 +1,100 @@
+// Summation density, eq.3 (L112): rho_i = sum_j m_j W(x_i - x_j, h_ij), with the Tait EOS
+// (eq.6, Listing 4) fused as the epilogue (the group barrier of L337/L382 is the kernel
+// boundary: every p is stored before the acceleration kernel starts).
+#include "sph_pair.cuh"
+
+template <int KERNEL, int DIM, bool VARH, bool PER>
+struct DensityPolicy : QueuePolicy<DensityPolicy<KERNEL, DIM, VARH, PER>> {
+    const float4* posh; const float4* velm;
+    float4 pi; float rho;
+    float Lx, Ly, Lz, iLx, iLy, iLz;
+    float sigma, hinv_c, fac_c;
+
+    __device__ __forceinline__ void body(uint32_t j) {
+        const float4 pj = __ldg(posh + j);
+        const float mj = __ldg(&velm[j].w);
+        const float dx = min_image<PER>(pi.x - pj.x, Lx, iLx);
+        const float dy = min_image<PER>(pi.y - pj.y, Ly, iLy);
+        float r2 = fmaf(dy, dy, dx * dx);
+        if (DIM == 3) { const float dz = min_image<PER>(pi.z - pj.z, Lz, iLz); r2 = fmaf(dz, dz, r2); }
+        const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;
+        const float r = r2 * rinv;
+        float hinv, fac;
+        if (VARH) {
+            hinv = rcp_approx(0.5f * (pi.w + pj.w));
+            fac = sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
+        } else { hinv = hinv_c; fac = fac_c; }
+        float f, df;
+        kernel_profile<KERNEL, DIM>(r * hinv, f, df);
+        rho = fmaf(mj * fac, f, rho);
+    }
+};
+
+template <int KERNEL, int DIM, bool VARH, bool MERGED, bool PER>
+__global__ void __launch_bounds__(PAIR_BLOCK)
+k_density(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
+          unsigned long long* __restrict__ counters) {
+    extern __shared__ uint32_t smem_q[];
+    const int i = blockIdx.x * PAIR_BLOCK + threadIdx.x;
+    const bool in = i < n;
+    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
+    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; }
+    const uint32_t my_mask = in ? pc.src_mask[meta >> SPH_META_IDX_BITS] : 0u;
+    const bool active = my_mask != 0u;
+    if (!__any_sync(SPH_FULL_MASK, active)) return;
+
+    DensityPolicy<KERNEL, DIM, VARH, PER> pol;
+    pol.init(smem_q);
+    pol.posh = S.posh; pol.velm = S.velm; pol.pi = pi; pol.rho = 0.0f;
+    pol.Lx = g.L[0]; pol.Ly = g.L[1]; pol.Lz = g.L[2];
+    pol.iLx = 1.0f / g.L[0]; pol.iLy = 1.0f / g.L[1]; pol.iLz = 1.0f / g.L[2];
+    pol.sigma = pc.sigma; pol.hinv_c = pc.hinv_const; pol.fac_c = pc.fac_const;
+
+    walk_candidates<DIM, VARH, MERGED>(g, pc, S.posh, cell_start, active, pi, ci, my_mask, pol);
+    pol.flush();
+
+    if (active) {
+        const float rho = pol.rho;
+        const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
+        S.rp[i] = make_float2(rho, p / (rho * rho));
+        if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
+    }
+    const unsigned long long h = warp_sum_u64(pol.hits), t = warp_sum_u64(pol.tests);
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CANDIDATES], t); }
+}
+
+template <int KERNEL, int DIM>
+static int launch_density_kd(sph_ctx* c, bool merged) {
+    const int n = (int)c->n_total;
+    if (n == 0) return SPH_OK;
+    const int grid = (n + PAIR_BLOCK - 1) / PAIR_BLOCK;
+    const size_t smem = (size_t)PAIR_QCAP * PAIR_BLOCK * sizeof(uint32_t);
+    const bool per = c->grid.per[0] || c->grid.per[1] || c->grid.per[2];
+    SortedState& S = c->S[c->cur];
+#define LD(VARH, MERGED, PER) do { \
+        auto kern = k_density<KERNEL, DIM, VARH, MERGED, PER>; \
+        SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        SPH_LAUNCH(c, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, c->counters); } while (0)
+    if (c->variable_h) { if (merged) { if (per) LD(true, true, true); else LD(true, true, false); }
+                         else        { if (per) LD(true, false, true); else LD(true, false, false); } }
+    else               { if (merged) { if (per) LD(false, true, true); else LD(false, true, false); }
+                         else        { if (per) LD(false, false, true); else LD(false, false, false); } }
+#undef LD
+    return SPH_OK;
+}
+
+// One launch computes rho,p for every array whose src_mask_per_dest entry is non-zero.
+int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest) {
+    bool merged = true;
+    for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
+        c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
+        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) merged = false;
+    }
+    const int k = c->prm.kernel, d = c->grid.dim;
+#define KD(K, D) if (k == K && d == D) return launch_density_kd<K, D>(c, merged)
+    KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
+    KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
+    KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);
+#undef KD
+    return sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
+}

@@ -1,0 +1,117 @@
+// Internal declarations of the CUDA path (sm_100a).  Not part of the ABI; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sph.h"
+
+#define SPH_FULL_MASK 0xffffffffu
+#define SPH_META_IDX_BITS 28u                    // meta = (array id << 28) | original index
+#define SPH_META_IDX_MASK ((1u << SPH_META_IDX_BITS) - 1u)
+
+// Uniform cell grid (cells of size >= the support radius; 3^d neighbouring boxes).
+struct GridDesc {
+    int dim;
+    int nc[3];                 // cells per axis (nc[2] = 1 in 2-D)
+    int per[3];                // periodic per axis
+    int na;                    // particle arrays merged into the grid: key = cell * na + array
+    float lo[3];               // domain origin
+    float inv_cell[3];         // 1 / cell size
+    float L[3];                // (float)(hi - lo): the period used by the neighbour predicate (R7)
+    float hi[3];
+};
+
+// Per-launch constants of the pair loops.
+struct PairConsts {
+    float kh;                  // k/2: cut = kh * (h_i + h_j)
+    float sigma;               // kernel normalisation sigma_d
+    float h_const;             // constant-h fast path: h, 1/h, sigma/h^d
+    float hinv_const;
+    float fac_const;
+    float rho0, B, gamma;      // Tait EOS
+    int   gamma_is_7;
+    float visc;                // -2 alpha c0   (Pi = visc * h vr / ((r2 + eps h^2)(rho_i + rho_j)))
+    float eps;
+    float g[3];
+    uint32_t src_mask[SPH_MAX_ARRAYS];   // per DEST array: source-array bitmask; 0 = not a destination of this launch
+    uint32_t all_mask;         // (1 << na) - 1
+};
+
+// Cell-sorted particle state (struct of float4 groups: one 16-B vector load per candidate test).
+struct SortedState {
+    float4* posh;              // x, y, z, h
+    float4* velm;              // u, v, w, m
+    float2* rp;                // rho, p / rho^2   (p itself is returned as (p/rho^2) * rho^2)
+    float4* acc;               // ax, ay, az, arho
+    uint32_t* meta;            // (array << 28) | original index
+    uint32_t* cell;            // linear cell id of the particle (x fastest)
+};
+
+// ---- device math ------------------------------------------------------------------------------
+__device__ __forceinline__ float rcp_approx(float x)  { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_approx(float x){ float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// Neighbour predicate, R7 (bit-specified):
+//   d_a = fl(x_i - x_j) - shift_a   (shift_a in {-L_a, 0, +L_a}: the minimum image; exact when 0)
+//   r2  = fma(dz, dz, fma(dy, dy, fl(dx*dx)));   cut = fl(kh * fl(h_i + h_j));   hit <=> r2 < fl(cut*cut)
+__device__ __forceinline__ float pair_r2(float dx, float dy, float dz) {
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+}
+__device__ __forceinline__ float pair_cut2(float kh, float hi, float hj) {
+    float cut = __fmul_rn(kh, __fadd_rn(hi, hj));
+    return __fmul_rn(cut, cut);
+}
+
+// Dimensionless kernel profile f(q) and f'(q); W = sigma h^-d f, dW/dr = sigma h^-(d+1) f'.
+template <int KERNEL, int DIM>
+__device__ __forceinline__ void kernel_profile(float q, float& f, float& df) {
+    if (KERNEL == SPH_KERNEL_CUBIC) {
+        float t = 2.0f - q;
+        float inner_f  = fmaf(q * q, fmaf(0.75f, q, -1.5f), 1.0f);    // 1 - 1.5 q^2 + 0.75 q^3
+        float inner_df = q * fmaf(2.25f, q, -3.0f);                     // -3 q + 2.25 q^2
+        float outer_f  = 0.25f * t * t * t;
+        float outer_df = -0.75f * t * t;
+        bool in = q < 1.0f;
+        f  = in ? inner_f : outer_f;
+        df = in ? inner_df : outer_df;
+        if (q >= 2.0f) { f = 0.0f; df = 0.0f; }
+    } else if (KERNEL == SPH_KERNEL_QUINTIC) {
+        float a = fmaxf(3.0f - q, 0.0f), b = fmaxf(2.0f - q, 0.0f), c = fmaxf(1.0f - q, 0.0f);
+        float a2 = a * a, b2 = b * b, c2 = c * c;
+        float a4 = a2 * a2, b4 = b2 * b2, c4 = c2 * c2;
+        f  = fmaf(15.0f, c4 * c, fmaf(-6.0f, b4 * b, a4 * a));
+        df = fmaf(-75.0f, c4, fmaf(30.0f, b4, -5.0f * a4));
+    } else {
+        float t = fmaxf(fmaf(-0.5f, q, 1.0f), 0.0f);
+        float t2 = t * t;
+        if (DIM == 1) { f = t2 * t * fmaf(1.5f, q, 1.0f); df = -3.0f * q * t2; }
+        else          { f = t2 * t2 * fmaf(2.0f, q, 1.0f); df = -5.0f * q * t2 * t; }
+    }
+}
+
+__host__ __device__ inline double kernel_sigma(int kernel, int dim) {
+    const double pi = 3.141592653589793238462643383279502884;
+    if (kernel == SPH_KERNEL_CUBIC)   return dim == 1 ? 2.0 / 3.0 : dim == 2 ? 10.0 / (7.0 * pi) : 1.0 / pi;
+    if (kernel == SPH_KERNEL_QUINTIC) return dim == 1 ? 1.0 / 120.0 : dim == 2 ? 7.0 / (478.0 * pi) : 1.0 / (120.0 * pi);
+    return dim == 1 ? 5.0 / 8.0 : dim == 2 ? 7.0 / (4.0 * pi) : 21.0 / (16.0 * pi);
+}
+__host__ __device__ inline double kernel_support(int kernel) { return kernel == SPH_KERNEL_QUINTIC ? 3.0 : 2.0; }
+
+// Tait EOS, eq.6 (L122) / Listing 4 L393-400.
+// In float, (rho/rho0)^gamma - 1 cancels catastrophically for a weakly compressible fluid (rho ~ rho0), so it
+// is evaluated from t = (rho - rho0)/rho0 (the subtraction is exact for rho within a factor 2 of rho0):
+//   gamma = 7:  (1+t)^7 - 1 = t (7 + 21 t + 35 t^2 + 35 t^3 + 21 t^4 + 7 t^5 + t^6)   (exact identity)
+//   otherwise:  expm1(gamma * log1p(t))
+__device__ __forceinline__ float eos_pressure(float rho, float rho0, float B, float gamma, int gamma_is_7) {
+    const float t = (rho - rho0) / rho0;
+    float s;
+    if (gamma_is_7) s = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.0f, 7.0f), 21.0f), 35.0f), 35.0f), 21.0f), 7.0f);
+    else s = expm1f(gamma * log1pf(t));
+    return B * s;
+}
+
+// Cell coordinate of a position on one axis (clamped; out-of-range on a non-periodic axis is flagged by the caller).
+__device__ __forceinline__ int cell_coord(float x, float lo, float inv, int n) {
+    int c = __float2int_rd((x - lo) * inv);
+    return min(max(c, 0), n - 1);
+}
+

@@ -1,0 +1,368 @@
+// NNPS build (Sec.2.2): cell key -> counting sort by key -> cell-start offsets -> gather of
+// every property into cell order; the fused predictor-corrector update (eqs. 12-14) that feeds it;
+// the caller-order output gathers; and the neighbour-list export used for the bit-exact set parity.
+// All of these stream each particle once: they are HBM-bandwidth kernels.
+#include "sph_pair.cuh"
+
+#define NB 256
+
+// ------------------------------------------------------------------------------------------------
+// cell of a position (a1).  Linear key, x fastest, so the 3 x-adjacent cells of a stencil row are one run.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, bool& oob) {
+    int c[3]; const float x[3] = { p.x, p.y, p.z };
+    oob = false;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (a < g.dim) {
+            if (!g.per[a] && !(x[a] >= g.lo[a] && x[a] <= g.hi[a])) oob = true;   // also catches NaN
+            c[a] = cell_coord(x[a], g.lo[a], g.inv_cell[a], g.nc[a]);
+        } else c[a] = 0;
+    }
+    return (uint32_t)((c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0]);
+}
+
+// Loads the caller's SoA arrays into the (not yet sorted) float4 groups and reduces h_min / h_max.
+__global__ void __launch_bounds__(NB)
+k_pack(PackArgs A, SortedState S, int n, PairConsts pc, int* __restrict__ hminmax) {
+    const int gidx = blockIdx.x * NB + threadIdx.x;
+    float hmin = 3.0e38f, hmax = 0.0f;
+    if (gidx < n) {
+        int a = 0;
+        while (a + 1 < A.na && gidx >= A.base[a + 1]) ++a;
+        const long long i = gidx - A.base[a];
+        const PackSrc s = A.a[a];
+        const float h = s.h[i];
+        const float rho = s.rho ? s.rho[i] : pc.rho0;
+        const float p = s.p ? s.p[i] : eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
+        S.posh[gidx] = make_float4(s.x[i], s.y[i], s.z ? s.z[i] : 0.0f, h);
+        S.velm[gidx] = make_float4(s.u ? s.u[i] : 0.0f, s.v ? s.v[i] : 0.0f, s.w ? s.w[i] : 0.0f, s.m ? s.m[i] : 0.0f);
+        S.rp[gidx] = make_float2(rho, p / (rho * rho));
+        S.meta[gidx] = ((uint32_t)a << SPH_META_IDX_BITS) | (uint32_t)i;
+        S.acc[gidx] = make_float4(0, 0, 0, 0);
+        hmin = hmax = h;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        hmin = fminf(hmin, __shfl_xor_sync(SPH_FULL_MASK, hmin, o));
+        hmax = fmaxf(hmax, __shfl_xor_sync(SPH_FULL_MASK, hmax, o));
+    }
+    if ((threadIdx.x & 31) == 0 && hmax > 0.0f) {      // positive floats order like their bit patterns
+        atomicMin(&hminmax[0], __float_as_int(hmin));
+        atomicMax(&hminmax[1], __float_as_int(hmax));
+    }
+}
+
+__global__ void __launch_bounds__(NB)
+k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_t* __restrict__ rank,
+           uint32_t* __restrict__ cell_count, unsigned long long* __restrict__ counters) {
+    const int i = blockIdx.x * NB + threadIdx.x;
+    if (i >= n) return;
+    bool oob;
+    const uint32_t cell = cell_of(g, S.posh[i], oob);
+    const uint32_t k = cell * (uint32_t)g.na + (S.meta[i] >> SPH_META_IDX_BITS);
+    key[i] = k;
+    rank[i] = atomicAdd(&cell_count[k], 1u);
+    if (oob) atomicAdd(&counters[CNT_OUT_OF_DOMAIN], 1ull);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a8 + a1 fused: [finish step n: u += dt/2 a] + [start step n+1: u += dt/2 a; x += dt u; wrap] + cell key +
+// histogram.  eqs. 12-14 (L148-152); update_domain() periodic wrap (L443).  Continuity mode steps rho the same
+// way on EVERY array (the tank particles too, L142) and re-evaluates the EOS (group 1 of Listing 3).
+// ------------------------------------------------------------------------------------------------
+struct UpdateArgs {
+    float dt_half, dt; int kick2, kick1, move, continuity, rekey;
+    int fixed[SPH_MAX_ARRAYS];
+};
+
+__global__ void __launch_bounds__(NB)
+k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
+         uint32_t* __restrict__ key, uint32_t* __restrict__ rank, uint32_t* __restrict__ cell_count,
+         unsigned long long* __restrict__ counters) {
+    const int i = blockIdx.x * NB + threadIdx.x;
+    if (i >= n) return;
+    float4 pos = S.posh[i];
+    const uint32_t meta = S.meta[i];
+    const uint32_t aid = meta >> SPH_META_IDX_BITS;
+    const float4 a = S.acc[i];
+    if (!U.fixed[aid]) {
+        float4 vel = S.velm[i];
+        if (U.kick2) {                                                  // eq.14
+            vel.x = fmaf(U.dt_half, a.x, vel.x); vel.y = fmaf(U.dt_half, a.y, vel.y);
+            if (g.dim == 3) vel.z = fmaf(U.dt_half, a.z, vel.z);
+        }
+        if (U.kick1) {
+            vel.x = fmaf(U.dt_half, a.x, vel.x); vel.y = fmaf(U.dt_half, a.y, vel.y);   // eq.12
+            if (g.dim == 3) vel.z = fmaf(U.dt_half, a.z, vel.z);
+            if (U.move) {                                                // eq.13 + periodic wrap
+                pos.x = fmaf(U.dt, vel.x, pos.x); pos.y = fmaf(U.dt, vel.y, pos.y);
+                if (g.dim == 3) pos.z = fmaf(U.dt, vel.z, pos.z);
+                if (g.per[0]) { if (pos.x >= g.hi[0]) pos.x -= g.L[0]; else if (pos.x < g.lo[0]) pos.x += g.L[0]; }
+                if (g.per[1]) { if (pos.y >= g.hi[1]) pos.y -= g.L[1]; else if (pos.y < g.lo[1]) pos.y += g.L[1]; }
+                if (g.dim == 3 && g.per[2]) { if (pos.z >= g.hi[2]) pos.z -= g.L[2]; else if (pos.z < g.lo[2]) pos.z += g.L[2]; }
+                S.posh[i] = pos;
+            }
+        }
+        S.velm[i] = vel;
+    }
+    if (U.continuity) {
+        float rho = S.rp[i].x;
+        if (U.kick2) rho = fmaf(U.dt_half, a.w, rho);
+        if (U.kick1) rho = fmaf(U.dt_half, a.w, rho);
+        const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
+        S.rp[i] = make_float2(rho, p / (rho * rho));
+    }
+    if (U.rekey) {
+        bool oob;
+        const uint32_t cell = cell_of(g, pos, oob);
+        const uint32_t k = cell * (uint32_t)g.na + aid;
+        key[i] = k;
+        rank[i] = atomicAdd(&cell_count[k], 1u);
+        if (oob) atomicAdd(&counters[CNT_OUT_OF_DOMAIN], 1ull);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// exclusive scan of n uint32 (out has n+1 entries; out[n] = total): reduce / scan of block sums / final.
+// ------------------------------------------------------------------------------------------------
+#define SCAN_T 512
+#define SCAN_ITEMS 4
+#define SCAN_TILE (SCAN_T * SCAN_ITEMS)
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total) {
+    __shared__ uint32_t warp_sums[SCAN_T / 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t inc = v;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(SPH_FULL_MASK, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) warp_sums[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t s = lane < SCAN_T / 32 ? warp_sums[lane] : 0u, si = s;
+        for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(SPH_FULL_MASK, si, o); if (lane >= o) si += t; }
+        if (lane < SCAN_T / 32) warp_sums[lane] = si - s;
+        if (lane == 31 && total) *total = si;
+    }
+    __syncthreads();
+    const uint32_t r = warp_sums[w] + inc - v;
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(SCAN_T)
+k_scan_reduce(const uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ block_sums) {
+    const long long b0 = (long long)blockIdx.x * SCAN_TILE;
+    uint32_t s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { long long i = b0 + k * SCAN_T + threadIdx.x; if (i < n) s += in[i]; }
+    __shared__ uint32_t tot;
+    block_exclusive_scan(s, &tot);
+    __syncthreads();
+    if (threadIdx.x == 0) block_sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(SCAN_T)
+k_scan_blocks(uint32_t* __restrict__ block_sums, int nb) {       // single block, in place -> exclusive
+    __shared__ uint32_t carry, tot;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nb; b0 += SCAN_T) {
+        const int i = b0 + threadIdx.x;
+        const uint32_t v = i < nb ? block_sums[i] : 0u;
+        const uint32_t ex = block_exclusive_scan(v, &tot);
+        if (i < nb) block_sums[i] = ex + carry;
+        __syncthreads();
+        if (threadIdx.x == 0) carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) block_sums[nb] = carry;
+}
+
+__global__ void __launch_bounds__(SCAN_T)
+k_scan_final(const uint32_t* __restrict__ in, long long n, const uint32_t* __restrict__ block_sums,
+             uint32_t* __restrict__ out, int nb) {
+    const long long b0 = (long long)blockIdx.x * SCAN_TILE;
+    const long long i0 = b0 + (long long)threadIdx.x * SCAN_ITEMS;
+    uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (i0 + k < n) ? in[i0 + k] : 0u; s += v[k]; }
+    uint32_t ex = block_exclusive_scan(s, nullptr) + block_sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { if (i0 + k < n) out[i0 + k] = ex; ex += v[k]; }
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = block_sums[nb];
+}
+
+static int scan_exclusive(sph_ctx* c, const uint32_t* in, uint32_t* out, long long n) {
+    const int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
+    if (nb == 0) { SPH_CUDA_OK(c, cudaMemsetAsync(out, 0, sizeof(uint32_t), c->stream)); return SPH_OK; }
+    SPH_LAUNCH(c, k_scan_reduce, nb, SCAN_T, 0, in, n, c->block_sums);
+    SPH_LAUNCH(c, k_scan_blocks, 1, SCAN_T, 0, c->block_sums, nb);
+    SPH_LAUNCH(c, k_scan_final, nb, SCAN_T, 0, in, n, c->block_sums, out, nb);
+    return SPH_OK;
+}
+
+// a3: gather every persistent property into cell order (double buffer A -> B).
+__global__ void __launch_bounds__(NB)
+k_scatter(SortedState A, SortedState B, int n, int na, const uint32_t* __restrict__ key,
+          const uint32_t* __restrict__ rank, const uint32_t* __restrict__ cell_start) {
+    const int i = blockIdx.x * NB + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t k = key[i];
+    const uint32_t d = cell_start[k] + rank[i];
+    B.posh[d] = A.posh[i];
+    B.velm[d] = A.velm[i];
+    B.rp[d] = A.rp[i];
+    B.meta[d] = A.meta[i];
+    B.cell[d] = k / (uint32_t)na;
+}
+
+int nnps_key_hist(sph_ctx* c) {
+    const int n = (int)c->n_total;
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));
+    if (n) SPH_LAUNCH(c, k_key_hist, (n + NB - 1) / NB, NB, 0, c->grid, c->S[c->cur], n, c->key, c->rank,
+                      c->cell_count, c->counters);
+    return SPH_OK;
+}
+
+int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey) {
+    const int n = (int)c->n_total;
+    UpdateArgs U;
+    U.dt_half = 0.5f * dt; U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
+    U.continuity = continuity; U.rekey = rekey;
+    for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
+    if (rekey) SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));
+    if (n) SPH_LAUNCH(c, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
+                      c->cell_count, c->counters);
+    return SPH_OK;
+}
+
+int nnps_sort_from_keys(sph_ctx* c) {
+    const int n = (int)c->n_total;
+    int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys);
+    if (rc) return rc;
+    if (n) SPH_LAUNCH(c, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
+                      c->key, c->rank, c->cell_start);
+    c->cur ^= 1;
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// caller-order outputs
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NB)
+k_gather_out(SortedState S, int n, uint32_t array, OutPtrs O) {
+    const int i = blockIdx.x * NB + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t meta = S.meta[i];
+    if ((meta >> SPH_META_IDX_BITS) != array) return;
+    const uint32_t o = meta & SPH_META_IDX_MASK;
+    if (O.x || O.y || O.z) { const float4 p = S.posh[i]; if (O.x) O.x[o] = p.x; if (O.y) O.y[o] = p.y; if (O.z) O.z[o] = p.z; }
+    if (O.u || O.v || O.w) { const float4 v = S.velm[i]; if (O.u) O.u[o] = v.x; if (O.v) O.v[o] = v.y; if (O.w) O.w[o] = v.z; }
+    if (O.rho || O.p) { const float2 r = S.rp[i]; if (O.rho) O.rho[o] = r.x; if (O.p) O.p[o] = r.y * r.x * r.x; }
+    if (O.ax || O.ay || O.az || O.arho) {
+        const float4 a = S.acc[i];
+        if (O.ax) O.ax[o] = a.x; if (O.ay) O.ay[o] = a.y; if (O.az) O.az[o] = a.z; if (O.arho) O.arho[o] = a.w;
+    }
+}
+
+int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O) {
+    const int n = (int)c->n_total;
+    if (n) SPH_LAUNCH(c, k_gather_out, (n + NB - 1) / NB, NB, 0, c->S[c->cur], n, (uint32_t)array, O);
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// neighbour-list export (verification): the same walker and the same predicate as the pair kernels.
+// ------------------------------------------------------------------------------------------------
+struct CountPolicy {
+    uint32_t cnt;
+    __device__ __forceinline__ void hit(uint32_t) { ++cnt; }
+    __device__ __forceinline__ void pre_chunk() {}
+    __device__ __forceinline__ void tested(int) {}
+};
+struct FillPolicy {
+    const uint32_t* meta; int32_t* row; uint32_t cnt;
+    __device__ __forceinline__ void hit(uint32_t j) { row[cnt++] = (int32_t)(meta[j] & SPH_META_IDX_MASK); }
+    __device__ __forceinline__ void pre_chunk() {}
+    __device__ __forceinline__ void tested(int) {}
+};
+
+template <int DIM, bool VARH, bool FILL>
+__global__ void __launch_bounds__(NB)
+k_neighbors(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
+            uint32_t dest, uint32_t src, uint32_t* __restrict__ counts, const uint32_t* __restrict__ offsets,
+            int32_t* __restrict__ indices) {
+    const int i = blockIdx.x * NB + threadIdx.x;
+    const bool in = i < n;
+    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
+    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; }
+    const bool active = in && (meta >> SPH_META_IDX_BITS) == dest;
+    if (!__any_sync(SPH_FULL_MASK, active)) return;
+    const uint32_t o = meta & SPH_META_IDX_MASK;
+    if (!FILL) {
+        CountPolicy pol; pol.cnt = 0;
+        walk_candidates<DIM, VARH, false>(g, pc, S.posh, cell_start, active, pi, ci, 1u << src, pol);
+        if (active) counts[o] = pol.cnt;
+    } else {
+        FillPolicy pol; pol.meta = S.meta; pol.cnt = 0; pol.row = indices + (active ? offsets[o] : 0u);
+        walk_candidates<DIM, VARH, false>(g, pc, S.posh, cell_start, active, pi, ci, 1u << src, pol);
+        if (active) {                                   // rows ascending (insertion sort; rows are short)
+            int32_t* r = pol.row; const int m = (int)pol.cnt;
+            for (int a = 1; a < m; ++a) { int32_t v = r[a]; int b = a - 1; while (b >= 0 && r[b] > v) { r[b + 1] = r[b]; --b; } r[b + 1] = v; }
+        }
+    }
+}
+
+__global__ void k_widen(const uint32_t* __restrict__ in, int64_t* __restrict__ out, long long n) {
+    const long long i = (long long)blockIdx.x * NB + threadIdx.x;
+    if (i < n) out[i] = (int64_t)in[i];
+}
+
+int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32_t* indices, int64_t cap,
+                          int64_t* total, int mem) {
+    const int n = (int)c->n_total;
+    const long long nd = c->n[dest];
+    uint32_t* counts = c->key;            // scratch: key/rank are dead between sorts
+    uint32_t* off32 = c->rank;
+    const int grid = (n + NB - 1) / NB;
+    SPH_CUDA_OK(c, cudaMemsetAsync(counts, 0, (size_t)(nd + 1) * sizeof(uint32_t), c->stream));
+    SortedState& S = c->S[c->cur];
+#define LN(FILL, IDX) do { \
+    if (c->grid.dim == 2) { if (c->variable_h) SPH_LAUNCH(c, (k_neighbors<2, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, (k_neighbors<2, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } \
+    else                  { if (c->variable_h) SPH_LAUNCH(c, (k_neighbors<3, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, (k_neighbors<3, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
+    if (n) LN(false, (int32_t*)nullptr);
+    int rc = scan_exclusive(c, counts, off32, nd);
+    if (rc) return rc;
+    uint32_t tot32 = 0;
+    SPH_CUDA_OK(c, cudaMemcpyAsync(&tot32, off32 + nd, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    *total = (int64_t)tot32;
+    int64_t* d_off = offsets; int32_t* d_idx = indices;
+    if (mem == SPH_MEM_HOST) {            // verification-only path: temporary device buffers
+        SPH_CUDA_OK(c, cudaMalloc(&d_off, (size_t)(nd + 1) * sizeof(int64_t)));
+        if (indices && cap >= *total && *total > 0) SPH_CUDA_OK(c, cudaMalloc(&d_idx, (size_t)(*total) * sizeof(int32_t)));
+    }
+    SPH_LAUNCH(c, k_widen, (int)((nd + 1 + NB - 1) / NB), NB, 0, off32, d_off, nd + 1);
+    const bool fill = indices && cap >= *total && *total > 0;
+    if (fill && n) LN(true, d_idx);
+#undef LN
+    if (mem == SPH_MEM_HOST) {
+        SPH_CUDA_OK(c, cudaMemcpyAsync(offsets, d_off, (size_t)(nd + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+        if (fill) SPH_CUDA_OK(c, cudaMemcpyAsync(indices, d_idx, (size_t)(*total) * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+        SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+        cudaFree(d_off); if (fill) cudaFree(d_idx);
+    } else SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// build entry used by sph_nnps_build: pack -> (host sizes the grid from h_max) -> key/hist -> sort
+// ------------------------------------------------------------------------------------------------
+int nnps_pack(sph_ctx* c, const PackArgs& A) {
+    const int n = (int)c->n_total;
+    const int init[2] = { 0x7f7fffff, 0 };
+    SPH_CUDA_OK(c, cudaMemcpyAsync(c->hminmax, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+    if (n) SPH_LAUNCH(c, k_pack, (n + NB - 1) / NB, NB, 0, A, c->S[c->cur], n, c->pc, (int*)c->hminmax);
+    return SPH_OK;
+}

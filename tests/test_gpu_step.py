@@ -1,0 +1,56 @@
+"""-m gpu parity of sph_pc_step (eqs. 12-14) against the oracle's step, one step from the same state
+(R15: float32 trajectories drift from float64 ones, so multi-step runs are gated by
+"one more step from the GPU's own state", with the GPU's a^n handed to the oracle)."""
+import numpy as np
+import pytest
+
+from gpu_helpers import TOL, assert_close, make_ctx, min_image_diff
+
+pytestmark = pytest.mark.gpu
+
+
+def _compare_state(wl, ctx, st, tag, tol=TOL):
+    for d, A in enumerate(st.arrays):
+        if wl.arrays[d].n == 0:
+            continue
+        out = {k: v.cpu().numpy() for k, v in ctx.sync_state(d).items()}
+        for k, axis in (("x", 0), ("y", 1), ("z", 2)):
+            if axis >= wl.dim:
+                continue
+            diff = min_image_diff(out[k], A[k], wl.lo[axis], wl.hi[axis], wl.periodic[axis])
+            scale = max(abs(wl.lo[axis]), abs(wl.hi[axis]))
+            assert np.abs(diff).max() <= tol * scale, f"{tag} {k}[{d}]: {np.abs(diff).max() / scale:.3e}"
+        vmax = max(np.abs(A["u"]).max(), np.abs(A["v"]).max(), np.abs(A["w"]).max())
+        for k, axis in (("u", 0), ("v", 1), ("w", 2)):
+            if axis >= wl.dim or vmax == 0:
+                continue
+            err = np.abs(out[k].astype(np.float64) - A[k]).max() / vmax
+            assert err <= tol, f"{tag} {k}[{d}]: {err:.3e} of max|u|"
+        assert_close(out["rho"], A["rho"], f"{tag} rho[{d}]", tol)
+
+
+def _step_cases(WL):
+    return [
+        ("C1", WL.taylor_green_2d(), "summation"),
+        ("3d_per", WL.periodic_box_3d((16, 16, 16), seed=1), "summation"),
+        ("3d_varh", WL.random_box(n=4000, dim=3, periodic=True, seed=61, kernel="cubic", variable_h=True), "summation"),
+        ("dam2d_cont", WL.dam_break_2d(dx=0.04), "continuity"),
+        ("dam2d_summ", WL.dam_break_2d(dx=0.04), "summation"),
+        ("dam3d_cont", WL.dam_break_3d(dx=0.05), "continuity"),
+    ]
+
+
+STEP_IDS = ["C1", "3d_per", "3d_varh", "dam2d_cont", "dam2d_summ", "dam3d_cont"]
+
+
+@pytest.mark.parametrize("idx", range(len(STEP_IDS)), ids=STEP_IDS)
+def test_one_step_from_the_same_state(O, WL, idx):
+    """a^0 evaluation + one full step (what BASELINE config 1 calls 'one step')."""
+    _, wl, mode = _step_cases(WL)[idx]
+    ctx, _ = make_ctx(wl)
+    ctx.pc_step(wl.dt, 1, mode)
+    st = O.State(wl)
+    O.pc_step(wl, st, wl.dt, mode)
+    _compare_state(wl, ctx, st, "step1")
+    ctx.synchronize()
+    ctx.close()
