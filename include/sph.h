@@ -92,6 +92,11 @@ typedef struct sph_array {      /* one named particle array (L316) */
     float *m;                   /* mass           (NULL -> 0: array only queries, never a source of mass) */
     float *rho;                 /* density        (NULL -> rho0) */
     float *p;                   /* pressure       (NULL -> EOS(rho)) */
+    float *ax, *ay, *az, *arho; /* accelerations of the last evaluation: the paper's au, av, aw, arho properties
+                                 * (L402-418).  Input to sph_nnps_build (restart: if every dynamic array gives
+                                 * ax,ay,(az) -- and, for continuity mode, every array gives arho -- the first
+                                 * sph_pc_step reuses them as a^n instead of re-evaluating); output of sph_sync_state.
+                                 * NULL -> 0 / not written. */
 } sph_array;
 
 typedef struct sph_stats {
@@ -100,12 +105,32 @@ typedef struct sph_stats {
     int64_t n_particles;        /* all arrays */
     int64_t pairs_density;      /* (i,j) pairs passing the predicate in the last density pass(es), self pairs included */
     int64_t pairs_accel;        /* same for the last acceleration pass(es) */
-    int64_t candidates;         /* predicate evaluations in the last pair pass */
+    int64_t candidates;         /* predicate evaluations of the last density + acceleration passes */
+    int64_t candidates_density, candidates_accel;
     int64_t kernel_launches;    /* CUDA kernels launched by this context since sph_create */
     int64_t steps_done;         /* predictor-corrector steps since the last sph_nnps_build */
     int32_t variable_h;         /* 1 if h_min != h_max at the last build */
     float h_max;
 } sph_stats;
+
+/* Per-kernel device timing (CUDA events on the context stream around every launch), for the roofline report. */
+enum sph_kernel_id {
+    SPH_K_PACK = 0,             /* caller SoA -> packed state + h_min/h_max                       */
+    SPH_K_KEY = 1,              /* a1: cell key + histogram                                       */
+    SPH_K_UPDATE = 2,           /* a8 + a1: predictor-corrector update fused with key + histogram */
+    SPH_K_SCAN = 3,             /* a2: exclusive scan of the cell histogram                       */
+    SPH_K_SCATTER = 4,          /* a2/a3: counting-sort scatter of every property into cell order */
+    SPH_K_DENSITY = 5,          /* a4 + a5: summation density + EOS                               */
+    SPH_K_ACCEL = 6,            /* a6 + a7: momentum (+ continuity) pair loop                     */
+    SPH_K_OUTPUT = 7,           /* caller-order output gather                                     */
+    SPH_K_NEIGHBORS = 8,        /* verification export                                            */
+    SPH_K_COUNT = 16
+};
+typedef struct sph_profile {
+    int64_t launches[SPH_K_COUNT];   /* launches recorded since sph_set_profiling(ctx, 1)         */
+    double ms[SPH_K_COUNT];          /* summed device time of those launches                      */
+    int64_t dropped;                 /* launches not recorded because the event pool was full     */
+} sph_profile;
 
 /* ---- lifetime ------------------------------------------------------------------------------- */
 
@@ -154,7 +179,7 @@ int sph_pc_step(sph_ctx* ctx, double dt, int n_steps, int density_mode);
 /* ---- state out, verification, diagnostics ------------------------------------------------------ */
 
 /* Writes the context's current state of array `array` into the non-NULL pointers of *out
- * (x,y,z,u,v,w,rho,p; h and m never change) in the caller's original particle order.  out->n must equal
+ * (x,y,z,u,v,w,rho,p,ax,ay,az,arho; h and m never change) in the caller's original particle order.  out->n must equal
  * the array's size.  Asynchronous for SPH_MEM_DEVICE; [sync] for SPH_MEM_HOST. */
 int sph_sync_state(sph_ctx* ctx, int array, const sph_array* out);
 
@@ -166,6 +191,12 @@ int sph_get_accel(sph_ctx* ctx, int array, float* ax, float* ay, float* az, floa
  * to get *total only.  Used for the bit-exact set parity.  Host pointers when mem == SPH_MEM_HOST.  [sync] */
 int sph_nnps_get_neighbors(sph_ctx* ctx, int dest, int src, int64_t* offsets, int32_t* indices,
                            int64_t cap, int64_t* total, int mem);
+
+/* enable != 0: record a CUDA event pair around every kernel launch from now on (clears earlier records);
+ * 0: stop.  Off by default (the events add a few microseconds per launch). */
+int sph_set_profiling(sph_ctx* ctx, int enable);
+int sph_get_profile(sph_ctx* ctx, sph_profile* out);                                     /* [sync] */
+const char* sph_kernel_name(int kernel_id);
 
 int sph_get_stats(sph_ctx* ctx, sph_stats* out);                                         /* [sync] */
 int sph_synchronize(sph_ctx* ctx);   /* [sync] waits for the stream and reports pending device-side errors */

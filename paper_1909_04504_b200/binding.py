@@ -24,9 +24,12 @@ ARRAY_DYNAMIC, ARRAY_FIXED = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_set_tables", "sph_nnps_build", "sph_summation_density",
            "sph_wcsph_accel", "sph_pc_step", "sph_sync_state", "sph_get_accel", "sph_nnps_get_neighbors",
-           "sph_get_stats", "sph_synchronize", "sph_strerror", "sph_last_error", "sph_abi_version"]
+           "sph_get_stats", "sph_synchronize", "sph_strerror", "sph_last_error", "sph_abi_version",
+           "sph_set_profiling", "sph_get_profile", "sph_kernel_name"]
 
 _FP = C.POINTER(C.c_float)
+FIELD_NAMES = ("x", "y", "z", "u", "v", "w", "h", "m", "rho", "p", "ax", "ay", "az", "arho")
+SPH_K_COUNT = 16
 
 
 class sph_domain(C.Structure):
@@ -40,14 +43,19 @@ class sph_params(C.Structure):
 
 class sph_array(C.Structure):
     _fields_ = [("n", C.c_int64), ("flags", C.c_int), ("mem", C.c_int)] + \
-               [(k, C.c_void_p) for k in ("x", "y", "z", "u", "v", "w", "h", "m", "rho", "p")]
+               [(k, C.c_void_p) for k in FIELD_NAMES]
 
 
 class sph_stats(C.Structure):
     _fields_ = [("n_cells", C.c_int32 * 3), ("cell_size", C.c_double * 3), ("n_particles", C.c_int64),
                 ("pairs_density", C.c_int64), ("pairs_accel", C.c_int64), ("candidates", C.c_int64),
+                ("candidates_density", C.c_int64), ("candidates_accel", C.c_int64),
                 ("kernel_launches", C.c_int64), ("steps_done", C.c_int64), ("variable_h", C.c_int32),
                 ("h_max", C.c_float)]
+
+
+class sph_profile(C.Structure):
+    _fields_ = [("launches", C.c_int64 * SPH_K_COUNT), ("ms", C.c_double * SPH_K_COUNT), ("dropped", C.c_int64)]
 
 
 class SphError(RuntimeError):
@@ -80,10 +88,13 @@ def load() -> C.CDLL:
         L.sph_nnps_get_neighbors.argtypes = [vp, i32, i32, vp, vp, i64, C.POINTER(i64), i32]
         L.sph_get_stats.argtypes = [vp, C.POINTER(sph_stats)]
         L.sph_synchronize.argtypes = [vp]
+        L.sph_set_profiling.argtypes = [vp, i32]
+        L.sph_get_profile.argtypes = [vp, C.POINTER(sph_profile)]
+        L.sph_kernel_name.argtypes = [i32]; L.sph_kernel_name.restype = C.c_char_p
         L.sph_strerror.argtypes = [i32]; L.sph_strerror.restype = C.c_char_p
         L.sph_last_error.argtypes = [vp]; L.sph_last_error.restype = C.c_char_p
         for name in EXPORTS:
-            if name not in ("sph_strerror", "sph_last_error"):
+            if name not in ("sph_strerror", "sph_last_error", "sph_kernel_name"):
                 getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -106,7 +117,7 @@ def make_array(fields: Dict[str, object], fixed: bool) -> sph_array:
     a.flags = ARRAY_FIXED if fixed else ARRAY_DYNAMIC
     mem = None
     n = None
-    for k in ("x", "y", "z", "u", "v", "w", "h", "m", "rho", "p"):
+    for k in FIELD_NAMES:
         ptr, m = _ptr_and_mem(fields.get(k))
         setattr(a, k, ptr)
         if ptr is not None or (fields.get(k) is not None):
@@ -212,9 +223,10 @@ class SphContext:
     def pc_step(self, dt: float, n_steps: int, mode):
         self._check(self.L.sph_pc_step(self.ctx, float(dt), int(n_steps), MODE_ID.get(mode, mode)))
 
-    def sync_state(self, array: int, fields=("x", "y", "z", "u", "v", "w", "rho", "p"), host: bool = False):
+    def sync_state(self, array: int, fields=("x", "y", "z", "u", "v", "w", "rho", "p"), host: bool = False, out=None):
         n = self.n[array]
-        out = {k: self._out(n, host) for k in fields if not (self.dim == 2 and k in ("z", "w"))}
+        if out is None:
+            out = {k: self._out(n, host) for k in fields if not (self.dim == 2 and k in ("z", "w", "az"))}
         a = make_array(out, False)
         a.n = n; a.mem = MEM_HOST if host else MEM_DEVICE
         self._check(self.L.sph_sync_state(self.ctx, array, C.byref(a)))
@@ -244,6 +256,20 @@ class SphContext:
 
     def synchronize(self):
         self._check(self.L.sph_synchronize(self.ctx))
+
+    def set_profiling(self, enable: bool):
+        self._check(self.L.sph_set_profiling(self.ctx, int(bool(enable))))
+
+    def get_profile(self) -> Dict[str, Dict[str, float]]:
+        """{kernel name: {"launches": n, "ms": summed device time}} since set_profiling(True)."""
+        p = sph_profile()
+        self._check(self.L.sph_get_profile(self.ctx, C.byref(p)))
+        out = {}
+        for k in range(SPH_K_COUNT):
+            if p.launches[k]:
+                out[self.L.sph_kernel_name(k).decode()] = {"launches": int(p.launches[k]), "ms": float(p.ms[k])}
+        out["_dropped"] = int(p.dropped)
+        return out
 
 
 def device_arrays(wl, device=None):

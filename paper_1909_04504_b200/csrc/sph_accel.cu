@@ -84,7 +84,7 @@ k_accel(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ c
         if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
     const unsigned long long h = warp_sum_u64(pol.hits), t = warp_sum_u64(pol.tests);
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); atomicAdd(&counters[CNT_CANDIDATES], t); }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); atomicAdd(&counters[CNT_CAND_ACCEL], t); }
 }
 
 template <int KERNEL, int DIM>
@@ -100,7 +100,7 @@ static int launch_accel_kd(sph_ctx* c, bool merged, bool want_arho, bool arho_on
 #define LA(VARH, MERGED, PER, ARHO) do { \
         auto kern = k_accel<KERNEL, DIM, VARH, MERGED, PER, ARHO>; \
         SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        SPH_LAUNCH(c, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, ao, c->counters); } while (0)
+        SPH_LAUNCH(c, SPH_K_ACCEL, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, ao, c->counters); } while (0)
 #define LA2(VARH, MERGED, PER) do { if (want_arho) LA(VARH, MERGED, PER, true); else LA(VARH, MERGED, PER, false); } while (0)
 #define LA3(VARH, MERGED) do { if (per) LA2(VARH, MERGED, true); else LA2(VARH, MERGED, false); } while (0)
     if (varh) { if (merged) LA3(true, true); else LA3(true, false); }

@@ -4,9 +4,10 @@
 #include "sph_ctx.cuh"
 #include <math.h>
 #include <string.h>
+#include <stdlib.h>
 #include <new>
 
-static const int N_STAGE_FIELDS = 10;
+static const int N_STAGE_FIELDS = 14;
 
 
 extern "C" const char* sph_strerror(int code) {
@@ -94,8 +95,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].meta, N * sizeof(uint32_t)));
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].cell, N * sizeof(uint32_t)));
     }
-    SPH_CUDA_OK(c, cudaMalloc(&c->S[0].acc, N * sizeof(float4)));
-    c->S[1].acc = c->S[0].acc;
+    for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMalloc(&c->S[b].acc, N * sizeof(float4)));
     SPH_CUDA_OK(c, cudaMalloc(&c->key, (N + 1) * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMalloc(&c->rank, (N + 1) * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMalloc(&c->cell_count, (size_t)(c->max_keys + 2) * sizeof(uint32_t)));
@@ -106,7 +106,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     SPH_CUDA_OK(c, cudaMalloc(&c->counters, CNT_COUNT * sizeof(unsigned long long)));
     SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 2 * sizeof(float)));
     SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
-    SPH_CUDA_OK(c, cudaMemsetAsync(c->S[0].acc, 0, N * sizeof(float4), c->stream));
+    for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMemsetAsync(c->S[b].acc, 0, N * sizeof(float4), c->stream));
     SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
     return SPH_OK;
 }
@@ -117,8 +117,10 @@ extern "C" int sph_destroy(sph_ctx* c) {
     for (int b = 0; b < 2; ++b) {
         cudaFree(c->S[b].posh); cudaFree(c->S[b].velm); cudaFree(c->S[b].rp); cudaFree(c->S[b].meta); cudaFree(c->S[b].cell);
     }
-    cudaFree(c->S[0].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
+    cudaFree(c->S[0].acc); cudaFree(c->S[1].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
     cudaFree(c->block_sums); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
+    for (int k = 0; k < c->prof_cap; ++k) { cudaEventDestroy(c->prof[k].a); cudaEventDestroy(c->prof[k].b); }
+    free(c->prof);
     delete c;
     return SPH_OK;
 }
@@ -177,8 +179,9 @@ static float* stage_field(sph_ctx* c, int field, int array) { return c->staging 
 extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays) {
     if (!c || !arrays) return SPH_ERR_NULL;
     if (n_arrays != c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "n_arrays differs from sph_create");
-    c->built = false; c->have_accel = false;
+    c->built = false; c->have_accel = false; c->have_arho = false;
     int64_t tot = 0;
+    bool all_acc = true, all_arho = true;
     for (int a = 0; a < c->na; ++a) {
         const sph_array& A = arrays[a];
         if (A.n < 0) return sph_fail(c, SPH_ERR_BAD_ARG, "negative n");
@@ -187,6 +190,8 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
         if (A.mem != SPH_MEM_DEVICE && A.mem != SPH_MEM_HOST) return sph_fail(c, SPH_ERR_BAD_ARG, "bad mem");
         c->n[a] = A.n; c->base[a] = tot; c->fixed[a] = (A.flags & SPH_ARRAY_FIXED) ? 1 : 0;
         tot += A.n;
+        if (A.n > 0 && !c->fixed[a] && (!A.ax || !A.ay || (c->dom.dim == 3 && !A.az))) all_acc = false;
+        if (A.n > 0 && !A.arho) all_arho = false;
     }
     c->base[c->na] = tot; c->n_total = tot;
     if (!c->tables_user) default_tables(c);
@@ -196,7 +201,7 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     for (int a = 0; a <= c->na; ++a) P.base[a] = c->base[a];
     for (int a = 0; a < c->na; ++a) {
         const sph_array& A = arrays[a];
-        const float* src[N_STAGE_FIELDS] = { A.x, A.y, A.z, A.u, A.v, A.w, A.h, A.m, A.rho, A.p };
+        const float* src[N_STAGE_FIELDS] = { A.x, A.y, A.z, A.u, A.v, A.w, A.h, A.m, A.rho, A.p, A.ax, A.ay, A.az, A.arho };
         const float* use[N_STAGE_FIELDS];
         for (int f = 0; f < N_STAGE_FIELDS; ++f) {
             use[f] = src[f];
@@ -206,7 +211,8 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
                 use[f] = d;
             }
         }
-        P.a[a] = PackSrc{ use[0], use[1], use[2], use[3], use[4], use[5], use[6], use[7], use[8], use[9] };
+        P.a[a] = PackSrc{ use[0], use[1], use[2], use[3], use[4], use[5], use[6], use[7], use[8], use[9],
+                          use[10], use[11], use[12], use[13] };
     }
     SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
     c->cur = 0;
@@ -223,8 +229,9 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     c->pc.fac_const = (float)(kernel_sigma(c->prm.kernel, c->dom.dim) / pow((double)c->h_max, c->dom.dim));
     rc = size_grid(c); if (rc) return rc;
     rc = nnps_key_hist(c); if (rc) return rc;
-    rc = nnps_sort_from_keys(c); if (rc) return rc;
+    rc = nnps_sort_from_keys(c, true); if (rc) return rc;
     c->built = true; c->steps_done = 0;
+    c->have_accel = all_acc && tot > 0; c->have_arho = all_arho && tot > 0;     // restart from caller-supplied a^n
     return SPH_OK;
 }
 
@@ -254,7 +261,7 @@ extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask,
     uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
     masks[dest] = source_mask;
     int rc = zero_counter(c, CNT_PAIRS_DENSITY); if (rc) return rc;
-    rc = zero_counter(c, CNT_CANDIDATES); if (rc) return rc;
+    rc = zero_counter(c, CNT_CAND_DENSITY); if (rc) return rc;
     rc = launch_density(c, masks); if (rc) return rc;
     if (rho_out || p_out) { OutPtrs O; memset(&O, 0, sizeof(O)); O.rho = rho_out; O.p = p_out; return emit(c, dest, O, mem); }
     return SPH_OK;
@@ -267,7 +274,7 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
     uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
     masks[dest] = source_mask;
     int rc = zero_counter(c, CNT_PAIRS_ACCEL); if (rc) return rc;
-    rc = zero_counter(c, CNT_CANDIDATES); if (rc) return rc;
+    rc = zero_counter(c, CNT_CAND_ACCEL); if (rc) return rc;
     rc = launch_accel(c, masks, arho != nullptr, false); if (rc) return rc;
     if (ax || ay || az || arho) { OutPtrs O; memset(&O, 0, sizeof(O)); O.ax = ax; O.ay = ay; O.az = az; O.arho = arho; return emit(c, dest, O, mem); }
     return SPH_OK;
@@ -279,7 +286,8 @@ static int evaluate(sph_ctx* c, bool continuity) {
     int rc;
     rc = zero_counter(c, CNT_PAIRS_DENSITY); if (rc) return rc;
     rc = zero_counter(c, CNT_PAIRS_ACCEL); if (rc) return rc;
-    rc = zero_counter(c, CNT_CANDIDATES); if (rc) return rc;
+    rc = zero_counter(c, CNT_CAND_DENSITY); if (rc) return rc;
+    rc = zero_counter(c, CNT_CAND_ACCEL); if (rc) return rc;
     auto grouped = [&](const uint32_t* tbl, const bool* take, auto&& fn) -> int {
         bool done[SPH_MAX_ARRAYS] = { false, false, false, false };
         for (int a = 0; a < c->na; ++a) {
@@ -312,11 +320,14 @@ extern "C" int sph_pc_step(sph_ctx* c, double dt, int n_steps, int density_mode)
         return sph_fail(c, SPH_ERR_BAD_ARG, "bad n_steps / density_mode / dt");
     const bool cont = density_mode == SPH_DENSITY_CONTINUITY;
     int rc;
-    if (!c->have_accel) { rc = evaluate(c, cont); if (rc) return rc; c->have_accel = true; }   // a^0 = F(x^0, u^0)
+    if (!c->have_accel || (cont && !c->have_arho)) {                                             // a^0 = F(x^0, u^0)
+        rc = evaluate(c, cont); if (rc) return rc; c->have_accel = true; c->have_arho = cont;
+    }
     for (int s = 0; s < n_steps; ++s) {
         rc = nnps_update_key_hist(c, (float)dt, s > 0, true, cont, true); if (rc) return rc;    // (14 of step s-1) + 12 + 13 + key
-        rc = nnps_sort_from_keys(c); if (rc) return rc;                                         // NNPS rebuilt every step (L443)
+        rc = nnps_sort_from_keys(c, false); if (rc) return rc;                                  // NNPS rebuilt every step (L443)
         rc = evaluate(c, cont); if (rc) return rc;
+        c->have_arho = cont;
         c->steps_done++;
     }
     if (n_steps > 0) { rc = nnps_update_key_hist(c, (float)dt, true, false, cont, false); if (rc) return rc; }   // eq.14
@@ -330,6 +341,7 @@ extern "C" int sph_sync_state(sph_ctx* c, int array, const sph_array* out) {
     if (out->n != c->n[array]) return sph_fail(c, SPH_ERR_CAPACITY, "out->n differs from the array size");
     OutPtrs O; memset(&O, 0, sizeof(O));
     O.x = out->x; O.y = out->y; O.z = out->z; O.u = out->u; O.v = out->v; O.w = out->w; O.rho = out->rho; O.p = out->p;
+    O.ax = out->ax; O.ay = out->ay; O.az = out->az; O.arho = out->arho;
     return emit(c, array, O, out->mem);
 }
 
@@ -376,10 +388,70 @@ extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->n_particles = c->n_total;
     out->pairs_density = (int64_t)h[CNT_PAIRS_DENSITY];
     out->pairs_accel = (int64_t)h[CNT_PAIRS_ACCEL];
-    out->candidates = (int64_t)h[CNT_CANDIDATES];
+    out->candidates_density = (int64_t)h[CNT_CAND_DENSITY];
+    out->candidates_accel = (int64_t)h[CNT_CAND_ACCEL];
+    out->candidates = out->candidates_density + out->candidates_accel;
     out->kernel_launches = c->launches;
     out->steps_done = c->steps_done;
     out->variable_h = c->variable_h ? 1 : 0;
     out->h_max = c->h_max;
     return SPH_OK;
+}
+
+// ---- per-kernel device timing ----------------------------------------------------------------------
+static const int PROF_MAX = 1 << 15;
+
+int sph_prof_begin(sph_ctx* c, int id) {
+    if (c->prof_used >= PROF_MAX) { c->prof_dropped++; return -1; }
+    if (c->prof_used >= c->prof_cap) {
+        const int ncap = c->prof_cap ? c->prof_cap * 2 : 256;
+        sph_ctx::ProfRec* np = (sph_ctx::ProfRec*)realloc(c->prof, (size_t)ncap * sizeof(sph_ctx::ProfRec));
+        if (!np) { c->prof_dropped++; return -1; }
+        c->prof = np;
+        for (int k = c->prof_cap; k < ncap; ++k) {
+            if (cudaEventCreate(&c->prof[k].a) != cudaSuccess || cudaEventCreate(&c->prof[k].b) != cudaSuccess) { c->prof_cap = k; c->prof_dropped++; return -1; }
+        }
+        c->prof_cap = ncap;
+    }
+    const int r = c->prof_used++;
+    c->prof[r].id = id;
+    cudaEventRecord(c->prof[r].a, c->stream);
+    return r;
+}
+void sph_prof_end(sph_ctx* c, int rec) { cudaEventRecord(c->prof[rec].b, c->stream); }
+
+extern "C" int sph_set_profiling(sph_ctx* c, int enable) {
+    if (!c) return SPH_ERR_NULL;
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    c->prof_on = enable != 0; c->prof_used = 0; c->prof_dropped = 0;
+    return SPH_OK;
+}
+
+extern "C" int sph_get_profile(sph_ctx* c, sph_profile* out) {
+    if (!c || !out) return SPH_ERR_NULL;
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    memset(out, 0, sizeof(*out));
+    for (int r = 0; r < c->prof_used; ++r) {
+        float ms = 0.0f;
+        SPH_CUDA_OK(c, cudaEventElapsedTime(&ms, c->prof[r].a, c->prof[r].b));
+        const int id = c->prof[r].id;
+        if (id >= 0 && id < SPH_K_COUNT) { out->launches[id]++; out->ms[id] += (double)ms; }
+    }
+    out->dropped = c->prof_dropped;
+    return SPH_OK;
+}
+
+extern "C" const char* sph_kernel_name(int id) {
+    switch (id) {
+        case SPH_K_PACK: return "k_pack";
+        case SPH_K_KEY: return "k_key_hist";
+        case SPH_K_UPDATE: return "k_update";
+        case SPH_K_SCAN: return "k_scan";
+        case SPH_K_SCATTER: return "k_scatter";
+        case SPH_K_DENSITY: return "k_density";
+        case SPH_K_ACCEL: return "k_accel";
+        case SPH_K_OUTPUT: return "k_gather_out";
+        case SPH_K_NEIGHBORS: return "k_neighbors";
+    }
+    return "";
 }

@@ -4,7 +4,7 @@
 #include <stdio.h>
 
 enum { CNT_OUT_OF_DOMAIN = 0, CNT_NONFINITE = 1, CNT_PAIRS_DENSITY = 2, CNT_PAIRS_ACCEL = 3,
-       CNT_CANDIDATES = 4, CNT_OVERFLOW = 5, CNT_COUNT = 8 };
+       CNT_CAND_DENSITY = 4, CNT_OVERFLOW = 5, CNT_CAND_ACCEL = 6, CNT_COUNT = 8 };
 
 struct sph_ctx {
     cudaStream_t stream;
@@ -20,11 +20,12 @@ struct sph_ctx {
 
     GridDesc grid;
     PairConsts pc;
-    bool built, have_accel, variable_h;
+    bool built, have_accel, have_arho, variable_h;
     float h_min, h_max;
     int64_t n_keys, max_keys;
 
-    SortedState S[2];          // posh, velm, rp, meta, cell are double-buffered (permute A -> B); acc is shared
+    SortedState S[2];          // double-buffered (permute A -> B); acc is permuted only by sph_nnps_build (inside
+                               // sph_pc_step it is consumed by k_update before the sort and rewritten after it)
     int cur;
     uint32_t *key, *rank;      // per particle, pre-sort order
     uint32_t *cell_count, *cell_start, *block_sums;
@@ -34,6 +35,10 @@ struct sph_ctx {
     float* hminmax;            // device, 2 floats (as ordered ints)
 
     int64_t launches, steps_done;
+    // profiling: event pairs around launches (sph_set_profiling)
+    bool prof_on;
+    struct ProfRec { cudaEvent_t a, b; int id; }* prof;
+    int prof_cap, prof_used; int64_t prof_dropped;
     int64_t last_pairs_density, last_pairs_accel;
     char err[512];
 };
@@ -48,13 +53,17 @@ static inline int sph_fail(sph_ctx* c, int code, const char* msg) {
 }
 
 // launch accounting: every kernel of the library goes through this macro
-#define SPH_LAUNCH(ctx, kernel, grid, block, smem, ...) do { \
+int sph_prof_begin(sph_ctx* c, int id);          // returns the record index or -1
+void sph_prof_end(sph_ctx* c, int rec);
+#define SPH_LAUNCH(ctx, kid, kernel, grid, block, smem, ...) do { \
+    const int rec__ = (ctx)->prof_on ? sph_prof_begin((ctx), (kid)) : -1; \
     kernel<<<(grid), (block), (smem), (ctx)->stream>>>(__VA_ARGS__); (ctx)->launches++; \
+    if (rec__ >= 0) sph_prof_end((ctx), rec__); \
     cudaError_t e__ = cudaPeekAtLastError(); if (e__ != cudaSuccess) { \
         snprintf((ctx)->err, sizeof((ctx)->err), "launch %s: %s", #kernel, cudaGetErrorString(e__)); \
         return SPH_ERR_CUDA; } } while (0)
 
-struct PackSrc { const float *x, *y, *z, *u, *v, *w, *h, *m, *rho, *p; };
+struct PackSrc { const float *x, *y, *z, *u, *v, *w, *h, *m, *rho, *p, *ax, *ay, *az, *arho; };
 struct PackArgs { PackSrc a[SPH_MAX_ARRAYS]; long long base[SPH_MAX_ARRAYS + 1]; int na; };
 struct OutPtrs { float *x, *y, *z, *u, *v, *w, *rho, *p, *ax, *ay, *az, *arho; };
 
@@ -62,7 +71,7 @@ struct OutPtrs { float *x, *y, *z, *u, *v, *w, *rho, *p, *ax, *ay, *az, *arho; }
 int nnps_pack(sph_ctx* c, const PackArgs& A);        // caller SoA -> float4 groups (unsorted) + h_min/h_max
 int nnps_key_hist(sph_ctx* c);                       // key + rank + histogram from S[cur]
 int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey);
-int nnps_sort_from_keys(sph_ctx* c);                 // scan + scatter (key/rank/cell_count filled); swaps buffers
+int nnps_sort_from_keys(sph_ctx* c, bool with_acc);  // scan + scatter (key/rank/cell_count filled); swaps buffers
 int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O);
 int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32_t* indices, int64_t cap,
                           int64_t* total, int mem);

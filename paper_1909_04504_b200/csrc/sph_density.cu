@@ -60,7 +60,7 @@ k_density(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__
         if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
     const unsigned long long h = warp_sum_u64(pol.hits), t = warp_sum_u64(pol.tests);
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CANDIDATES], t); }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CAND_DENSITY], t); }
 }
 
 template <int KERNEL, int DIM>
@@ -74,7 +74,7 @@ static int launch_density_kd(sph_ctx* c, bool merged) {
 #define LD(VARH, MERGED, PER) do { \
         auto kern = k_density<KERNEL, DIM, VARH, MERGED, PER>; \
         SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        SPH_LAUNCH(c, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, c->counters); } while (0)
+        SPH_LAUNCH(c, SPH_K_DENSITY, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, c->counters); } while (0)
     if (c->variable_h) { if (merged) { if (per) LD(true, true, true); else LD(true, true, false); }
                          else        { if (per) LD(true, false, true); else LD(true, false, false); } }
     else               { if (merged) { if (per) LD(false, true, true); else LD(false, true, false); }

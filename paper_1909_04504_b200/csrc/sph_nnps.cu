@@ -39,7 +39,8 @@ k_pack(PackArgs A, SortedState S, int n, PairConsts pc, int* __restrict__ hminma
         S.velm[gidx] = make_float4(s.u ? s.u[i] : 0.0f, s.v ? s.v[i] : 0.0f, s.w ? s.w[i] : 0.0f, s.m ? s.m[i] : 0.0f);
         S.rp[gidx] = make_float2(rho, p / (rho * rho));
         S.meta[gidx] = ((uint32_t)a << SPH_META_IDX_BITS) | (uint32_t)i;
-        S.acc[gidx] = make_float4(0, 0, 0, 0);
+        S.acc[gidx] = make_float4(s.ax ? s.ax[i] : 0.0f, s.ay ? s.ay[i] : 0.0f, s.az ? s.az[i] : 0.0f,
+                                  s.arho ? s.arho[i] : 0.0f);
         hmin = hmax = h;
     }
     for (int o = 16; o > 0; o >>= 1) {
@@ -194,15 +195,15 @@ k_scan_final(const uint32_t* __restrict__ in, long long n, const uint32_t* __res
 static int scan_exclusive(sph_ctx* c, const uint32_t* in, uint32_t* out, long long n) {
     const int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
     if (nb == 0) { SPH_CUDA_OK(c, cudaMemsetAsync(out, 0, sizeof(uint32_t), c->stream)); return SPH_OK; }
-    SPH_LAUNCH(c, k_scan_reduce, nb, SCAN_T, 0, in, n, c->block_sums);
-    SPH_LAUNCH(c, k_scan_blocks, 1, SCAN_T, 0, c->block_sums, nb);
-    SPH_LAUNCH(c, k_scan_final, nb, SCAN_T, 0, in, n, c->block_sums, out, nb);
+    SPH_LAUNCH(c, SPH_K_SCAN, k_scan_reduce, nb, SCAN_T, 0, in, n, c->block_sums);
+    SPH_LAUNCH(c, SPH_K_SCAN, k_scan_blocks, 1, SCAN_T, 0, c->block_sums, nb);
+    SPH_LAUNCH(c, SPH_K_SCAN, k_scan_final, nb, SCAN_T, 0, in, n, c->block_sums, out, nb);
     return SPH_OK;
 }
 
 // a3: gather every persistent property into cell order (double buffer A -> B).
 __global__ void __launch_bounds__(NB)
-k_scatter(SortedState A, SortedState B, int n, int na, const uint32_t* __restrict__ key,
+k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, const uint32_t* __restrict__ key,
           const uint32_t* __restrict__ rank, const uint32_t* __restrict__ cell_start) {
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
@@ -213,12 +214,13 @@ k_scatter(SortedState A, SortedState B, int n, int na, const uint32_t* __restric
     B.rp[d] = A.rp[i];
     B.meta[d] = A.meta[i];
     B.cell[d] = k / (uint32_t)na;
+    if (with_acc) B.acc[d] = A.acc[i];
 }
 
 int nnps_key_hist(sph_ctx* c) {
     const int n = (int)c->n_total;
     SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));
-    if (n) SPH_LAUNCH(c, k_key_hist, (n + NB - 1) / NB, NB, 0, c->grid, c->S[c->cur], n, c->key, c->rank,
+    if (n) SPH_LAUNCH(c, SPH_K_KEY, k_key_hist, (n + NB - 1) / NB, NB, 0, c->grid, c->S[c->cur], n, c->key, c->rank,
                       c->cell_count, c->counters);
     return SPH_OK;
 }
@@ -230,17 +232,17 @@ int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, boo
     U.continuity = continuity; U.rekey = rekey;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
     if (rekey) SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));
-    if (n) SPH_LAUNCH(c, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
+    if (n) SPH_LAUNCH(c, SPH_K_UPDATE, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
                       c->cell_count, c->counters);
     return SPH_OK;
 }
 
-int nnps_sort_from_keys(sph_ctx* c) {
+int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     const int n = (int)c->n_total;
     int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys);
     if (rc) return rc;
-    if (n) SPH_LAUNCH(c, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
-                      c->key, c->rank, c->cell_start);
+    if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
+                      with_acc ? 1 : 0, c->key, c->rank, c->cell_start);
     c->cur ^= 1;
     return SPH_OK;
 }
@@ -266,7 +268,7 @@ k_gather_out(SortedState S, int n, uint32_t array, OutPtrs O) {
 
 int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O) {
     const int n = (int)c->n_total;
-    if (n) SPH_LAUNCH(c, k_gather_out, (n + NB - 1) / NB, NB, 0, c->S[c->cur], n, (uint32_t)array, O);
+    if (n) SPH_LAUNCH(c, SPH_K_OUTPUT, k_gather_out, (n + NB - 1) / NB, NB, 0, c->S[c->cur], n, (uint32_t)array, O);
     return SPH_OK;
 }
 
@@ -327,10 +329,10 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
     SPH_CUDA_OK(c, cudaMemsetAsync(counts, 0, (size_t)(nd + 1) * sizeof(uint32_t), c->stream));
     SortedState& S = c->S[c->cur];
 #define LN(FILL, IDX) do { \
-    if (c->grid.dim == 2) { if (c->variable_h) SPH_LAUNCH(c, (k_neighbors<2, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
-                            else SPH_LAUNCH(c, (k_neighbors<2, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } \
-    else                  { if (c->variable_h) SPH_LAUNCH(c, (k_neighbors<3, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
-                            else SPH_LAUNCH(c, (k_neighbors<3, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
+    if (c->grid.dim == 2) { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<2, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<2, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } \
+    else                  { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<3, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<3, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
     if (n) LN(false, (int32_t*)nullptr);
     int rc = scan_exclusive(c, counts, off32, nd);
     if (rc) return rc;
@@ -343,7 +345,7 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
         SPH_CUDA_OK(c, cudaMalloc(&d_off, (size_t)(nd + 1) * sizeof(int64_t)));
         if (indices && cap >= *total && *total > 0) SPH_CUDA_OK(c, cudaMalloc(&d_idx, (size_t)(*total) * sizeof(int32_t)));
     }
-    SPH_LAUNCH(c, k_widen, (int)((nd + 1 + NB - 1) / NB), NB, 0, off32, d_off, nd + 1);
+    SPH_LAUNCH(c, SPH_K_NEIGHBORS, k_widen, (int)((nd + 1 + NB - 1) / NB), NB, 0, off32, d_off, nd + 1);
     const bool fill = indices && cap >= *total && *total > 0;
     if (fill && n) LN(true, d_idx);
 #undef LN
@@ -363,6 +365,6 @@ int nnps_pack(sph_ctx* c, const PackArgs& A) {
     const int n = (int)c->n_total;
     const int init[2] = { 0x7f7fffff, 0 };
     SPH_CUDA_OK(c, cudaMemcpyAsync(c->hminmax, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
-    if (n) SPH_LAUNCH(c, k_pack, (n + NB - 1) / NB, NB, 0, A, c->S[c->cur], n, c->pc, (int*)c->hminmax);
+    if (n) SPH_LAUNCH(c, SPH_K_PACK, k_pack, (n + NB - 1) / NB, NB, 0, A, c->S[c->cur], n, c->pc, (int*)c->hminmax);
     return SPH_OK;
 }

@@ -54,3 +54,28 @@ def test_one_step_from_the_same_state(O, WL, idx):
     _compare_state(wl, ctx, st, "step1")
     ctx.synchronize()
     ctx.close()
+
+
+def test_restart_from_synced_state_continues_the_run(WL):
+    """sph_sync_state (incl. ax..arho) -> sph_nnps_build with those accelerations -> the next step reuses a^n
+    (no re-evaluation): two steps in one call == step, sync out, rebuild, step."""
+    for wl, mode in ((WL.periodic_box_3d((16, 16, 16), seed=3), "summation"), (WL.dam_break_2d(dx=0.04), "continuity")):
+        ctx, _ = make_ctx(wl)
+        ctx.pc_step(wl.dt, 2, mode)
+        ref = [ctx.sync_state(d) for d in range(len(wl.arrays))]
+        ctx2, arrays = make_ctx(wl)
+        ctx2.pc_step(wl.dt, 1, mode)
+        keys = ("x", "y", "z", "u", "v", "w", "rho", "p", "ax", "ay", "az", "arho")
+        mid = [ctx2.sync_state(d, fields=keys) for d in range(len(wl.arrays))]
+        l0 = ctx2.get_stats().kernel_launches
+        for d, a in enumerate(arrays):
+            mid[d]["h"], mid[d]["m"] = a["h"], a["m"]
+        ctx2.nnps_build(mid, [a.fixed for a in wl.arrays])
+        ctx2.pc_step(wl.dt, 1, mode)
+        for d in range(len(wl.arrays)):
+            got = ctx2.sync_state(d)
+            for k in ("x", "y", "u", "v", "rho"):
+                w_ = ref[d][k].cpu().numpy().astype(np.float64); g_ = got[k].cpu().numpy().astype(np.float64)
+                scale = max(np.abs(w_).max(), 1e-30)
+                assert np.abs(g_ - w_).max() <= TOL * scale, f"{wl.name} {k}[{d}]"
+        ctx.close(); ctx2.close()
