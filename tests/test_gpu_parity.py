@@ -121,6 +121,9 @@ def test_accel_and_continuity_parity(O, case):
             for name, g_, w_ in (("ax", ax, o["au"]), ("ay", ay, o["av"]), ("az", az, o["aw"])):
                 if g_ is None:
                     continue
+                if scale == 0.0:                       # every pair term is exactly 0 (p = 0, u = 0): so must the GPU's be
+                    assert not g_.cpu().numpy().any(), f"{name}[{d}<-{srcs}]: non-zero where every term is 0"
+                    continue
                 err = np.abs(g_.cpu().numpy().astype(np.float64) - w_).max() / scale
                 assert err <= TOL, f"{name}[{d}<-{srcs}]: {err:.3e} of max|a|"
             if np.abs(o["arho"]).max() > 0:
