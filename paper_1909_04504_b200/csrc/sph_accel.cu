@@ -6,8 +6,8 @@
 // Gravity is the initial value of the accumulator (Listing 4).
 #include "sph_pair.cuh"
 
-template <int KERNEL, int DIM, bool VARH, bool PER, bool ARHO>
-struct AccelPolicy : QueuePolicy<AccelPolicy<KERNEL, DIM, VARH, PER, ARHO>> {
+template <int KERNEL, int DIM, bool VARH, bool PER, bool ARHO, bool FILTER>
+struct AccelPolicy : QueuePolicy<AccelPolicy<KERNEL, DIM, VARH, PER, ARHO, FILTER>, FILTER, false> {
     const float4* posh; const float4* velm; const float2* rp;
     float4 pi, vi; float rho_i, pr_i;
     float ax, ay, az, ar;
@@ -49,7 +49,29 @@ struct AccelPolicy : QueuePolicy<AccelPolicy<KERNEL, DIM, VARH, PER, ARHO>> {
 
 // ARHO_ONLY launches serve ContinuityEquation(dest=solid, sources=[fluid]) (Listing 3): the same
 // loop, only arho is stored.
-template <int KERNEL, int DIM, bool VARH, bool MERGED, bool PER, bool ARHO>
+template <class Pol>
+__device__ __forceinline__ void accel_setup(Pol& pol, const GridDesc& g, const PairConsts& pc, const SortedState& S,
+                                            float4 pi, float4 vi, float2 ri) {
+    pol.posh = S.posh; pol.velm = S.velm; pol.rp = S.rp;
+    pol.pi = pi; pol.vi = vi; pol.rho_i = ri.x; pol.pr_i = ri.y;
+    pol.ax = pc.g[0]; pol.ay = pc.g[1]; pol.az = pc.g[2]; pol.ar = 0.0f;
+    pol.Lx = g.L[0]; pol.Ly = g.L[1]; pol.Lz = g.L[2];
+    pol.iLx = 1.0f / g.L[0]; pol.iLy = 1.0f / g.L[1]; pol.iLz = 1.0f / g.L[2];
+    pol.sigma = pc.sigma; pol.h_c = pc.h_const; pol.hinv_c = pc.hinv_const; pol.fac_c = pc.fac_const;
+    pol.visc = pc.visc; pol.eps = pc.eps;
+}
+
+template <int DIM, bool ARHO, class Pol>
+__device__ __forceinline__ void accel_store(const Pol& pol, SortedState& S, int i, int arho_only,
+                                            unsigned long long* counters) {
+    float4 a = S.acc[i];
+    if (arho_only) a.w = pol.ar;
+    else a = make_float4(pol.ax, pol.ay, DIM == 3 ? pol.az : 0.0f, ARHO ? pol.ar : a.w);
+    S.acc[i] = a;
+    if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
+}
+
+template <int KERNEL, int DIM, bool VARH, bool PER, bool ARHO, bool FILTER>
 __global__ void __launch_bounds__(PAIR_BLOCK)
 k_accel(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
         int arho_only, unsigned long long* __restrict__ counters) {
@@ -63,48 +85,85 @@ k_accel(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ c
     const bool active = my_mask != 0u;
     if (!__any_sync(SPH_FULL_MASK, active)) return;
 
-    AccelPolicy<KERNEL, DIM, VARH, PER, ARHO> pol;
-    pol.init(smem_q);
-    pol.posh = S.posh; pol.velm = S.velm; pol.rp = S.rp;
-    pol.pi = pi; pol.vi = vi; pol.rho_i = ri.x; pol.pr_i = ri.y;
-    pol.ax = pc.g[0]; pol.ay = pc.g[1]; pol.az = pc.g[2]; pol.ar = 0.0f;
-    pol.Lx = g.L[0]; pol.Ly = g.L[1]; pol.Lz = g.L[2];
-    pol.iLx = 1.0f / g.L[0]; pol.iLy = 1.0f / g.L[1]; pol.iLz = 1.0f / g.L[2];
-    pol.sigma = pc.sigma; pol.h_c = pc.h_const; pol.hinv_c = pc.hinv_const; pol.fac_c = pc.fac_const;
-    pol.visc = pc.visc; pol.eps = pc.eps;
+    AccelPolicy<KERNEL, DIM, VARH, PER, ARHO, FILTER> pol;
+    pol.init(smem_q, active, S.meta, my_mask);
+    accel_setup(pol, g, pc, S, pi, vi, ri);
 
-    walk_candidates<DIM, VARH, MERGED>(g, pc, S.posh, cell_start, active, pi, ci, my_mask, pol);
+    walk_candidates<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, ci, pol);
     pol.flush();
 
-    if (active) {
-        float4 a = S.acc[i];
-        if (arho_only) a.w = pol.ar;
-        else a = make_float4(pol.ax, pol.ay, DIM == 3 ? pol.az : 0.0f, ARHO ? pol.ar : a.w);
-        S.acc[i] = a;
-        if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
-    }
+    if (active) accel_store<DIM, ARHO>(pol, S, i, arho_only, counters);
     const unsigned long long h = warp_sum_u64(pol.hits), t = warp_sum_u64(pol.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); atomicAdd(&counters[CNT_CAND_ACCEL], t); }
 }
 
+// The same pair body replayed over the neighbour rows recorded by the density pass of this evaluation
+// (sph_density.cu, RECORD): no candidate tests, no queue, no shared memory.  Lane l of the warp that owns
+// sorted particles [32w, 32w+32) reads word l of every row of the warp's blocks (coalesced, streaming).
+#define LIST_BLOCK 128
+template <int KERNEL, int DIM, bool VARH, bool PER, bool ARHO>
+__global__ void __launch_bounds__(LIST_BLOCK)
+k_accel_list(GridDesc g, PairConsts pc, SortedState S, int n, NList nl, unsigned long long* __restrict__ counters) {
+    const int i = blockIdx.x * LIST_BLOCK + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool in = i < n;
+    uint32_t meta = 0; float4 pi = make_float4(0, 0, 0, 1), vi = make_float4(0, 0, 0, 0);
+    float2 ri = make_float2(1, 0);
+    if (in) { meta = S.meta[i]; pi = S.posh[i]; vi = S.velm[i]; ri = S.rp[i]; }
+    const bool active = in && pc.src_mask[meta >> SPH_META_IDX_BITS] != 0u;
+    if (!__any_sync(SPH_FULL_MASK, active)) return;
+
+    AccelPolicy<KERNEL, DIM, VARH, PER, ARHO, false> pol;
+    pol.init(nullptr, active, nullptr, 0u);
+    accel_setup(pol, g, pc, S, pi, vi, ri);
+
+    unsigned long long pairs = 0;
+    uint32_t blk = __ldg(nl.head + (i >> 5));
+    while (blk) {
+        const uint32_t* hdr = nl.pool + (size_t)blk * 32;
+        const uint32_t next = __ldcs(hdr), rows = __ldcs(hdr + 1);
+        const uint32_t* row = hdr + 32 + lane;
+        uint32_t j = rows ? __ldcs(row) : SPH_NL_NONE;
+        for (uint32_t t = 0; t < rows; ++t) {
+            const uint32_t jn = (t + 1 < rows) ? __ldcs(row + (size_t)(t + 1) * 32) : SPH_NL_NONE;   // prefetch
+            if (active && j != SPH_NL_NONE) { pol.body(j); ++pairs; }
+            j = jn;
+        }
+        blk = next;
+    }
+    if (active) accel_store<DIM, ARHO>(pol, S, i, 0, counters);
+    pairs = warp_sum_u64(pairs);
+    if (lane == 0) atomicAdd(&counters[CNT_PAIRS_ACCEL], pairs);
+}
+
 template <int KERNEL, int DIM>
-static int launch_accel_kd(sph_ctx* c, bool merged, bool want_arho, bool arho_only) {
+static int launch_accel_kd(sph_ctx* c, bool filter, bool want_arho, bool arho_only, bool use_list) {
     const int n = (int)c->n_total;
     if (n == 0) return SPH_OK;
-    const int grid = (n + PAIR_BLOCK - 1) / PAIR_BLOCK;
-    const size_t smem = (size_t)PAIR_QCAP * PAIR_BLOCK * sizeof(uint32_t);
     const bool per = c->grid.per[0] || c->grid.per[1] || c->grid.per[2];
     const bool varh = c->variable_h;
     SortedState& S = c->S[c->cur];
+    if (use_list) {
+        const int grid = (n + LIST_BLOCK - 1) / LIST_BLOCK;
+#define LL(VARH, PER, ARHO) SPH_LAUNCH(c, SPH_K_ACCEL_LIST, (k_accel_list<KERNEL, DIM, VARH, PER, ARHO>), grid, LIST_BLOCK, 0, c->grid, c->pc, S, n, c->nl, c->counters)
+#define LL2(VARH, PER) do { if (want_arho) LL(VARH, PER, true); else LL(VARH, PER, false); } while (0)
+        if (varh) { if (per) LL2(true, true); else LL2(true, false); }
+        else      { if (per) LL2(false, true); else LL2(false, false); }
+#undef LL2
+#undef LL
+        return SPH_OK;
+    }
+    const int grid = (n + PAIR_BLOCK - 1) / PAIR_BLOCK;
+    const size_t smem = (size_t)PAIR_QCAP * PAIR_BLOCK * sizeof(uint32_t);
     const int ao = arho_only ? 1 : 0;
-#define LA(VARH, MERGED, PER, ARHO) do { \
-        auto kern = k_accel<KERNEL, DIM, VARH, MERGED, PER, ARHO>; \
+#define LA(VARH, PER, ARHO, FILTER) do { \
+        auto kern = k_accel<KERNEL, DIM, VARH, PER, ARHO, FILTER>; \
         SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
         SPH_LAUNCH(c, SPH_K_ACCEL, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, ao, c->counters); } while (0)
-#define LA2(VARH, MERGED, PER) do { if (want_arho) LA(VARH, MERGED, PER, true); else LA(VARH, MERGED, PER, false); } while (0)
-#define LA3(VARH, MERGED) do { if (per) LA2(VARH, MERGED, true); else LA2(VARH, MERGED, false); } while (0)
-    if (varh) { if (merged) LA3(true, true); else LA3(true, false); }
-    else      { if (merged) LA3(false, true); else LA3(false, false); }
+#define LA2(VARH, PER, ARHO) do { if (filter) LA(VARH, PER, ARHO, true); else LA(VARH, PER, ARHO, false); } while (0)
+#define LA3(VARH, PER) do { if (want_arho) LA2(VARH, PER, true); else LA2(VARH, PER, false); } while (0)
+    if (varh) { if (per) LA3(true, true); else LA3(true, false); }
+    else      { if (per) LA3(false, true); else LA3(false, false); }
 #undef LA3
 #undef LA2
 #undef LA
@@ -112,13 +171,15 @@ static int launch_accel_kd(sph_ctx* c, bool merged, bool want_arho, bool arho_on
 }
 
 int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, bool arho_only) {
-    bool merged = true;
+    bool filter = false, use_list = c->nl_valid && !arho_only;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
-        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) merged = false;
+        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) filter = true;
+        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->nl_mask[a]) use_list = false;   // rows recorded with another mask
     }
+    c->last_used_rows = use_list;
     const int k = c->prm.kernel, d = c->grid.dim;
-#define KD(K, D) if (k == K && d == D) return launch_accel_kd<K, D>(c, merged, want_arho || arho_only, arho_only)
+#define KD(K, D) if (k == K && d == D) return launch_accel_kd<K, D>(c, filter, want_arho || arho_only, arho_only, use_list)
     KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
     KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
     KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);

@@ -62,6 +62,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     if (domain->dim != 2 && domain->dim != 3) return SPH_ERR_BAD_ARG;
     if (params->kernel < 0 || params->kernel > SPH_KERNEL_WENDLAND_C2) return SPH_ERR_BAD_ARG;
     if (!(params->rho0 > 0) || !(params->c0 > 0) || !(params->gamma > 0)) return SPH_ERR_BAD_ARG;
+    if (params->xsub < 0 || params->xsub > 16) return SPH_ERR_BAD_ARG;
     for (int k = 0; k < domain->dim; ++k) if (!(domain->hi[k] > domain->lo[k])) return SPH_ERR_BAD_ARG;
     int64_t tot = 0;
     for (int a = 0; a < n_arrays; ++a) {
@@ -82,12 +83,16 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     c->cap_total = tot;
     default_tables(c);
     set_consts(c);
+    c->xsub = params->xsub ? params->xsub : 4;
+    if (const char* e = getenv("SPH_XSUB")) { int v = atoi(e); if (v >= 1 && v <= 16) c->xsub = v; }   // tuning override
+    int nl_slots = params->nlist_slots ? params->nlist_slots : 192;
+    if (const char* e = getenv("SPH_NLIST_SLOTS")) { int v = atoi(e); if (v != 0) nl_slots = v; }
     *out = c;                                  // so the caller can read sph_last_error / destroy on failure
     SPH_CUDA_OK(c, cudaGetDevice(&c->device));
     SPH_CUDA_OK(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
 
     const size_t N = (size_t)tot + 1;
-    c->max_keys = 4 * tot + 65536; if (c->max_keys > ((int64_t)1 << 26)) c->max_keys = (int64_t)1 << 26;
+    c->max_keys = 8 * tot + 65536; if (c->max_keys > ((int64_t)1 << 26)) c->max_keys = (int64_t)1 << 26;
     for (int b = 0; b < 2; ++b) {
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].posh, N * sizeof(float4)));
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].velm, N * sizeof(float4)));
@@ -105,6 +110,16 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(float)));
     SPH_CUDA_OK(c, cudaMalloc(&c->counters, CNT_COUNT * sizeof(unsigned long long)));
     SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 2 * sizeof(float)));
+    if (nl_slots > 0 && tot > 0) {
+        const size_t warps = (size_t)(tot + 31) / 32;
+        size_t rows = warps * (size_t)nl_slots + 65536;
+        if (rows > 0xfffffff0ull) rows = 0xfffffff0ull;
+        c->nl.pool_rows = (uint32_t)rows;
+        SPH_CUDA_OK(c, cudaMalloc(&c->nl.pool, rows * 32 * sizeof(uint32_t)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->nl.head, (warps + 2) * sizeof(uint32_t)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->nl.used, sizeof(uint32_t)));
+        SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.used, 0, sizeof(uint32_t), c->stream));
+    }
     SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
     for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMemsetAsync(c->S[b].acc, 0, N * sizeof(float4), c->stream));
     SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
@@ -118,6 +133,7 @@ extern "C" int sph_destroy(sph_ctx* c) {
         cudaFree(c->S[b].posh); cudaFree(c->S[b].velm); cudaFree(c->S[b].rp); cudaFree(c->S[b].meta); cudaFree(c->S[b].cell);
     }
     cudaFree(c->S[0].acc); cudaFree(c->S[1].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
+    cudaFree(c->nl.pool); cudaFree(c->nl.head); cudaFree(c->nl.used);
     cudaFree(c->block_sums); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
     for (int k = 0; k < c->prof_cap; ++k) { cudaEventDestroy(c->prof[k].a); cudaEventDestroy(c->prof[k].b); }
     free(c->prof);
@@ -144,6 +160,7 @@ static int size_grid(sph_ctx* c) {
     const double cutoff = kernel_support(c->prm.kernel) * (double)c->h_max;
     if (!(cutoff > 0.0)) return sph_fail(c, SPH_ERR_BAD_ARG, "h_max must be positive");
     double scale = 1.0;
+    int xsub = c->xsub;
     for (int iter = 0; iter < 64; ++iter) {
         int64_t total = 1; bool ok = true;
         for (int k = 0; k < 3; ++k) {
@@ -161,15 +178,22 @@ static int size_grid(sph_ctx* c) {
                     else return sph_fail(c, SPH_ERR_BAD_ARG, "a periodic axis needs at least 3 cells of size k*h_max");
                 }
             }
+            if (k == 0) n *= xsub;
             g.nc[k] = n;
             g.lo[k] = (float)c->dom.lo[k]; g.hi[k] = (float)c->dom.hi[k];
             g.L[k] = (float)(c->dom.hi[k] - c->dom.lo[k]);
             g.inv_cell[k] = (float)(n / L);
+            g.cell[k] = (float)(L / n);
+            // culling margin: 1e-3 cell + 8 ulp of the largest coordinate (rounding of positions, cell
+            // coordinates and slab bounds; the bounds only have to be conservative)
+            const double big = fmax(fmax(fabs(c->dom.lo[k]), fabs(c->dom.hi[k])), L);
+            g.marg[k] = (float)(1.0e-3 * (L / n) + 8.0 * 1.1920929e-7 * big + 4.0e-7 * L);
             total *= n;
         }
+        g.xsub = xsub;
         if (!ok) return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
         if (total * c->na <= c->max_keys) { c->n_keys = total * c->na; return SPH_OK; }
-        scale *= 1.26;
+        if (xsub > 1) xsub /= 2; else scale *= 1.26;
     }
     return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
 }
@@ -179,7 +203,7 @@ static float* stage_field(sph_ctx* c, int field, int array) { return c->staging 
 extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays) {
     if (!c || !arrays) return SPH_ERR_NULL;
     if (n_arrays != c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "n_arrays differs from sph_create");
-    c->built = false; c->have_accel = false; c->have_arho = false;
+    c->built = false; c->have_accel = false; c->have_arho = false; c->nl_valid = false;
     int64_t tot = 0;
     bool all_acc = true, all_arho = true;
     for (int a = 0; a < c->na; ++a) {
@@ -262,7 +286,7 @@ extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask,
     masks[dest] = source_mask;
     int rc = zero_counter(c, CNT_PAIRS_DENSITY); if (rc) return rc;
     rc = zero_counter(c, CNT_CAND_DENSITY); if (rc) return rc;
-    rc = launch_density(c, masks); if (rc) return rc;
+    rc = launch_density(c, masks, true); if (rc) return rc;
     if (rho_out || p_out) { OutPtrs O; memset(&O, 0, sizeof(O)); O.rho = rho_out; O.p = p_out; return emit(c, dest, O, mem); }
     return SPH_OK;
 }
@@ -299,7 +323,20 @@ static int evaluate(sph_ctx* c, bool continuity) {
         return SPH_OK;
     };
     bool all[SPH_MAX_ARRAYS] = { true, true, true, true };
-    if (!continuity) { rc = grouped(c->tbl_density, all, [&](const uint32_t* m) { return launch_density(c, m); }); if (rc) return rc; }
+    if (!continuity) {
+        // a density launch records its neighbour rows when it serves every destination of the momentum pass
+        // with the same source masks (the default tables do): the momentum pass then replays the rows.
+        rc = grouped(c->tbl_density, all, [&](const uint32_t* m) {
+            bool rec = false;
+            for (int a = 0; a < c->na; ++a) if (c->tbl_accel[a]) rec = true;
+            for (int a = 0; a < c->na; ++a) if (c->tbl_accel[a] && m[a] != c->tbl_accel[a]) rec = false;
+            const bool keep = c->nl_valid;                     // rows of an earlier launch of this evaluation
+            uint32_t keep_mask[SPH_MAX_ARRAYS]; memcpy(keep_mask, c->nl_mask, sizeof(keep_mask));
+            int r = launch_density(c, m, rec);
+            if (!rec && keep) { c->nl_valid = true; memcpy(c->nl_mask, keep_mask, sizeof(keep_mask)); }
+            return r; });
+        if (rc) return rc;
+    }
     bool fused[SPH_MAX_ARRAYS], plain[SPH_MAX_ARRAYS], only[SPH_MAX_ARRAYS];
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         const bool acc = a < c->na && c->tbl_accel[a] != 0;
@@ -372,6 +409,7 @@ extern "C" int sph_synchronize(sph_ctx* c) {
     unsigned long long h[CNT_COUNT];
     int rc = read_counters(c, h); if (rc) return rc;
     if (h[CNT_OUT_OF_DOMAIN]) { snprintf(c->err, sizeof(c->err), "%llu particle updates fell outside the non-periodic domain box", h[CNT_OUT_OF_DOMAIN]); return SPH_ERR_OUT_OF_DOMAIN; }
+    if (h[CNT_OVERFLOW]) { snprintf(c->err, sizeof(c->err), "the neighbour-row pool ran out in %llu warps: raise sph_params.nlist_slots (or pass < 0)", h[CNT_OVERFLOW]); return SPH_ERR_CAPACITY; }
     if (h[CNT_NONFINITE]) { snprintf(c->err, sizeof(c->err), "%llu non-finite results", h[CNT_NONFINITE]); return SPH_ERR_NONFINITE; }
     return SPH_OK;
 }
@@ -395,6 +433,15 @@ extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->steps_done = c->steps_done;
     out->variable_h = c->variable_h ? 1 : 0;
     out->h_max = c->h_max;
+    out->xsub = c->grid.xsub;
+    out->used_rows = c->last_used_rows ? 1 : 0;
+    out->nlist_rows_capacity = c->nl.pool_rows;
+    if (c->nl.used) {
+        uint32_t u = 0;
+        SPH_CUDA_OK(c, cudaMemcpyAsync(&u, c->nl.used, sizeof(u), cudaMemcpyDeviceToHost, c->stream));
+        SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+        out->nlist_rows_used = u;
+    }
     return SPH_OK;
 }
 
@@ -452,6 +499,7 @@ extern "C" const char* sph_kernel_name(int id) {
         case SPH_K_ACCEL: return "k_accel";
         case SPH_K_OUTPUT: return "k_gather_out";
         case SPH_K_NEIGHBORS: return "k_neighbors";
+        case SPH_K_ACCEL_LIST: return "k_accel_list";
     }
     return "";
 }

@@ -34,6 +34,13 @@ struct sph_ctx {
     unsigned long long* counters;     // device, CNT_COUNT entries
     float* hminmax;            // device, 2 floats (as ordered ints)
 
+    // neighbour rows recorded by a density launch for the acceleration launch that follows it
+    NList nl;                  // nl.pool == nullptr: recording disabled
+    bool nl_valid;             // rows match the current sort and the masks below
+    uint32_t nl_mask[SPH_MAX_ARRAYS];   // per dest array: the source mask the rows were recorded with (0 = none)
+    bool last_used_rows;       // the last acceleration launch replayed recorded rows
+    int xsub;                  // x sub-cells per support radius requested (GridDesc::xsub is what the grid got)
+
     int64_t launches, steps_done;
     // profiling: event pairs around launches (sph_set_profiling)
     bool prof_on;
@@ -76,5 +83,5 @@ int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O);
 int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32_t* indices, int64_t cap,
                           int64_t* total, int mem);
 // sph_density.cu / sph_accel.cu: one launch serves every dest array whose mask is non-zero
-int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest);
+int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record);
 int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, bool arho_only);

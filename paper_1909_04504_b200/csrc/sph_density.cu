@@ -1,10 +1,11 @@
 // Summation density, eq.3 (L112): rho_i = sum_j m_j W(x_i - x_j, h_ij), with the Tait EOS
 // (eq.6, Listing 4) fused as the epilogue (the group barrier of L337/L382 is the kernel
-// boundary: every p is stored before the acceleration kernel starts).
+// boundary: every p is stored before the acceleration kernel starts).  A RECORD launch also writes the
+// neighbour rows it found, for the acceleration pass of the same evaluation to replay (sph_accel.cu).
 #include "sph_pair.cuh"
 
-template <int KERNEL, int DIM, bool VARH, bool PER>
-struct DensityPolicy : QueuePolicy<DensityPolicy<KERNEL, DIM, VARH, PER>> {
+template <int KERNEL, int DIM, bool VARH, bool PER, bool FILTER, bool RECORD>
+struct DensityPolicy : QueuePolicy<DensityPolicy<KERNEL, DIM, VARH, PER, FILTER, RECORD>, FILTER, RECORD> {
     const float4* posh; const float4* velm;
     float4 pi; float rho;
     float Lx, Ly, Lz, iLx, iLy, iLz;
@@ -30,10 +31,10 @@ struct DensityPolicy : QueuePolicy<DensityPolicy<KERNEL, DIM, VARH, PER>> {
     }
 };
 
-template <int KERNEL, int DIM, bool VARH, bool MERGED, bool PER>
+template <int KERNEL, int DIM, bool VARH, bool PER, bool FILTER, bool RECORD>
 __global__ void __launch_bounds__(PAIR_BLOCK)
 k_density(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
-          unsigned long long* __restrict__ counters) {
+          NList nl, unsigned long long* __restrict__ counters) {
     extern __shared__ uint32_t smem_q[];
     const int i = blockIdx.x * PAIR_BLOCK + threadIdx.x;
     const bool in = i < n;
@@ -43,14 +44,15 @@ k_density(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__
     const bool active = my_mask != 0u;
     if (!__any_sync(SPH_FULL_MASK, active)) return;
 
-    DensityPolicy<KERNEL, DIM, VARH, PER> pol;
-    pol.init(smem_q);
+    DensityPolicy<KERNEL, DIM, VARH, PER, FILTER, RECORD> pol;
+    pol.init(smem_q, active, S.meta, my_mask);
+    pol.nl = nl; pol.counters = counters;
     pol.posh = S.posh; pol.velm = S.velm; pol.pi = pi; pol.rho = 0.0f;
     pol.Lx = g.L[0]; pol.Ly = g.L[1]; pol.Lz = g.L[2];
     pol.iLx = 1.0f / g.L[0]; pol.iLy = 1.0f / g.L[1]; pol.iLz = 1.0f / g.L[2];
     pol.sigma = pc.sigma; pol.hinv_c = pc.hinv_const; pol.fac_c = pc.fac_const;
 
-    walk_candidates<DIM, VARH, MERGED>(g, pc, S.posh, cell_start, active, pi, ci, my_mask, pol);
+    walk_candidates<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, ci, pol);
     pol.flush();
 
     if (active) {
@@ -64,37 +66,50 @@ k_density(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__
 }
 
 template <int KERNEL, int DIM>
-static int launch_density_kd(sph_ctx* c, bool merged) {
+static int launch_density_kd(sph_ctx* c, bool filter, bool record) {
     const int n = (int)c->n_total;
     if (n == 0) return SPH_OK;
     const int grid = (n + PAIR_BLOCK - 1) / PAIR_BLOCK;
     const size_t smem = (size_t)PAIR_QCAP * PAIR_BLOCK * sizeof(uint32_t);
     const bool per = c->grid.per[0] || c->grid.per[1] || c->grid.per[2];
     SortedState& S = c->S[c->cur];
-#define LD(VARH, MERGED, PER) do { \
-        auto kern = k_density<KERNEL, DIM, VARH, MERGED, PER>; \
+#define LD(VARH, PER, FILTER, RECORD) do { \
+        auto kern = k_density<KERNEL, DIM, VARH, PER, FILTER, RECORD>; \
         SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        SPH_LAUNCH(c, SPH_K_DENSITY, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, c->counters); } while (0)
-    if (c->variable_h) { if (merged) { if (per) LD(true, true, true); else LD(true, true, false); }
-                         else        { if (per) LD(true, false, true); else LD(true, false, false); } }
-    else               { if (merged) { if (per) LD(false, true, true); else LD(false, true, false); }
-                         else        { if (per) LD(false, false, true); else LD(false, false, false); } }
+        SPH_LAUNCH(c, SPH_K_DENSITY, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters); } while (0)
+#define LD2(VARH, PER, FILTER) do { if (record) LD(VARH, PER, FILTER, true); else LD(VARH, PER, FILTER, false); } while (0)
+#define LD3(VARH, PER) do { if (filter) LD2(VARH, PER, true); else LD2(VARH, PER, false); } while (0)
+    if (c->variable_h) { if (per) LD3(true, true); else LD3(true, false); }
+    else               { if (per) LD3(false, true); else LD3(false, false); }
+#undef LD3
+#undef LD2
 #undef LD
     return SPH_OK;
 }
 
 // One launch computes rho,p for every array whose src_mask_per_dest entry is non-zero.
-int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest) {
-    bool merged = true;
+int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record) {
+    bool filter = false;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
-        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) merged = false;
+        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) filter = true;
+    }
+    record = record && c->nl.pool != nullptr && c->n_total > 0;
+    c->nl_valid = false;
+    if (record) {
+        SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.head, 0, (size_t)((c->n_total + 31) / 32 + 1) * sizeof(uint32_t), c->stream));
+        SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.used, 0, sizeof(uint32_t), c->stream));
     }
     const int k = c->prm.kernel, d = c->grid.dim;
-#define KD(K, D) if (k == K && d == D) return launch_density_kd<K, D>(c, merged)
+    int rc = sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
+#define KD(K, D) if (k == K && d == D) rc = launch_density_kd<K, D>(c, filter, record)
     KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
     KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
     KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);
 #undef KD
-    return sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
+    if (rc == SPH_OK && record) {
+        c->nl_valid = true;
+        for (int a = 0; a < SPH_MAX_ARRAYS; ++a) c->nl_mask[a] = c->pc.src_mask[a];
+    }
+    return rc;
 }

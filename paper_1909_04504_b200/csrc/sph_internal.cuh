@@ -9,15 +9,32 @@
 #define SPH_META_IDX_MASK ((1u << SPH_META_IDX_BITS) - 1u)
 
 // Uniform cell grid (cells of size >= the support radius; 3^d neighbouring boxes).
+// y and z cells are >= the support radius; every such cell is split into `xsub` sub-cells along x (x is the
+// fastest key digit, so a stencil row is one contiguous run and an x-interval of it is a contiguous sub-run).
 struct GridDesc {
     int dim;
-    int nc[3];                 // cells per axis (nc[2] = 1 in 2-D)
+    int nc[3];                 // cells per axis (nc[2] = 1 in 2-D); nc[0] counts the x SUB-cells
+    int xsub;                  // x sub-cells per support radius
     int per[3];                // periodic per axis
     int na;                    // particle arrays merged into the grid: key = cell * na + array
     float lo[3];               // domain origin
     float inv_cell[3];         // 1 / cell size
     float L[3];                // (float)(hi - lo): the period used by the neighbour predicate (R7)
     float hi[3];
+    float cell[3];             // cell size per axis (x: sub-cell size)
+    float marg[3];             // absolute safety margin of the conservative culling bounds
+};
+
+// Neighbour rows recorded by the density pass and replayed by the acceleration pass.
+// The pool is an array of ROWS of 32 words (one word per lane of the warp that owns the row).  A warp appends
+// BLOCKS: a header row {next block (row index, 0 = end), number of rows} followed by that many rows of sorted
+// particle indices, SPH_NL_NONE where a lane has no entry.
+#define SPH_NL_NONE 0xffffffffu
+struct NList {
+    uint32_t* pool;            // pool_rows * 32 words
+    uint32_t* head;            // per warp of the sorted order: first block (row index), 0 = none
+    uint32_t* used;            // rows handed out so far (row 0 is reserved: allocation returns used + 1)
+    uint32_t pool_rows;
 };
 
 // Per-launch constants of the pair loops.

@@ -15,7 +15,8 @@ __device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, bool& o
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         if (a < g.dim) {
-            if (!g.per[a] && !(x[a] >= g.lo[a] && x[a] <= g.hi[a])) oob = true;   // also catches NaN
+            if (!(x[a] >= g.lo[a] && x[a] <= g.hi[a])) oob = true;   // also catches NaN; periodic axes too:
+                                                                      // the caller's positions must lie in the box
             c[a] = cell_coord(x[a], g.lo[a], g.inv_cell[a], g.nc[a]);
         } else c[a] = 0;
     }
@@ -244,6 +245,7 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
                       with_acc ? 1 : 0, c->key, c->rank, c->cell_start);
     c->cur ^= 1;
+    c->nl_valid = false;                 // recorded neighbour rows index the previous sorted order
     return SPH_OK;
 }
 
@@ -276,14 +278,17 @@ int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O) {
 // neighbour-list export (verification): the same walker and the same predicate as the pair kernels.
 // ------------------------------------------------------------------------------------------------
 struct CountPolicy {
-    uint32_t cnt;
-    __device__ __forceinline__ void hit(uint32_t) { ++cnt; }
+    const uint32_t* meta; uint32_t src; uint32_t cnt;
+    __device__ __forceinline__ void hit(uint32_t j) { if ((meta[j] >> SPH_META_IDX_BITS) == src) ++cnt; }
     __device__ __forceinline__ void pre_chunk() {}
     __device__ __forceinline__ void tested(int) {}
 };
 struct FillPolicy {
-    const uint32_t* meta; int32_t* row; uint32_t cnt;
-    __device__ __forceinline__ void hit(uint32_t j) { row[cnt++] = (int32_t)(meta[j] & SPH_META_IDX_MASK); }
+    const uint32_t* meta; uint32_t src; int32_t* row; uint32_t cnt;
+    __device__ __forceinline__ void hit(uint32_t j) {
+        const uint32_t m = meta[j];
+        if ((m >> SPH_META_IDX_BITS) == src) row[cnt++] = (int32_t)(m & SPH_META_IDX_MASK);
+    }
     __device__ __forceinline__ void pre_chunk() {}
     __device__ __forceinline__ void tested(int) {}
 };
@@ -301,12 +306,12 @@ k_neighbors(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict
     if (!__any_sync(SPH_FULL_MASK, active)) return;
     const uint32_t o = meta & SPH_META_IDX_MASK;
     if (!FILL) {
-        CountPolicy pol; pol.cnt = 0;
-        walk_candidates<DIM, VARH, false>(g, pc, S.posh, cell_start, active, pi, ci, 1u << src, pol);
+        CountPolicy pol; pol.meta = S.meta; pol.src = src; pol.cnt = 0;
+        walk_candidates<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, ci, pol);
         if (active) counts[o] = pol.cnt;
     } else {
-        FillPolicy pol; pol.meta = S.meta; pol.cnt = 0; pol.row = indices + (active ? offsets[o] : 0u);
-        walk_candidates<DIM, VARH, false>(g, pc, S.posh, cell_start, active, pi, ci, 1u << src, pol);
+        FillPolicy pol; pol.meta = S.meta; pol.src = src; pol.cnt = 0; pol.row = indices + (active ? offsets[o] : 0u);
+        walk_candidates<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, ci, pol);
         if (active) {                                   // rows ascending (insertion sort; rows are short)
             int32_t* r = pol.row; const int m = (int)pol.cnt;
             for (int a = 1; a < m; ++a) { int32_t v = r[a]; int b = a - 1; while (b >= 0 && r[b] > v) { r[b + 1] = r[b]; --b; } r[b + 1] = v; }

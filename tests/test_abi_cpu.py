@@ -33,21 +33,22 @@ def test_header_symbols_are_exported(lib):
     for n in names:
         assert hasattr(lib, n), f"{n} declared in sph.h but not exported"
     assert sorted(binding.EXPORTS) == names
-    assert lib.sph_abi_version() == 1
+    assert lib.sph_abi_version() == 2
 
 
 def test_struct_layouts_match_the_c_compiler(tmp_path):
     from paper_1909_04504_b200 import binding
     prog = tmp_path / "sz.c"
-    prog.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "sph.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu %zu\\n",'
+    prog.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "sph.h"\nint main(void){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",'
                     'sizeof(sph_domain),sizeof(sph_params),sizeof(sph_array),sizeof(sph_stats),'
-                    'offsetof(sph_array,x),offsetof(sph_params,g),offsetof(sph_stats,h_max));return 0;}\n')
+                    'offsetof(sph_array,x),offsetof(sph_params,g),offsetof(sph_stats,h_max),offsetof(sph_params,nlist_slots),offsetof(sph_stats,nlist_rows_capacity));return 0;}\n')
     exe = tmp_path / "sz"
     subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(prog), "-o", str(exe)])
     got = [int(v) for v in subprocess.check_output([str(exe)]).split()]
     want = [C.sizeof(binding.sph_domain), C.sizeof(binding.sph_params), C.sizeof(binding.sph_array),
             C.sizeof(binding.sph_stats), binding.sph_array.x.offset, binding.sph_params.g.offset,
-            binding.sph_stats.h_max.offset]
+            binding.sph_stats.h_max.offset, binding.sph_params.nlist_slots.offset,
+            binding.sph_stats.nlist_rows_capacity.offset]
     assert got == want
 
 
