@@ -13,7 +13,7 @@ from typing import Dict, List, Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsph_b200.so")
+LIB_PATH = os.environ.get("SPH_B200_LIB") or os.path.join(_HERE, "libsph_b200.so")
 
 SPH_MAX_ARRAYS = 4
 KERNEL_ID = {"cubic": 0, "quintic": 1, "wendland_c2": 2}

@@ -15,8 +15,11 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-LIB = os.path.join(HERE, "libsph_b200.so")
-OBJ = os.path.join(HERE, "build")
+# SPH_B200_LIB / SPH_B200_NVCC_FLAGS: build (and load, see binding.py) a tuning variant beside the default library
+LIB = os.environ.get("SPH_B200_LIB") or os.path.join(HERE, "libsph_b200.so")
+EXTRA = os.environ.get("SPH_B200_NVCC_FLAGS", "").split()
+OBJ = os.path.join(HERE, "build" if not os.environ.get("SPH_B200_LIB") else
+                   "build_" + hashlib.sha256(LIB.encode()).hexdigest()[:8])
 SOURCES = ["sph_api.cu", "sph_nnps.cu", "sph_density.cu", "sph_accel.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
@@ -36,7 +39,7 @@ def _digest() -> str:
         p = os.path.normpath(os.path.join(CSRC, n))
         if os.path.isfile(p):
             h.update(n.encode()); h.update(open(p, "rb").read())
-    h.update(" ".join(ARCH + FLAGS).encode())
+    h.update(" ".join(ARCH + FLAGS + EXTRA).encode())
     return h.hexdigest()
 
 
@@ -50,7 +53,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src: str) -> str:
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
-        cmd = [nvcc, *ARCH, *FLAGS, "-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc, *ARCH, *FLAGS, *EXTRA, "-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]
         r = subprocess.run(cmd, capture_output=True, text=True)

@@ -159,6 +159,7 @@ static int launch_accel_kd(sph_ctx* c, bool filter, bool want_arho, bool arho_on
 #define LA(VARH, PER, ARHO, FILTER) do { \
         auto kern = k_accel<KERNEL, DIM, VARH, PER, ARHO, FILTER>; \
         SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        if (c->carveout >= 0) SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, c->carveout)); \
         SPH_LAUNCH(c, SPH_K_ACCEL, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, ao, c->counters); } while (0)
 #define LA2(VARH, PER, ARHO) do { if (filter) LA(VARH, PER, ARHO, true); else LA(VARH, PER, ARHO, false); } while (0)
 #define LA3(VARH, PER) do { if (want_arho) LA2(VARH, PER, true); else LA2(VARH, PER, false); } while (0)

@@ -76,6 +76,7 @@ static int launch_density_kd(sph_ctx* c, bool filter, bool record) {
 #define LD(VARH, PER, FILTER, RECORD) do { \
         auto kern = k_density<KERNEL, DIM, VARH, PER, FILTER, RECORD>; \
         SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        if (c->carveout >= 0) SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, c->carveout)); \
         SPH_LAUNCH(c, SPH_K_DENSITY, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters); } while (0)
 #define LD2(VARH, PER, FILTER) do { if (record) LD(VARH, PER, FILTER, true); else LD(VARH, PER, FILTER, false); } while (0)
 #define LD3(VARH, PER) do { if (filter) LD2(VARH, PER, true); else LD2(VARH, PER, false); } while (0)

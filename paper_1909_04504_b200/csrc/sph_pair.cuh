@@ -21,9 +21,20 @@
 #include <type_traits>
 
 #define PAIR_BLOCK 128
-#define PAIR_QCAP 64              // power of two
-#define PAIR_CHUNK 16
+#ifndef PAIR_QCAP
+#define PAIR_QCAP 64              // queue slots per thread, power of two
+#endif
+#ifndef PAIR_CHUNK
+#define PAIR_CHUNK 16             // candidates tested between two queue-level checks
+#endif
+#ifndef PAIR_MIN_DRAIN
 #define PAIR_MIN_DRAIN 16
+#endif
+#define PAIR_QSTRIDE (PAIR_BLOCK * 4u)                 // bytes between two slots of one thread
+#define PAIR_QBYTES_MASK (PAIR_QCAP * PAIR_QSTRIDE - 1u)
+
+__device__ __forceinline__ void sts_u32(uint32_t saddr, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" :: "r"(saddr), "r"(v) : "memory"); }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t saddr) { uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory"); return v; }
 
 // Walks all candidate runs of one destination particle.  Every lane of the warp must call this (inactive
 // lanes pass active = false) because the run loops are warp-uniform and use warp votes.
@@ -134,20 +145,22 @@ __device__ __forceinline__ float min_image(float d, float L, float invL) {
 // RECORD: drained rows are appended to the neighbour-row pool.
 template <class Derived, bool FILTER, bool RECORD>
 struct QueuePolicy {
-    uint32_t* q;               // shared memory, already offset by threadIdx.x
-    int head, cnt;
+    uint32_t qaddr;            // shared-space address of this thread's slot 0
+    uint32_t rpos, wpos;       // byte offsets (multiples of PAIR_QSTRIDE, unmasked) of the read / write slot
+    int cnt;
     bool is_active;
     unsigned long long hits, tests;
     const uint32_t* meta; uint32_t src_mask;      // FILTER
     NList nl; uint32_t prev_hdr; bool rec_ok; unsigned long long* counters;   // RECORD
 
     __device__ __forceinline__ void init(uint32_t* smem, bool active, const uint32_t* meta_, uint32_t mask_) {
-        q = smem + threadIdx.x; head = 0; cnt = 0; hits = 0; tests = 0; is_active = active;
+        qaddr = (uint32_t)__cvta_generic_to_shared(smem + threadIdx.x); rpos = 0; wpos = 0; cnt = 0;
+        hits = 0; tests = 0; is_active = active;
         meta = meta_; src_mask = mask_; prev_hdr = 0; rec_ok = RECORD; counters = nullptr;
     }
     __device__ __forceinline__ void hit(uint32_t j) {
         if (FILTER) { if (!((src_mask >> (__ldg(meta + j) >> SPH_META_IDX_BITS)) & 1u)) return; }
-        q[((head + cnt) & (PAIR_QCAP - 1)) * PAIR_BLOCK] = j; ++cnt;
+        sts_u32(qaddr + (wpos & PAIR_QBYTES_MASK), j); wpos += PAIR_QSTRIDE; ++cnt;
     }
     __device__ __forceinline__ void tested(int len) { tests += (unsigned)len; }
 
@@ -177,11 +190,11 @@ struct QueuePolicy {
 #pragma unroll 2
         for (int t = 0; t < T; ++t) {
             uint32_t j = SPH_NL_NONE;
-            if (t < mine) { j = q[((head + t) & (PAIR_QCAP - 1)) * PAIR_BLOCK]; static_cast<Derived*>(this)->body(j); }
+            if (t < mine) { j = lds_u32(qaddr + ((rpos + (uint32_t)t * PAIR_QSTRIDE) & PAIR_QBYTES_MASK)); static_cast<Derived*>(this)->body(j); }
             if (RECORD && rec_ok) nl.pool[row0 + (size_t)t * 32] = j;
         }
         hits += (unsigned)mine;
-        head = (head + mine) & (PAIR_QCAP - 1); cnt -= mine;
+        rpos += (uint32_t)mine * PAIR_QSTRIDE; cnt -= mine;
     }
     __device__ __forceinline__ void pre_chunk() {
         const int maxc = __reduce_max_sync(SPH_FULL_MASK, cnt);
