@@ -213,6 +213,12 @@ const char* sph_kernel_name(int kernel_id);
 int sph_get_stats(sph_ctx* ctx, sph_stats* out);                                         /* [sync] */
 int sph_synchronize(sph_ctx* ctx);   /* [sync] waits for the stream and reports pending device-side errors */
 
+/* Diagnostic, not a step of the path: sustained FP32 fused-multiply-add rate of this GPU, scalar (packed == 0,
+ * FFMA) or packed (packed != 0, FFMA2), over `iters` iterations of 16 independent accumulators per thread on
+ * 8 blocks of 256 threads per SM.  *tflops counts 2 flop per lane FMA; *ms (nullable) is the best of 3 timed
+ * launches.  It is the measured denominator of the pair kernels' ALU roofline.  [sync] */
+int sph_fp32_probe(sph_ctx* ctx, int packed, int iters, double* tflops, double* ms);
+
 const char* sph_strerror(int code);
 const char* sph_last_error(const sph_ctx* ctx);
 int sph_abi_version(void);

@@ -25,7 +25,7 @@ ARRAY_DYNAMIC, ARRAY_FIXED = 0, 1
 EXPORTS = ["sph_create", "sph_destroy", "sph_set_tables", "sph_nnps_build", "sph_summation_density",
            "sph_wcsph_accel", "sph_pc_step", "sph_sync_state", "sph_get_accel", "sph_nnps_get_neighbors",
            "sph_get_stats", "sph_synchronize", "sph_strerror", "sph_last_error", "sph_abi_version",
-           "sph_set_profiling", "sph_get_profile", "sph_kernel_name"]
+           "sph_set_profiling", "sph_get_profile", "sph_kernel_name", "sph_fp32_probe"]
 
 _FP = C.POINTER(C.c_float)
 FIELD_NAMES = ("x", "y", "z", "u", "v", "w", "h", "m", "rho", "p", "ax", "ay", "az", "arho")
@@ -93,6 +93,7 @@ def load() -> C.CDLL:
         L.sph_set_profiling.argtypes = [vp, i32]
         L.sph_get_profile.argtypes = [vp, C.POINTER(sph_profile)]
         L.sph_kernel_name.argtypes = [i32]; L.sph_kernel_name.restype = C.c_char_p
+        L.sph_fp32_probe.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.sph_strerror.argtypes = [i32]; L.sph_strerror.restype = C.c_char_p
         L.sph_last_error.argtypes = [vp]; L.sph_last_error.restype = C.c_char_p
         for name in EXPORTS:
@@ -262,6 +263,12 @@ class SphContext:
 
     def set_profiling(self, enable: bool):
         self._check(self.L.sph_set_profiling(self.ctx, int(bool(enable))))
+
+    def fp32_probe(self, packed: bool, iters: int = 4096):
+        """(TFLOP/s, ms) of the FP32 FMA issue-rate probe (diagnostic; the ALU roofline denominator)."""
+        tf, ms = C.c_double(0.0), C.c_double(0.0)
+        self._check(self.L.sph_fp32_probe(self.ctx, int(bool(packed)), int(iters), C.byref(tf), C.byref(ms)))
+        return tf.value, ms.value
 
     def get_profile(self) -> Dict[str, Dict[str, float]]:
         """{kernel name: {"launches": n, "ms": summed device time}} since set_profiling(True)."""

@@ -20,7 +20,7 @@ LIB = os.environ.get("SPH_B200_LIB") or os.path.join(HERE, "libsph_b200.so")
 EXTRA = os.environ.get("SPH_B200_NVCC_FLAGS", "").split()
 OBJ = os.path.join(HERE, "build" if not os.environ.get("SPH_B200_LIB") else
                    "build_" + hashlib.sha256(LIB.encode()).hexdigest()[:8])
-SOURCES = ["sph_api.cu", "sph_nnps.cu", "sph_density.cu", "sph_accel.cu"]
+SOURCES = ["sph_api.cu", "sph_nnps.cu", "sph_density.cu", "sph_accel.cu", "sph_probe.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 

@@ -85,6 +85,8 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     set_consts(c);
     c->xsub = params->xsub ? params->xsub : 4;
     if (const char* e = getenv("SPH_XSUB")) { int v = atoi(e); if (v >= 1 && v <= 16) c->xsub = v; }   // tuning override
+    c->tile = true;
+    if (const char* e = getenv("SPH_PAIR")) c->tile = strcmp(e, "thread") != 0;                       // tuning override
     c->carveout = -1;
     if (const char* e = getenv("SPH_CARVEOUT")) c->carveout = atoi(e);                                  // tuning override
     int nl_slots = params->nlist_slots ? params->nlist_slots : 192;

@@ -55,7 +55,9 @@ struct PairConsts {
 
 // Cell-sorted particle state (struct of float4 groups: one 16-B vector load per candidate test).
 struct SortedState {
-    float4* posh;              // x, y, z, h
+    float4* posh;              // x, y, z, h  -- after the sort, when h is constant (h_min == h_max, the kernels
+                               // then take h from PairConsts), .w carries the MASS instead: the density pair
+                               // loop gathers one 16-byte word per neighbour (k_scatter, w_mass)
     float4* velm;              // u, v, w, m
     float2* rp;                // rho, p / rho^2   (p itself is returned as (p/rho^2) * rho^2)
     float4* acc;               // ax, ay, az, arho

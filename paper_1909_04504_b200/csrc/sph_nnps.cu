@@ -2,7 +2,7 @@
 // every property into cell order; the fused predictor-corrector update (eqs. 12-14) that feeds it;
 // the caller-order output gathers; and the neighbour-list export used for the bit-exact set parity.
 // All of these stream each particle once: they are HBM-bandwidth kernels.
-#include "sph_pair.cuh"
+#include "sph_tile.cuh"
 
 #define NB 256
 
@@ -204,14 +204,17 @@ static int scan_exclusive(sph_ctx* c, const uint32_t* in, uint32_t* out, long lo
 
 // a3: gather every persistent property into cell order (double buffer A -> B).
 __global__ void __launch_bounds__(NB)
-k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, const uint32_t* __restrict__ key,
+k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass, const uint32_t* __restrict__ key,
           const uint32_t* __restrict__ rank, const uint32_t* __restrict__ cell_start) {
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
     const uint32_t k = key[i];
     const uint32_t d = cell_start[k] + rank[i];
-    B.posh[d] = A.posh[i];
-    B.velm[d] = A.velm[i];
+    float4 p = A.posh[i];
+    const float4 v = A.velm[i];
+    if (w_mass) p.w = v.w;                      // constant h: posh.w of the sorted state carries the mass
+    B.posh[d] = p;
+    B.velm[d] = v;
     B.rp[d] = A.rp[i];
     B.meta[d] = A.meta[i];
     B.cell[d] = k / (uint32_t)na;
@@ -243,7 +246,7 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys);
     if (rc) return rc;
     if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
-                      with_acc ? 1 : 0, c->key, c->rank, c->cell_start);
+                      with_acc ? 1 : 0, c->variable_h ? 0 : 1, c->key, c->rank, c->cell_start);
     c->cur ^= 1;
     c->nl_valid = false;                 // recorded neighbour rows index the previous sorted order
     return SPH_OK;
@@ -319,6 +322,42 @@ k_neighbors(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict
     }
 }
 
+// the same export through the warp-tile walker (the predicate code the tile pair kernels run)
+template <int DIM, bool VARH, bool FILL>
+__global__ void __launch_bounds__(TILE_BLOCK)
+k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
+                 uint32_t dest, uint32_t src, uint32_t* __restrict__ counts, const uint32_t* __restrict__ offsets,
+                 int32_t* __restrict__ indices) {
+    __shared__ TileWarpSmem smem[TILE_WARPS];
+    TileWarpSmem& ws = smem[threadIdx.x >> 5];
+    const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
+    const bool in = i < n;
+    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
+    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; }
+    const bool active = in && (meta >> SPH_META_IDX_BITS) == dest;
+    if (!__any_sync(SPH_FULL_MASK, active)) return;
+    const uint32_t o = meta & SPH_META_IDX_MASK;
+    const int row = in ? (int)(ci / (uint32_t)g.nc[0]) : -1;
+    const int sub = in ? (int)(ci % (uint32_t)g.nc[0]) : 0;
+    uint32_t cnt = 0;
+    int32_t* out = FILL ? indices + (active ? offsets[o] : 0u) : nullptr;
+    auto load = [&](uint32_t j) { return __ldg(S.meta + j); };
+    auto compute = [&](const uint32_t& m) {
+        if ((m >> SPH_META_IDX_BITS) != src) return;
+        if (FILL) out[cnt] = (int32_t)(m & SPH_META_IDX_MASK);
+        ++cnt;
+    };
+    TileState st; st.reset(); st.tests = 0;
+    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st,
+                         [&]() { tile_drain<uint32_t>(ws, st.nz, load, compute); st.reset(); });
+    if (!active) return;
+    if (!FILL) counts[o] = cnt;
+    else {                                              // rows ascending (insertion sort; rows are short)
+        const int m = (int)cnt;
+        for (int a = 1; a < m; ++a) { int32_t v = out[a]; int b = a - 1; while (b >= 0 && out[b] > v) { out[b + 1] = out[b]; --b; } out[b + 1] = v; }
+    }
+}
+
 __global__ void k_widen(const uint32_t* __restrict__ in, int64_t* __restrict__ out, long long n) {
     const long long i = (long long)blockIdx.x * NB + threadIdx.x;
     if (i < n) out[i] = (int64_t)in[i];
@@ -333,11 +372,12 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
     const int grid = (n + NB - 1) / NB;
     SPH_CUDA_OK(c, cudaMemsetAsync(counts, 0, (size_t)(nd + 1) * sizeof(uint32_t), c->stream));
     SortedState& S = c->S[c->cur];
-#define LN(FILL, IDX) do { \
-    if (c->grid.dim == 2) { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<2, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
-                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<2, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } \
-    else                  { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<3, true, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
-                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors<3, false, FILL>), grid, NB, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
+#define LNK(K, GRID, BLOCK, FILL, IDX) do { \
+    if (c->grid.dim == 2) { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<2, true, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<2, false, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } \
+    else                  { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<3, true, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<3, false, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
+#define LN(FILL, IDX) do { if (c->tile) LNK(k_neighbors_tile, (n + TILE_BLOCK - 1) / TILE_BLOCK, TILE_BLOCK, FILL, IDX); else LNK(k_neighbors, grid, NB, FILL, IDX); } while (0)
     if (n) LN(false, (int32_t*)nullptr);
     int rc = scan_exclusive(c, counts, off32, nd);
     if (rc) return rc;
@@ -354,6 +394,7 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
     const bool fill = indices && cap >= *total && *total > 0;
     if (fill && n) LN(true, d_idx);
 #undef LN
+#undef LNK
     if (mem == SPH_MEM_HOST) {
         SPH_CUDA_OK(c, cudaMemcpyAsync(offsets, d_off, (size_t)(nd + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
         if (fill) SPH_CUDA_OK(c, cudaMemcpyAsync(indices, d_idx, (size_t)(*total) * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));

@@ -23,7 +23,7 @@ def lib():
 def _declared():
     src = open(HEADER).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(sph_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(sph_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_symbols_are_exported(lib):
