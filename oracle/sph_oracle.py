@@ -147,10 +147,21 @@ def neighbors(wl, dest: Dict[str, np.ndarray], src: Dict[str, np.ndarray], pred3
     return off, idx[:int(total)]
 
 
-def density(wl, st: State, dest: int, sources: Sequence[int], pred32: bool = True, method: str = "cell"):
-    """eq.3: returns (rho, abs_sum, n_pairs) for array `dest` summed over `sources` in order."""
+def _dest(st: State, dest: int, subset):
+    """Destination fields of array `dest`, or of the particles `subset` (index array) of it: the sums are per
+    destination particle, so a subset of destinations against ALL sources gives those particles' full sums."""
+    D = st.arrays[dest]
+    if subset is None:
+        return D
+    idx = np.asarray(subset, dtype=np.int64)
+    return {k: (np.ascontiguousarray(v[idx]) if isinstance(v, np.ndarray) else v) for k, v in D.items()}
+
+
+def density(wl, st: State, dest: int, sources: Sequence[int], pred32: bool = True, method: str = "cell",
+            subset=None):
+    """eq.3: returns (rho, abs_sum, n_pairs) for array `dest` (or its particles `subset`) summed over `sources`."""
     L = lib(); dom = _domain(wl); kid = KERNEL_ID[wl.kernel]
-    D = st.arrays[dest]; nd = len(D["x"])
+    D = _dest(st, dest, subset); nd = len(D["x"])
     rho = np.zeros(nd); ab = np.zeros(nd); npairs = np.zeros(1, dtype=np.int64)
     for s in sources:
         S = st.arrays[s]
@@ -169,11 +180,11 @@ def eos(wl, rho: np.ndarray) -> np.ndarray:
 
 
 def accel(wl, st: State, dest: int, sources: Sequence[int], pred32: bool = True, method: str = "cell",
-          gravity: bool = True, alpha: Optional[float] = None):
+          gravity: bool = True, alpha: Optional[float] = None, subset=None):
     """eq.8-9 + Pi_ij (+ eq.7): dict(au,av,aw,arho,abs_a,abs_arho,visc_power,n_pairs) for array `dest`.
     The accumulators start at g (Listing 4: gravity is the initial value) and arho at 0 (L402-403)."""
     L = lib(); dom = _domain(wl); kid = KERNEL_ID[wl.kernel]
-    D = st.arrays[dest]; nd = len(D["x"])
+    D = _dest(st, dest, subset); nd = len(D["x"])
     g = wl.g if gravity else (0.0, 0.0, 0.0)
     out = {k: np.full(nd, float(g[i])) for i, k in enumerate(("au", "av", "aw"))}
     for k in ("arho", "abs_a", "abs_arho", "visc_power"):

@@ -253,6 +253,14 @@ class SphContext:
                                                   total.value, C.byref(total), MEM_HOST))
         return off, idx[:total.value]
 
+    def neighbor_counts(self, dest: int, src: int):
+        """|N_src(i)| for every particle i of `dest` (the counting pass of the verification export only)."""
+        n = self.n[dest]
+        off = np.zeros(n + 1, dtype=np.int64)
+        total = C.c_int64(0)
+        self._check(self.L.sph_nnps_get_neighbors(self.ctx, dest, src, off.ctypes.data, None, 0, C.byref(total), MEM_HOST))
+        return np.diff(off)
+
     def get_stats(self) -> sph_stats:
         s = sph_stats()
         self._check(self.L.sph_get_stats(self.ctx, C.byref(s)))

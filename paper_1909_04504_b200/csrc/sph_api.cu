@@ -85,10 +85,6 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     set_consts(c);
     c->xsub = params->xsub ? params->xsub : 4;
     if (const char* e = getenv("SPH_XSUB")) { int v = atoi(e); if (v >= 1 && v <= 16) c->xsub = v; }   // tuning override
-    c->tile = true;
-    if (const char* e = getenv("SPH_PAIR")) c->tile = strcmp(e, "thread") != 0;                       // tuning override
-    c->carveout = -1;
-    if (const char* e = getenv("SPH_CARVEOUT")) c->carveout = atoi(e);                                  // tuning override
     int nl_slots = params->nlist_slots ? params->nlist_slots : 192;
     if (const char* e = getenv("SPH_NLIST_SLOTS")) { int v = atoi(e); if (v != 0) nl_slots = v; }
     *out = c;                                  // so the caller can read sph_last_error / destroy on failure

@@ -39,8 +39,6 @@ struct sph_ctx {
     bool nl_valid;             // rows match the current sort and the masks below
     uint32_t nl_mask[SPH_MAX_ARRAYS];   // per dest array: the source mask the rows were recorded with (0 = none)
     bool last_used_rows;       // the last acceleration launch replayed recorded rows
-    bool tile;                 // pair passes use the warp-tile kernels (sph_tile.cuh); false: thread-per-particle walker
-    int carveout;              // preferred shared-memory carve-out (percent) of the queue kernels, -1 = driver default
     int xsub;                  // x sub-cells per support radius requested (GridDesc::xsub is what the grid got)
 
     int64_t launches, steps_done;

@@ -1,96 +1,9 @@
 // Summation density, eq.3 (L112): rho_i = sum_j m_j W(x_i - x_j, h_ij), with the Tait EOS
 // (eq.6, Listing 4) fused as the epilogue (the group barrier of L337/L382 is the kernel
 // boundary: every p is stored before the acceleration kernel starts).  A RECORD launch also writes the
-// neighbour rows it found, for the acceleration pass of the same evaluation to replay (sph_accel.cu).
+// hit masks of its candidate tests (sph_tile.cuh), for the acceleration pass of the same evaluation to replay.
 #include "sph_tile.cuh"
 
-template <int KERNEL, int DIM, bool VARH, bool PER, bool FILTER, bool RECORD>
-struct DensityPolicy : QueuePolicy<DensityPolicy<KERNEL, DIM, VARH, PER, FILTER, RECORD>, FILTER, RECORD> {
-    const float4* posh; const float4* velm;
-    float4 pi; float rho;
-    float Lx, Ly, Lz, iLx, iLy, iLz;
-    float sigma, hinv_c, fac_c;
-
-    __device__ __forceinline__ void body(uint32_t j) {
-        const float4 pj = __ldg(posh + j);
-        const float mj = __ldg(&velm[j].w);
-        const float dx = min_image<PER>(pi.x - pj.x, Lx, iLx);
-        const float dy = min_image<PER>(pi.y - pj.y, Ly, iLy);
-        float r2 = fmaf(dy, dy, dx * dx);
-        if (DIM == 3) { const float dz = min_image<PER>(pi.z - pj.z, Lz, iLz); r2 = fmaf(dz, dz, r2); }
-        const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;
-        const float r = r2 * rinv;
-        float hinv, fac;
-        if (VARH) {
-            hinv = rcp_approx(0.5f * (pi.w + pj.w));
-            fac = sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
-        } else { hinv = hinv_c; fac = fac_c; }
-        float f, df;
-        kernel_profile<KERNEL, DIM>(r * hinv, f, df);
-        rho = fmaf(mj * fac, f, rho);
-    }
-};
-
-template <int KERNEL, int DIM, bool VARH, bool PER, bool FILTER, bool RECORD>
-__global__ void __launch_bounds__(PAIR_BLOCK)
-k_density(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
-          NList nl, unsigned long long* __restrict__ counters) {
-    extern __shared__ uint32_t smem_q[];
-    const int i = blockIdx.x * PAIR_BLOCK + threadIdx.x;
-    const bool in = i < n;
-    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
-    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; }
-    const uint32_t my_mask = in ? pc.src_mask[meta >> SPH_META_IDX_BITS] : 0u;
-    const bool active = my_mask != 0u;
-    if (!__any_sync(SPH_FULL_MASK, active)) return;
-
-    DensityPolicy<KERNEL, DIM, VARH, PER, FILTER, RECORD> pol;
-    pol.init(smem_q, active, S.meta, my_mask);
-    pol.nl = nl; pol.counters = counters;
-    pol.posh = S.posh; pol.velm = S.velm; pol.pi = pi; pol.rho = 0.0f;
-    pol.Lx = g.L[0]; pol.Ly = g.L[1]; pol.Lz = g.L[2];
-    pol.iLx = 1.0f / g.L[0]; pol.iLy = 1.0f / g.L[1]; pol.iLz = 1.0f / g.L[2];
-    pol.sigma = pc.sigma; pol.hinv_c = pc.hinv_const; pol.fac_c = pc.fac_const;
-
-    walk_candidates<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, ci, pol);
-    pol.flush();
-
-    if (active) {
-        const float rho = pol.rho;
-        const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
-        S.rp[i] = make_float2(rho, p / (rho * rho));
-        if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
-    }
-    const unsigned long long h = warp_sum_u64(pol.hits), t = warp_sum_u64(pol.tests);
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CAND_DENSITY], t); }
-}
-
-template <int KERNEL, int DIM>
-static int launch_density_kd(sph_ctx* c, bool filter, bool record) {
-    const int n = (int)c->n_total;
-    if (n == 0) return SPH_OK;
-    const int grid = (n + PAIR_BLOCK - 1) / PAIR_BLOCK;
-    const size_t smem = (size_t)PAIR_QCAP * PAIR_BLOCK * sizeof(uint32_t);
-    const bool per = c->grid.per[0] || c->grid.per[1] || c->grid.per[2];
-    SortedState& S = c->S[c->cur];
-#define LD(VARH, PER, FILTER, RECORD) do { \
-        auto kern = k_density<KERNEL, DIM, VARH, PER, FILTER, RECORD>; \
-        SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        if (c->carveout >= 0) SPH_CUDA_OK(c, cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, c->carveout)); \
-        SPH_LAUNCH(c, SPH_K_DENSITY, kern, grid, PAIR_BLOCK, smem, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters); } while (0)
-#define LD2(VARH, PER, FILTER) do { if (record) LD(VARH, PER, FILTER, true); else LD(VARH, PER, FILTER, false); } while (0)
-#define LD3(VARH, PER) do { if (filter) LD2(VARH, PER, true); else LD2(VARH, PER, false); } while (0)
-    if (c->variable_h) { if (per) LD3(true, true); else LD3(true, false); }
-    else               { if (per) LD3(false, true); else LD3(false, false); }
-#undef LD3
-#undef LD2
-#undef LD
-    return SPH_OK;
-}
-
-// ------------------------------------------------------------------------------------------------
-// Warp-tile variant (sph_tile.cuh): broadcast candidate tests from shared memory, hit masks, drain.
-// ------------------------------------------------------------------------------------------------
 struct DensitySrc { float4 pj; float mj; uint32_t aid; };
 
 template <int KERNEL, int DIM, bool VARH, bool FILTER, bool RECORD>
@@ -128,8 +41,8 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         if (FILTER) { if (!((my_mask >> s.aid) & 1u)) return; }
         float dx = pi.x - s.pj.x, dy = pi.y - s.pj.y, dz = DIM == 3 ? pi.z - s.pj.z : 0.0f;
         if (per) {
-            dx = min_image<true>(dx, Lx, iLx); dy = min_image<true>(dy, Ly, iLy);
-            if (DIM == 3) dz = min_image<true>(dz, Lz, iLz);
+            dx = min_image(dx, Lx, iLx); dy = min_image(dy, Ly, iLy);
+            if (DIM == 3) dz = min_image(dz, Lz, iLz);
         }
         float r2 = fmaf(dy, dy, dx * dx);
         if (DIM == 3) r2 = fmaf(dz, dz, r2);
@@ -198,7 +111,7 @@ int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record) {
     }
     const int k = c->prm.kernel, d = c->grid.dim;
     int rc = sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
-#define KD(K, D) if (k == K && d == D) rc = c->tile ? launch_density_tile_kd<K, D>(c, filter, record) : launch_density_kd<K, D>(c, filter, record)
+#define KD(K, D) if (k == K && d == D) rc = launch_density_tile_kd<K, D>(c, filter, record)
     KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
     KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
     KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);

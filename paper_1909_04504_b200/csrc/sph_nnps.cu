@@ -278,51 +278,8 @@ int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// neighbour-list export (verification): the same walker and the same predicate as the pair kernels.
+// neighbour-list export (verification): the same warp-tile walker and predicate code as the pair kernels.
 // ------------------------------------------------------------------------------------------------
-struct CountPolicy {
-    const uint32_t* meta; uint32_t src; uint32_t cnt;
-    __device__ __forceinline__ void hit(uint32_t j) { if ((meta[j] >> SPH_META_IDX_BITS) == src) ++cnt; }
-    __device__ __forceinline__ void pre_chunk() {}
-    __device__ __forceinline__ void tested(int) {}
-};
-struct FillPolicy {
-    const uint32_t* meta; uint32_t src; int32_t* row; uint32_t cnt;
-    __device__ __forceinline__ void hit(uint32_t j) {
-        const uint32_t m = meta[j];
-        if ((m >> SPH_META_IDX_BITS) == src) row[cnt++] = (int32_t)(m & SPH_META_IDX_MASK);
-    }
-    __device__ __forceinline__ void pre_chunk() {}
-    __device__ __forceinline__ void tested(int) {}
-};
-
-template <int DIM, bool VARH, bool FILL>
-__global__ void __launch_bounds__(NB)
-k_neighbors(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
-            uint32_t dest, uint32_t src, uint32_t* __restrict__ counts, const uint32_t* __restrict__ offsets,
-            int32_t* __restrict__ indices) {
-    const int i = blockIdx.x * NB + threadIdx.x;
-    const bool in = i < n;
-    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
-    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; }
-    const bool active = in && (meta >> SPH_META_IDX_BITS) == dest;
-    if (!__any_sync(SPH_FULL_MASK, active)) return;
-    const uint32_t o = meta & SPH_META_IDX_MASK;
-    if (!FILL) {
-        CountPolicy pol; pol.meta = S.meta; pol.src = src; pol.cnt = 0;
-        walk_candidates<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, ci, pol);
-        if (active) counts[o] = pol.cnt;
-    } else {
-        FillPolicy pol; pol.meta = S.meta; pol.src = src; pol.cnt = 0; pol.row = indices + (active ? offsets[o] : 0u);
-        walk_candidates<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, ci, pol);
-        if (active) {                                   // rows ascending (insertion sort; rows are short)
-            int32_t* r = pol.row; const int m = (int)pol.cnt;
-            for (int a = 1; a < m; ++a) { int32_t v = r[a]; int b = a - 1; while (b >= 0 && r[b] > v) { r[b + 1] = r[b]; --b; } r[b + 1] = v; }
-        }
-    }
-}
-
-// the same export through the warp-tile walker (the predicate code the tile pair kernels run)
 template <int DIM, bool VARH, bool FILL>
 __global__ void __launch_bounds__(TILE_BLOCK)
 k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
@@ -369,15 +326,14 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
     const long long nd = c->n[dest];
     uint32_t* counts = c->key;            // scratch: key/rank are dead between sorts
     uint32_t* off32 = c->rank;
-    const int grid = (n + NB - 1) / NB;
     SPH_CUDA_OK(c, cudaMemsetAsync(counts, 0, (size_t)(nd + 1) * sizeof(uint32_t), c->stream));
     SortedState& S = c->S[c->cur];
-#define LNK(K, GRID, BLOCK, FILL, IDX) do { \
-    if (c->grid.dim == 2) { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<2, true, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
-                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<2, false, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } \
-    else                  { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<3, true, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
-                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (K<3, false, FILL>), GRID, BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
-#define LN(FILL, IDX) do { if (c->tile) LNK(k_neighbors_tile, (n + TILE_BLOCK - 1) / TILE_BLOCK, TILE_BLOCK, FILL, IDX); else LNK(k_neighbors, grid, NB, FILL, IDX); } while (0)
+    const int tgrid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
+#define LN(FILL, IDX) do { \
+    if (c->grid.dim == 2) { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors_tile<2, true, FILL>), tgrid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors_tile<2, false, FILL>), tgrid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } \
+    else                  { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors_tile<3, true, FILL>), tgrid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
+                            else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors_tile<3, false, FILL>), tgrid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
     if (n) LN(false, (int32_t*)nullptr);
     int rc = scan_exclusive(c, counts, off32, nd);
     if (rc) return rc;
@@ -394,7 +350,6 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
     const bool fill = indices && cap >= *total && *total > 0;
     if (fill && n) LN(true, d_idx);
 #undef LN
-#undef LNK
     if (mem == SPH_MEM_HOST) {
         SPH_CUDA_OK(c, cudaMemcpyAsync(offsets, d_off, (size_t)(nd + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
         if (fill) SPH_CUDA_OK(c, cudaMemcpyAsync(indices, d_idx, (size_t)(*total) * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));

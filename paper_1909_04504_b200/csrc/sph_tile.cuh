@@ -18,7 +18,8 @@
 // 4 B per hit) to the record pool; the acceleration pass of the same evaluation replays them (tile_replay)
 // and tests nothing.
 #pragma once
-#include "sph_pair.cuh"
+#include "sph_ctx.cuh"
+#include <type_traits>
 
 #define TILE_BLOCK 128
 #define TILE_WARPS (TILE_BLOCK / 32)
@@ -221,14 +222,17 @@ __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, Load&&
         const int k = __ffs(cur) - 1; cur &= cur - 1u; j = b + (uint32_t)k;
         return true;
     };
-    Src A, B; uint32_t j = 0u;
+    Src A, B; uint32_t j = 0u;                     // two hits in flight, roles alternate (no register moves)
     bool hasA = pop(j);
     if (hasA) A = load(j);
-    while (__any_sync(SPH_FULL_MASK, hasA)) {
+    for (;;) {
         const bool hasB = pop(j);
         if (hasB) B = load(j);
         if (hasA) compute(A);
-        A = B; hasA = hasB;
+        hasA = pop(j);
+        if (hasA) A = load(j);
+        if (hasB) compute(B);
+        if (!__any_sync(SPH_FULL_MASK, hasA)) break;
     }
     __syncwarp();
 }
@@ -285,3 +289,12 @@ __device__ __forceinline__ void tile_replay(const NList& nl, int warp_id, TileWa
         blk = next;
     }
 }
+
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(SPH_FULL_MASK, v, o);
+    return v;
+}
+
+// Minimum image for the FIELD arithmetic of phase 2 (any accurate image will do there; the set membership was
+// decided bit-exactly in phase 1).  For a true neighbour |d_min| < L/3, so rint picks the same image as R7.
+__device__ __forceinline__ float min_image(float d, float L, float invL) { return fmaf(-rintf(d * invL), L, d); }
