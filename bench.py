@@ -11,9 +11,10 @@ workload.  Prints ONE JSON line (rank 0).
              events on the context stream, L2 flushed (256 MiB write) between timed steps; max over ranks.
   e2e        the same metric through the C ABI with HOST (pinned) buffers: every step does sph_nnps_build(host
              arrays incl. a^n) + sph_pc_step(dt, 1) + sph_sync_state(host, incl. a^{n+1}); copies inside the timing.
-  roofline   the dominant kernel (the momentum pair loop k_accel): algorithmic flops per launch / its mean launch
-             duration from CUDA event pairs recorded around every launch (sph_set_profiling) during a second pass
-             of the same K steps.  bound = "alu" (plain FP32 pipes).
+  roofline   the dominant kernel (a pair loop: k_density searches + sums eq.3, k_accel_list replays its hit masks
+             for eq.8-9): algorithmic flops per launch / its mean launch duration from CUDA event pairs recorded
+             around every launch (sph_set_profiling) during a second pass of the same K steps.  bound = "alu"
+             (plain FP32 pipes); peak = the FMA rate sph_fp32_probe measures in this run.
   cpu_baseline  the fp64 oracle (oracle/, as it stands, OpenMP over destinations) on this box's host cores.
 
 N > 1: the path does not shard (north_star: one GPU) -> N independent replicas (seed + rank), no data-path
@@ -121,6 +122,21 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def ncu_traffic(kernel: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the committed
+    `ncu --set full` capture summarised in profiles/r1_dram_traffic.csv (kernel,workload,read_bytes,write_bytes),
+    or None when no capture of that kernel/workload is committed."""
+    path = os.path.join(ROOT, "profiles", "r1_dram_traffic.csv")
+    try:
+        for line in open(path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 4 and f[0] == kernel and f[1] == workload:
+                return float(f[2]) + float(f[3])
+    except OSError:
+        pass
+    return None
+
+
 def aggregate(elapsed_ms: float, units: float, world: int):
     """max-over-ranks time and summed units (replicas): returns (ms, total_units).  gloo/nccl all_reduce."""
     if world <= 1:
@@ -215,6 +231,9 @@ def run_ours(args):
     with torch.cuda.stream(stream):
         ctx = binding.SphContext.from_workload(wl, stream=stream, move=move)
         dev = binding.device_arrays(wl)
+        fp32_peak = None
+        if rank == 0:
+            fp32_peak = {"ffma": ctx.fp32_probe(False, 8192)[0], "ffma2": ctx.fp32_probe(True, 8192)[0]}
         ctx.nnps_build(dev, fixed)
         ctx.pc_step(wl.dt, 1, mode)                       # a^0 + first step
         for _ in range(max(Wm - 1, 0)):
@@ -302,27 +321,51 @@ def run_ours(args):
     value = units / (ms_max * 1e-3)
     pairs_per_step = stats.pairs_density + stats.pairs_accel
     variable_h = bool(stats.variable_h)
-    # dominant kernel
-    dom = max((k for k in prof if not k.startswith("_")), key=lambda k: prof[k]["ms"])
     step_kernel_ms = sum(v["ms"] for k, v in prof.items() if not k.startswith("_"))
     kernels = {k: {"launches": v["launches"], "ms_per_launch": v["ms"] / v["launches"], "share": v["ms"] / step_kernel_ms}
                for k, v in prof.items() if not k.startswith("_")}
     cont = mode == "continuity"
+    # ---- ALU roofline of the pair kernels (DESIGN.md "Rooflines" / "Algorithmic work"):
+    # algorithmic flops of one launch = [searching passes only] the paper's own candidate set, the 3^d cells of
+    # size >= the support radius around each destination (L158), x flops per predicate test, + the true pairs x
+    # flops per pair.  The candidates the kernel REALLY tests (stats.candidates_*) are reported beside it, not used.
     c_test = flops_per_test(wl.dim, variable_h)
-    if dom == "k_density":
-        n_launch = prof[dom]["launches"] / K
-        flops_launch = (stats.candidates_density * c_test + stats.pairs_density * flops_per_pair("density", wl.kernel, wl.dim, variable_h, False)) / max(n_launch, 1)
-        cand_note = "candidate tests + pairs"
-    else:
-        n_launch = prof.get("k_accel", {"launches": K})["launches"] / K
-        flops_launch = (stats.candidates_accel * c_test + stats.pairs_accel * flops_per_pair("accel", wl.kernel, wl.dim, variable_h, cont)) / max(n_launch, 1)
-        cand_note = "candidate tests + pairs"
+    coarse_cells = 1
+    for k in range(wl.dim):
+        coarse_cells *= max(1, stats.n_cells[k] // (stats.xsub if k == 0 else 1))
+    ref_candidates = (3 ** wl.dim) * float(N) * float(N) / coarse_cells          # uniform-occupancy figure
+    alu = {}
+    if "k_density" in prof:
+        nl_ = prof["k_density"]["launches"] / K
+        fl = (ref_candidates * c_test + stats.pairs_density * flops_per_pair("density", wl.kernel, wl.dim, variable_h, False)) / max(nl_, 1)
+        alu["k_density"] = {"flops": fl, "searches": True}
+    for kname, searches in (("k_accel", True), ("k_accel_list", False)):
+        if kname in prof:
+            nl_ = prof[kname]["launches"] / K
+            fl = ((ref_candidates * c_test if searches else 0.0)
+                  + stats.pairs_accel * flops_per_pair("accel", wl.kernel, wl.dim, variable_h, cont)) / max(nl_, 1)
+            alu[kname] = {"flops": fl, "searches": searches}
+    peak_tf, peak_src = ALU_PEAK_TFLOPS, "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz"
+    if fp32_peak:
+        peak_tf = max(fp32_peak.values())
+        peak_src = ("measured in this run by sph_fp32_probe (dependent-free FMA streams, 8 blocks x 256 threads per SM): "
+                    f"FFMA {fp32_peak['ffma']:.1f}, FFMA2 {fp32_peak['ffma2']:.1f} TFLOP/s; nominal {ALU_PEAK_TFLOPS:.1f}")
+    for kname, v in alu.items():
+        dur = prof[kname]["ms"] / prof[kname]["launches"]
+        v["achieved_tflops"] = v["flops"] / (dur * 1e-3) / 1e12
+        v["frac"] = v["achieved_tflops"] / peak_tf
+        kernels[kname].update({"algorithmic_flops_per_launch": v["flops"], "achieved_tflops": v["achieved_tflops"],
+                               "alu_frac": v["frac"]})
+    dom = max(alu, key=lambda k: prof[k]["ms"]) if alu else max((k for k in prof if not k.startswith("_")), key=lambda k: prof[k]["ms"])
     dur_ms = prof[dom]["ms"] / prof[dom]["launches"]
-    achieved = flops_launch / (dur_ms * 1e-3) / 1e12
-    roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved / ALU_PEAK_TFLOPS, "traffic": None,
-                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md Rooflines); no measured FP32 peak in MEASURED_PEAKS.json",
-                "algorithmic_flops_per_launch": flops_launch, "counts": cand_note, "ms_per_launch": dur_ms,
+    roofline = {"kernel": dom, "bound": "alu", "achieved": alu[dom]["achieved_tflops"], "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": alu[dom]["frac"], "traffic": ncu_traffic(dom, args.workload),
+                "peak_source": peak_src,
+                "algorithmic_flops_per_launch": alu[dom]["flops"],
+                "counts": (f"{'3^d-cell candidates of L158 x ' + str(c_test) + ' flop + ' if alu[dom]['searches'] else ''}"
+                           f"true pairs x flops per pair (DESIGN.md Algorithmic work); the kernel really tested "
+                           f"{stats.candidates_density if dom == 'k_density' else stats.candidates_accel} candidates"),
+                "ms_per_launch": dur_ms,
                 "share_of_step_kernel_time": prof[dom]["ms"] / step_kernel_ms,
                 "timing": "CUDA event pair around every launch in a second pass of the same K steps"}
     try:

@@ -39,7 +39,7 @@ extern "C" {
 #endif
 
 #define SPH_MAX_ARRAYS 4
-#define SPH_ABI_VERSION 2
+#define SPH_ABI_VERSION 3
 
 typedef struct sph_ctx sph_ctx;
 
@@ -47,8 +47,7 @@ enum sph_error {
     SPH_OK = 0,
     SPH_ERR_NULL = -1,          /* a required pointer is NULL                                  */
     SPH_ERR_BAD_ARG = -2,       /* invalid value (dim, kernel, mask, periodic axis with < 3 cells ...) */
-    SPH_ERR_CAPACITY = -3,      /* n exceeds the capacity given to sph_create, output too small, or [sync] the
-                                   neighbour-row pool ran out (sph_params.nlist_slots)              */
+    SPH_ERR_CAPACITY = -3,      /* n exceeds the capacity given to sph_create, or an output is too small */
     SPH_ERR_STALE_NNPS = -4,    /* call needs a neighbour structure and none has been built      */
     SPH_ERR_OUT_OF_DOMAIN = -5, /* [sync] particles left a non-periodic domain box               */
     SPH_ERR_NONFINITE = -6,     /* [sync] NaN/Inf produced by a pair loop                        */
@@ -83,10 +82,12 @@ typedef struct sph_params {
     int move;                   /* 1: sph_pc_step applies eq.13 (default); 0: positions frozen (config C5) */
     /* Tuning knobs of the neighbour search; results do not depend on them (0 = default). */
     int xsub;                   /* x sub-cells per support radius (default 4, 1..16): finer x-interval culling   */
-    int nlist_slots;            /* neighbour-row pool, in rows of 32 particles per warp of capacity (default 192,
-                                 * i.e. 768 B per particle of capacity; < 0: never record rows, every pair pass
-                                 * searches).  A pool that runs out is reported as SPH_ERR_CAPACITY by the next
-                                 * [sync] call; raise nlist_slots or pass a negative value. */
+    int nlist_slots;            /* record pool of the pair passes, in rows of 32 words per warp (32 particles) of
+                                 * capacity (default 192, i.e. 768 B per particle of capacity; < 0: no pool, every
+                                 * pair pass searches).  The summation-density pass records one 32-bit hit mask
+                                 * per particle and batch of 32 candidates; the momentum pass of the same
+                                 * evaluation replays them instead of searching again.  A warp whose masks do
+                                 * not fit simply searches again (sph_stats.nlist_fallback_warps counts them). */
 } sph_params;
 
 typedef struct sph_array {      /* one named particle array (L316) */
@@ -119,8 +120,9 @@ typedef struct sph_stats {
     int32_t variable_h;         /* 1 if h_min != h_max at the last build */
     float h_max;
     int32_t xsub;               /* x sub-cells per support radius of the current grid (n_cells[0] counts sub-cells) */
-    int32_t used_rows;          /* 1 if the last acceleration pass replayed recorded neighbour rows */
-    int64_t nlist_rows_used, nlist_rows_capacity;   /* neighbour-row pool occupancy after the last recording pass */
+    int32_t used_rows;          /* 1 if the last acceleration pass replayed the hit masks recorded by the density pass */
+    int64_t nlist_rows_used, nlist_rows_capacity;   /* record pool occupancy after the last recording pass */
+    int64_t nlist_fallback_warps;                   /* warps whose masks did not fit the pool in that pass (they search again) */
 } sph_stats;
 
 /* Per-kernel device timing (CUDA events on the context stream around every launch), for the roofline report. */
@@ -134,7 +136,7 @@ enum sph_kernel_id {
     SPH_K_ACCEL = 6,            /* a6 + a7: momentum (+ continuity) pair loop                     */
     SPH_K_OUTPUT = 7,           /* caller-order output gather                                     */
     SPH_K_NEIGHBORS = 8,        /* verification export                                            */
-    SPH_K_ACCEL_LIST = 9,       /* a6 + a7 replayed over the neighbour rows recorded by a4         */
+    SPH_K_ACCEL_LIST = 9,       /* a6 + a7 replayed over the hit masks recorded by a4              */
     SPH_K_COUNT = 16
 };
 typedef struct sph_profile {
@@ -147,7 +149,7 @@ typedef struct sph_profile {
 
 /* Creates a context for `n_arrays` (1..SPH_MAX_ARRAYS) particle arrays of at most capacity[a] particles.
  * cuda_stream: a cudaStream_t (e.g. torch.cuda.Stream.cuda_stream), NULL = the legacy default stream.
- * Allocates all workspace (about 190 B per particle of capacity + the cell tables + the neighbour-row pool,
+ * Allocates all workspace (about 190 B per particle of capacity + the cell tables + the record pool,
  * 768 B per particle of capacity by default, see sph_params.nlist_slots).  [sync] */
 int sph_create(sph_ctx** out, const sph_params* params, const sph_domain* domain,
                int n_arrays, const int64_t* capacity, void* cuda_stream);

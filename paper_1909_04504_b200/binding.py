@@ -53,7 +53,8 @@ class sph_stats(C.Structure):
                 ("candidates_density", C.c_int64), ("candidates_accel", C.c_int64),
                 ("kernel_launches", C.c_int64), ("steps_done", C.c_int64), ("variable_h", C.c_int32),
                 ("h_max", C.c_float), ("xsub", C.c_int32), ("used_rows", C.c_int32),
-                ("nlist_rows_used", C.c_int64), ("nlist_rows_capacity", C.c_int64)]
+                ("nlist_rows_used", C.c_int64), ("nlist_rows_capacity", C.c_int64),
+                ("nlist_fallback_warps", C.c_int64)]
 
 
 class sph_profile(C.Structure):

@@ -23,7 +23,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const bool in = i < n;
     uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1), vi = make_float4(0, 0, 0, 0);
     float2 ri = make_float2(1, 0);
-    if (in) { meta = S.meta[i]; pi = S.posh[i]; vi = S.velm[i]; ri = S.rp[i]; if (!REPLAY) ci = S.cell[i]; }
+    if (in) { meta = S.meta[i]; pi = S.posh[i]; vi = S.velm[i]; ri = S.rp[i]; ci = S.cell[i]; }
     const uint32_t my_mask = in ? pc.src_mask[meta >> SPH_META_IDX_BITS] : 0u;
     const bool active = my_mask != 0u;
     if (!__any_sync(SPH_FULL_MASK, active)) return;
@@ -79,9 +79,10 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     auto drain = [&](uint32_t nz, bool shifted) { per = shifted; tile_drain<AccelSrc>(ws, nz, load, compute); };
 
     TileState st; st.reset(); st.tests = 0;
-    if (REPLAY) {
-        tile_replay(nl, warp_id, ws, drain);
-    } else {
+    const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
+    if (head != SPH_NL_NONE) {
+        tile_replay(nl, head, ws, drain);
+    } else {                                    // no record (or one that did not fit the pool): search
         const int row = in ? (int)(ci / (uint32_t)g.nc[0]) : -1;
         const int sub = in ? (int)(ci % (uint32_t)g.nc[0]) : 0;
         tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
@@ -94,7 +95,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
     const unsigned long long h = warp_sum_u64(hits), t = warp_sum_u64(st.tests);
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); if (!REPLAY) atomicAdd(&counters[CNT_CAND_ACCEL], t); }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); if (t) atomicAdd(&counters[CNT_CAND_ACCEL], t); }
 }
 
 template <int KERNEL, int DIM>

@@ -112,7 +112,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 2 * sizeof(float)));
     if (nl_slots > 0 && tot > 0) {
         const size_t warps = (size_t)(tot + 31) / 32;
-        size_t rows = warps * (size_t)nl_slots + 65536;
+        size_t rows = warps * (size_t)nl_slots + 32;
         if (rows > 0xfffffff0ull) rows = 0xfffffff0ull;
         c->nl.pool_rows = (uint32_t)rows;
         SPH_CUDA_OK(c, cudaMalloc(&c->nl.pool, rows * 32 * sizeof(uint32_t)));
@@ -409,7 +409,6 @@ extern "C" int sph_synchronize(sph_ctx* c) {
     unsigned long long h[CNT_COUNT];
     int rc = read_counters(c, h); if (rc) return rc;
     if (h[CNT_OUT_OF_DOMAIN]) { snprintf(c->err, sizeof(c->err), "%llu particle updates fell outside the non-periodic domain box", h[CNT_OUT_OF_DOMAIN]); return SPH_ERR_OUT_OF_DOMAIN; }
-    if (h[CNT_OVERFLOW]) { snprintf(c->err, sizeof(c->err), "the neighbour-row pool ran out in %llu warps: raise sph_params.nlist_slots (or pass < 0)", h[CNT_OVERFLOW]); return SPH_ERR_CAPACITY; }
     if (h[CNT_NONFINITE]) { snprintf(c->err, sizeof(c->err), "%llu non-finite results", h[CNT_NONFINITE]); return SPH_ERR_NONFINITE; }
     return SPH_OK;
 }
@@ -436,6 +435,7 @@ extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->xsub = c->grid.xsub;
     out->used_rows = c->last_used_rows ? 1 : 0;
     out->nlist_rows_capacity = c->nl.pool_rows;
+    out->nlist_fallback_warps = (int64_t)h[CNT_OVERFLOW];
     if (c->nl.used) {
         uint32_t u = 0;
         SPH_CUDA_OK(c, cudaMemcpyAsync(&u, c->nl.used, sizeof(u), cudaMemcpyDeviceToHost, c->stream));

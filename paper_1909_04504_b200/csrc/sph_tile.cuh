@@ -240,7 +240,7 @@ __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, Load&&
 // ---- mask records (recorded by the density pass, replayed by the acceleration pass) -----------------------
 // The pool is an array of ROWS of 32 words.  A warp appends BLOCKS: a header row {next block (row index, 0 =
 // end), number of batches M <= TILE_MMAX | 0x100 if a batch came from a periodic image, base[0..M-1]} followed
-// by M rows of masks (word = lane).
+// by M rows of masks (word = lane).  head[warp] = SPH_NL_NONE marks a warp whose masks did not fit the pool.
 struct TileRecorder {
     NList nl; uint32_t prev_hdr; bool ok;
     __device__ __forceinline__ void init(const NList& n) { nl = n; prev_hdr = 0u; ok = n.pool != nullptr; }
@@ -251,8 +251,8 @@ struct TileRecorder {
         if (lane == 0) blk = atomicAdd(nl.used, (uint32_t)M + 1u) + 1u;
         blk = __shfl_sync(SPH_FULL_MASK, blk, 0);
         if ((unsigned long long)blk + (unsigned)M + 1ull > (unsigned long long)nl.pool_rows) {
-            ok = false;
-            if (lane == 0) atomicAdd(&counters[CNT_OVERFLOW], 1ull);
+            ok = false;                         // the warp's record is incomplete: the replaying pass searches again
+            if (lane == 0) { nl.head[warp_id] = SPH_NL_NONE; atomicAdd(&counters[CNT_OVERFLOW], 1ull); }
             return;
         }
         __syncwarp();
@@ -266,9 +266,8 @@ struct TileRecorder {
 
 // drain(nz, shifted) is called once per recorded block with the masks and bases in ws
 template <class Drain>
-__device__ __forceinline__ void tile_replay(const NList& nl, int warp_id, TileWarpSmem& ws, Drain&& drain) {
+__device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileWarpSmem& ws, Drain&& drain) {
     const int lane = threadIdx.x & 31;
-    uint32_t blk = __ldg(nl.head + warp_id);
     while (blk) {
         const uint32_t* hdr = nl.pool + (size_t)blk * 32;
         const uint32_t hw = __ldcs(hdr + lane);

@@ -79,3 +79,27 @@ def test_restart_from_synced_state_continues_the_run(WL):
                 scale = max(np.abs(w_).max(), 1e-30)
                 assert np.abs(g_ - w_).max() <= TOL * scale, f"{wl.name} {k}[{d}]"
         ctx.close(); ctx2.close()
+
+
+def test_record_pool_overflow_falls_back_to_searching(WL):
+    """A record pool too small for the density pass's hit masks: the warps that did not fit search again in the
+    momentum pass (no error, same pairs, same result as with the default pool or with no pool at all)."""
+    wl = WL.periodic_box_3d((24, 24, 24), seed=5)
+    res = []
+    for slots in (0, 2, -1):                       # default pool, a pool of 2 rows per warp, no pool
+        ctx, _ = make_ctx(wl, nlist_slots=slots)
+        ctx.pc_step(wl.dt, 2, "summation")
+        ctx.synchronize()
+        s = ctx.get_stats()
+        out = {k: v.cpu().numpy() for k, v in ctx.sync_state(0).items()}
+        res.append((s.pairs_density, s.pairs_accel, s.nlist_fallback_warps, s.candidates_accel, out))
+        ctx.close()
+    (pd0, pa0, fb0, ca0, o0), (pd1, pa1, fb1, ca1, o1), (pd2, pa2, fb2, ca2, o2) = res
+    assert pd0 == pa0 == pd1 == pa1 == pd2 == pa2
+    assert fb0 == 0 and ca0 == 0                    # everything replayed
+    assert fb1 > 0 and 0 < ca1 <= ca2               # some warps searched again
+    assert fb2 == 0 and ca2 > 0                     # no pool: the whole momentum pass searched
+    for k in ("x", "u", "v", "w", "rho"):
+        for o in (o1, o2):
+            scale = np.abs(o0[k]).max()
+            assert np.abs(o[k].astype(np.float64) - o0[k]).max() <= 2e-6 * scale, k
