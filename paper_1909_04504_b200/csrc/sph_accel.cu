@@ -35,16 +35,15 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const float hi = VARH ? pi.w : h_c;
     const float rho_i = ri.x, pr_i = ri.y;
     float ax = pc.g[0], ay = pc.g[1], az = pc.g[2], ar = 0.0f;      // gravity = accumulator init (Listing 4)
-    unsigned long long hits = 0;
+    unsigned long long fhits = 0, rhits = 0;                            // FILTER: hits passing the source mask; replayed hits
     auto load = [&](uint32_t j) {
         AccelSrc s; s.pj = __ldg(S.posh + j); s.vj = __ldg(S.velm + j); s.rj = __ldg(S.rp + j); s.aid = 0u;
         if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
         return s;
     };
     bool per = false;                                                   // warp-uniform: some stored batch is a periodic image
-    auto compute = [&](const AccelSrc& s) {
-        if (FILTER) { if (!((my_mask >> s.aid) & 1u)) return; }
-        if (REPLAY) { if (!active) return; }
+    auto compute = [&](const AccelSrc& s, bool has) {
+        if (FILTER) { has = has && ((my_mask >> s.aid) & 1u); fhits += has ? 1u : 0u; }
         float dx = pi.x - s.pj.x, dy = pi.y - s.pj.y, dz = DIM == 3 ? pi.z - s.pj.z : 0.0f;
         if (per) {
             dx = min_image(dx, Lx, iLx); dy = min_image(dy, Ly, iLy);
@@ -69,19 +68,19 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
         const float den = fmaf(eps * hij, hij, r2) * (rho_i + s.rj.x);
         const float Pi = vr < 0.0f ? visc * hij * vr * rcp_approx(den) : 0.0f;
-        const float mg = s.vj.w * gc;
+        const float mg = has ? s.vj.w * gc : 0.0f;                      // a lane that has run out contributes nothing
         const float sc = -mg * (pr_i + s.rj.y + Pi);
         ax = fmaf(sc, dx, ax); ay = fmaf(sc, dy, ay);
         if (DIM == 3) az = fmaf(sc, dz, az);
         if (ARHO) ar = fmaf(mg, vr, ar);
-        ++hits;
     };
-    auto drain = [&](uint32_t nz, bool shifted) { per = shifted; tile_drain<AccelSrc>(ws, nz, load, compute); };
+    const uint32_t idle = in ? (uint32_t)i : 0u;
+    auto drain = [&](uint32_t nz, bool shifted) { per = shifted; tile_drain<AccelSrc>(ws, nz, idle, load, compute); };
 
-    TileState st; st.reset(); st.tests = 0;
+    TileState st; st.reset(); st.tests = 0; st.hits = 0;
     const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
     if (head != SPH_NL_NONE) {
-        tile_replay(nl, head, ws, drain);
+        tile_replay(nl, head, ws, active, rhits, drain);
     } else {                                    // no record (or one that did not fit the pool): search
         const int row = in ? (int)(ci / (uint32_t)g.nc[0]) : -1;
         const int sub = in ? (int)(ci % (uint32_t)g.nc[0]) : 0;
@@ -94,7 +93,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         S.acc[i] = a;
         if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
-    const unsigned long long h = warp_sum_u64(hits), t = warp_sum_u64(st.tests);
+    const unsigned long long h = warp_sum_u64(FILTER ? fhits : st.hits + rhits), t = warp_sum_u64(st.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); if (t) atomicAdd(&counters[CNT_CAND_ACCEL], t); }
 }
 

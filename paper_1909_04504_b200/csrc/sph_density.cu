@@ -28,7 +28,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     const float sigma = pc.sigma, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
     const float hi = VARH ? pi.w : pc.h_const;
     float rho = 0.0f;
-    unsigned long long hits = 0;
+    unsigned long long fhits = 0;                                       // FILTER: hits that pass the source mask
     // constant h: posh.w of the sorted state carries the MASS (SortedState), one 16-byte gather per pair
     auto load = [&](uint32_t j) {
         DensitySrc s; s.pj = __ldg(S.posh + j); s.mj = 0.0f; s.aid = 0u;
@@ -37,8 +37,8 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         return s;
     };
     bool per = false;                                                   // warp-uniform: some stored batch is a periodic image
-    auto compute = [&](const DensitySrc& s) {
-        if (FILTER) { if (!((my_mask >> s.aid) & 1u)) return; }
+    auto compute = [&](const DensitySrc& s, bool has) {
+        if (FILTER) { has = has && ((my_mask >> s.aid) & 1u); fhits += has ? 1u : 0u; }
         float dx = pi.x - s.pj.x, dy = pi.y - s.pj.y, dz = DIM == 3 ? pi.z - s.pj.z : 0.0f;
         if (per) {
             dx = min_image(dx, Lx, iLx); dy = min_image(dy, Ly, iLy);
@@ -56,16 +56,16 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         } else { hinv = hinv_c; fac = fac_c; mj = s.pj.w; }
         float f, df;
         kernel_profile<KERNEL, DIM>(r * hinv, f, df);
-        rho = fmaf(mj * fac, f, rho);
-        ++hits;
+        rho = has ? fmaf(mj * fac, f, rho) : rho;
     };
 
-    TileState st; st.reset(); st.tests = 0;
+    TileState st; st.reset(); st.tests = 0; st.hits = 0;
+    const uint32_t idle = in ? (uint32_t)i : 0u;
     TileRecorder rec; rec.init(nl); if (!RECORD) rec.ok = false;
     auto drain = [&]() {
         if (RECORD) rec.append(ws, st.M, st.shifted, warp_id, counters);
         per = st.shifted;
-        tile_drain<DensitySrc>(ws, st.nz, load, compute);
+        tile_drain<DensitySrc>(ws, st.nz, idle, load, compute);
         st.reset();
     };
     tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st, drain);
@@ -75,7 +75,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         S.rp[i] = make_float2(rho, p / (rho * rho));
         if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
-    const unsigned long long h = warp_sum_u64(hits), t = warp_sum_u64(st.tests);
+    const unsigned long long h = warp_sum_u64(FILTER ? fhits : st.hits), t = warp_sum_u64(st.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CAND_DENSITY], t); }
 }
 

@@ -299,14 +299,15 @@ k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __res
     uint32_t cnt = 0;
     int32_t* out = FILL ? indices + (active ? offsets[o] : 0u) : nullptr;
     auto load = [&](uint32_t j) { return __ldg(S.meta + j); };
-    auto compute = [&](const uint32_t& m) {
-        if ((m >> SPH_META_IDX_BITS) != src) return;
+    auto compute = [&](const uint32_t& m, bool has) {
+        if (!has || (m >> SPH_META_IDX_BITS) != src) return;
         if (FILL) out[cnt] = (int32_t)(m & SPH_META_IDX_MASK);
         ++cnt;
     };
-    TileState st; st.reset(); st.tests = 0;
+    TileState st; st.reset(); st.tests = 0; st.hits = 0;
+    const uint32_t idle = in ? (uint32_t)i : 0u;
     tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st,
-                         [&]() { tile_drain<uint32_t>(ws, st.nz, load, compute); st.reset(); });
+                         [&]() { tile_drain<uint32_t>(ws, st.nz, idle, load, compute); st.reset(); });
     if (!active) return;
     if (!FILL) counts[o] = cnt;
     else {                                              // rows ascending (insertion sort; rows are short)

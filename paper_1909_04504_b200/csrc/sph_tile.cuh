@@ -42,6 +42,7 @@ struct TileState {
     uint32_t nz;                           // bit m: this lane's mask m has hits
     bool shifted;                          // some stored batch came from a periodic image (warp-uniform)
     unsigned long long tests;              // predicate evaluations of this lane's particle
+    unsigned long long hits;               // predicate hits of this lane's particle
     __device__ __forceinline__ void reset() { M = 0; nz = 0u; shifted = false; }
 };
 
@@ -201,6 +202,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
             if (mask) st.nz |= 1u << st.M;
             if (lane == 0) ws.base[st.M] = b0;
             if (ing) st.tests += (unsigned)len;
+            st.hits += (unsigned)__popc(mask);
             ++st.M;
             b0 += 32u;
         }
@@ -209,29 +211,33 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
 }
 
 // Every lane pops its own hits of the stored batches in order (nz: the lane's non-empty masks) and evaluates
-// them, software-pipelined: the source data of hit t+1 is loaded (Src = load(sorted index)) before hit t is
-// computed, so the gather latency (L2: the sorted state does not fit L1) overlaps the arithmetic.
+// them.  Branch-free and software-pipelined: two hits are in flight, the source data of the next hit is
+// gathered (Src = load(sorted index)) before the current one is computed, so the gather latency (L2: the sorted
+// state does not fit L1) overlaps the arithmetic.  A lane that has run out keeps executing with has = false and
+// the harmless index `idle` (its own particle) until the slowest lane of the warp is done; compute(src, has)
+// must contribute nothing when has is false.
 template <class Src, class Load, class Compute>
-__device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, Load&& load, Compute&& compute) {
+__device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
     const int lane = threadIdx.x & 31;
     __syncwarp();
     uint32_t cur = 0u, b = 0u;
-    auto pop = [&](uint32_t& j) -> bool {
-        if (cur == 0u && nz) { const int m = __ffs(nz) - 1; nz &= nz - 1u; cur = ws.mask[m][lane]; b = ws.base[m]; }
-        if (cur == 0u) return false;
-        const int k = __ffs(cur) - 1; cur &= cur - 1u; j = b + (uint32_t)k;
-        return true;
+    auto pop = [&](bool& has) -> uint32_t {
+        const bool refill = cur == 0u && nz != 0u;
+        const int m = max(__ffs(nz) - 1, 0);
+        const uint32_t nm = ws.mask[m][lane], nb = ws.base[m];
+        cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? (nz & (nz - 1u)) : nz;
+        has = cur != 0u;
+        const uint32_t j = has ? b + (uint32_t)(__ffs(cur) - 1) : idle;
+        cur &= cur - 1u;                        // stays 0 when it is 0
+        return j;
     };
-    Src A, B; uint32_t j = 0u;                     // two hits in flight, roles alternate (no register moves)
-    bool hasA = pop(j);
-    if (hasA) A = load(j);
+    Src A, B; bool hasA, hasB;
+    A = load(pop(hasA));
     for (;;) {
-        const bool hasB = pop(j);
-        if (hasB) B = load(j);
-        if (hasA) compute(A);
-        hasA = pop(j);
-        if (hasA) A = load(j);
-        if (hasB) compute(B);
+        B = load(pop(hasB));
+        compute(A, hasA);
+        A = load(pop(hasA));
+        compute(B, hasB);
         if (!__any_sync(SPH_FULL_MASK, hasA)) break;
     }
     __syncwarp();
@@ -266,7 +272,7 @@ struct TileRecorder {
 
 // drain(nz, shifted) is called once per recorded block with the masks and bases in ws
 template <class Drain>
-__device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileWarpSmem& ws, Drain&& drain) {
+__device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileWarpSmem& ws, bool active, unsigned long long& hits, Drain&& drain) {
     const int lane = threadIdx.x & 31;
     while (blk) {
         const uint32_t* hdr = nl.pool + (size_t)blk * 32;
@@ -280,9 +286,9 @@ __device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileW
         for (int m0 = 0; m0 < M; m0 += 8) {                              // 8 independent loads in flight
             uint32_t w[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) w[k] = m0 + k < M ? __ldcs(hdr + (size_t)(m0 + k + 1) * 32 + lane) : 0u;
+            for (int k = 0; k < 8; ++k) w[k] = (m0 + k < M && active) ? __ldcs(hdr + (size_t)(m0 + k + 1) * 32 + lane) : 0u;   // a lane that is no destination of this pass drops its masks
 #pragma unroll
-            for (int k = 0; k < 8; ++k) if (m0 + k < M) { ws.mask[m0 + k][lane] = w[k]; if (w[k]) nz |= 1u << (m0 + k); }
+            for (int k = 0; k < 8; ++k) if (m0 + k < M) { ws.mask[m0 + k][lane] = w[k]; if (w[k]) nz |= 1u << (m0 + k); hits += (unsigned)__popc(w[k]); }
         }
         drain(nz, (w1 & 0x100u) != 0u);
         blk = next;
