@@ -12,7 +12,7 @@
 // L372-374): the same loop, only arho is stored.
 struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
 
-template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY>
+template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, bool PEOS>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
 k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
              int arho_only, NList nl, unsigned long long* __restrict__ counters) {
@@ -33,11 +33,16 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const float sigma = pc.sigma, h_c = pc.h_const, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
     const float visc = pc.visc, eps = pc.eps;
     const float hi = VARH ? pi.w : h_c;
-    const float rho_i = ri.x, pr_i = ri.y;
+    // PEOS (constant h, gamma = 7, every p is the EOS of its rho): the neighbour's rho rides in velm.w and its
+    // p/rho^2 is recomputed, two 16-byte gathers per pair instead of three (the loop is L1-gather bound); the
+    // destination's own term is recomputed the same way so that the pair terms stay antisymmetric.
+    const float inv_rho0 = 1.0f / pc.rho0, rho0 = pc.rho0, Beos = pc.B;
+    const float rho_i = ri.x, pr_i = PEOS ? eos7_p_over_rho2(ri.x, rho0, inv_rho0, Beos) : ri.y;
     float ax = pc.g[0], ay = pc.g[1], az = pc.g[2], ar = 0.0f;      // gravity = accumulator init (Listing 4)
     unsigned long long fhits = 0, rhits = 0;                            // FILTER: hits passing the source mask; replayed hits
     auto load = [&](uint32_t j) {
-        AccelSrc s; s.pj = __ldg(S.posh + j); s.vj = __ldg(S.velm + j); s.rj = __ldg(S.rp + j); s.aid = 0u;
+        AccelSrc s; s.pj = __ldg(S.posh + j); s.vj = __ldg(S.velm + j); s.aid = 0u;
+        s.rj = PEOS ? make_float2(0.0f, 0.0f) : __ldg(S.rp + j);
         if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
         return s;
     };
@@ -66,10 +71,13 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         float vr = fmaf(vy, dy, vx * dx);
         if (DIM == 3) vr = fmaf(vi.z - s.vj.z, dz, vr);
         // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
-        const float den = fmaf(eps * hij, hij, r2) * (rho_i + s.rj.x);
+        const float mj = VARH ? s.vj.w : s.pj.w;                        // SortedState: constant h keeps m in posh.w
+        const float rho_j = PEOS ? s.vj.w : s.rj.x;
+        const float pr_j = PEOS ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y;
+        const float den = fmaf(eps * hij, hij, r2) * (rho_i + rho_j);
         const float Pi = vr < 0.0f ? visc * hij * vr * rcp_approx(den) : 0.0f;
-        const float mg = has ? s.vj.w * gc : 0.0f;                      // a lane that has run out contributes nothing
-        const float sc = -mg * (pr_i + s.rj.y + Pi);
+        const float mg = has ? mj * gc : 0.0f;                          // a lane that has run out contributes nothing
+        const float sc = -mg * (pr_i + pr_j + Pi);
         ax = fmaf(sc, dx, ax); ay = fmaf(sc, dy, ay);
         if (DIM == 3) az = fmaf(sc, dz, az);
         if (ARHO) ar = fmaf(mg, vr, ar);
@@ -105,12 +113,13 @@ static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, bool ar
     SortedState& S = c->S[c->cur];
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
     const int ao = arho_only ? 1 : 0;
-#define LT(VARH, ARHO, FILTER, REPLAY) \
-        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
-#define LT1(VARH, ARHO, FILTER) do { if (replay) LT(VARH, ARHO, FILTER, true); else LT(VARH, ARHO, FILTER, false); } while (0)
-#define LT2(VARH, ARHO) do { if (filter) LT1(VARH, ARHO, true); else LT1(VARH, ARHO, false); } while (0)
-#define LT3(VARH) do { if (want_arho) LT2(VARH, true); else LT2(VARH, false); } while (0)
-    if (varh) LT3(true); else LT3(false);
+    const bool peos = c->p_is_eos && c->pc.gamma_is_7 && !varh;
+#define LT(VARH, ARHO, FILTER, REPLAY, PEOS) \
+        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PEOS>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
+#define LT1(VARH, ARHO, FILTER, PEOS) do { if (replay) LT(VARH, ARHO, FILTER, true, PEOS); else LT(VARH, ARHO, FILTER, false, PEOS); } while (0)
+#define LT2(VARH, ARHO, PEOS) do { if (filter) LT1(VARH, ARHO, true, PEOS); else LT1(VARH, ARHO, false, PEOS); } while (0)
+#define LT3(VARH, PEOS) do { if (want_arho) LT2(VARH, true, PEOS); else LT2(VARH, false, PEOS); } while (0)
+    if (varh) LT3(true, false); else if (peos) LT3(false, true); else LT3(false, false);
 #undef LT3
 #undef LT2
 #undef LT1

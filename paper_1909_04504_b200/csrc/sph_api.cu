@@ -205,7 +205,7 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     if (n_arrays != c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "n_arrays differs from sph_create");
     c->built = false; c->have_accel = false; c->have_arho = false; c->nl_valid = false;
     int64_t tot = 0;
-    bool all_acc = true, all_arho = true;
+    bool all_acc = true, all_arho = true, any_p = false;
     for (int a = 0; a < c->na; ++a) {
         const sph_array& A = arrays[a];
         if (A.n < 0) return sph_fail(c, SPH_ERR_BAD_ARG, "negative n");
@@ -216,6 +216,7 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
         tot += A.n;
         if (A.n > 0 && !c->fixed[a] && (!A.ax || !A.ay || (c->dom.dim == 3 && !A.az))) all_acc = false;
         if (A.n > 0 && !A.arho) all_arho = false;
+        if (A.n > 0 && A.p) any_p = true;
     }
     c->base[c->na] = tot; c->n_total = tot;
     if (!c->tables_user) default_tables(c);
@@ -254,7 +255,7 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     rc = size_grid(c); if (rc) return rc;
     rc = nnps_key_hist(c); if (rc) return rc;
     rc = nnps_sort_from_keys(c, true); if (rc) return rc;
-    c->built = true; c->steps_done = 0;
+    c->built = true; c->steps_done = 0; c->p_is_eos = !any_p;
     c->have_accel = all_acc && tot > 0; c->have_arho = all_arho && tot > 0;     // restart from caller-supplied a^n
     return SPH_OK;
 }

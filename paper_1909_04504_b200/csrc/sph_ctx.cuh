@@ -21,6 +21,7 @@ struct sph_ctx {
     GridDesc grid;
     PairConsts pc;
     bool built, have_accel, have_arho, variable_h;
+    bool p_is_eos;             // every p of the state is the EOS of its rho (no array supplied p at the last build)
     float h_min, h_max;
     int64_t n_keys, max_keys;
 

@@ -73,6 +73,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     if (active) {
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
         S.rp[i] = make_float2(rho, p / (rho * rho));
+        if (!VARH) S.velm[i].w = rho;                                   // constant h: velm.w carries rho (SortedState)
         if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
     const unsigned long long h = warp_sum_u64(FILTER ? fhits : st.hits), t = warp_sum_u64(st.tests);

@@ -55,10 +55,11 @@ struct PairConsts {
 
 // Cell-sorted particle state (struct of float4 groups: one 16-B vector load per candidate test).
 struct SortedState {
-    float4* posh;              // x, y, z, h  -- after the sort, when h is constant (h_min == h_max, the kernels
-                               // then take h from PairConsts), .w carries the MASS instead: the density pair
-                               // loop gathers one 16-byte word per neighbour (k_scatter, w_mass)
-    float4* velm;              // u, v, w, m
+    float4* posh;              // x, y, z, h          | constant h (h_min == h_max; the kernels then take h from
+    float4* velm;              // u, v, w, m          | PairConsts): after the sort posh = (x, y, z, M) and velm =
+                               //                     | (u, v, w, RHO), so that the density pair loop gathers ONE
+                               //                     | 16-byte word per neighbour and the momentum pair loop TWO
+                               //                     | (p/rho^2 is recomputed from rho when p is the EOS of rho)
     float2* rp;                // rho, p / rho^2   (p itself is returned as (p/rho^2) * rho^2)
     float4* acc;               // ax, ay, az, arho
     uint32_t* meta;            // (array << 28) | original index
@@ -126,6 +127,14 @@ __device__ __forceinline__ float eos_pressure(float rho, float rho0, float B, fl
     if (gamma_is_7) s = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.0f, 7.0f), 21.0f), 35.0f), 35.0f), 21.0f), 7.0f);
     else s = expm1f(gamma * log1pf(t));
     return B * s;
+}
+
+// p/rho^2 of the Tait EOS with gamma = 7 from rho alone (the momentum pair loop recomputes it per neighbour
+// instead of gathering it): same polynomial as eos_pressure, t formed with a multiplication by 1/rho0.
+__device__ __forceinline__ float eos7_p_over_rho2(float rho, float rho0, float inv_rho0, float B) {
+    const float t = (rho - rho0) * inv_rho0;
+    const float s = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.0f, 7.0f), 21.0f), 35.0f), 35.0f), 21.0f), 7.0f);
+    return B * s * rcp_approx(rho * rho);
 }
 
 // Cell coordinate of a position on one axis (clamped; out-of-range on a non-periodic axis is flagged by the caller).

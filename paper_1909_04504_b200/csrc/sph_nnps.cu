@@ -73,7 +73,7 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
 // way on EVERY array (the tank particles too, L142) and re-evaluates the EOS (group 1 of Listing 3).
 // ------------------------------------------------------------------------------------------------
 struct UpdateArgs {
-    float dt_half, dt; int kick2, kick1, move, continuity, rekey;
+    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho;
     int fixed[SPH_MAX_ARRAYS];
 };
 
@@ -113,6 +113,7 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
         if (U.kick1) rho = fmaf(U.dt_half, a.w, rho);
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
         S.rp[i] = make_float2(rho, p / (rho * rho));
+        if (U.w_rho) S.velm[i].w = rho;         // constant h: velm.w of the sorted state carries rho (SortedState)
     }
     if (U.rekey) {
         bool oob;
@@ -211,11 +212,12 @@ k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass,
     const uint32_t k = key[i];
     const uint32_t d = cell_start[k] + rank[i];
     float4 p = A.posh[i];
-    const float4 v = A.velm[i];
-    if (w_mass) p.w = v.w;                      // constant h: posh.w of the sorted state carries the mass
+    float4 v = A.velm[i];
+    const float2 r = A.rp[i];
+    if (w_mass) { p.w = v.w; v.w = r.x; }       // constant h, first sort after the pack: posh.w <- m, velm.w <- rho (SortedState)
     B.posh[d] = p;
     B.velm[d] = v;
-    B.rp[d] = A.rp[i];
+    B.rp[d] = r;
     B.meta[d] = A.meta[i];
     B.cell[d] = k / (uint32_t)na;
     if (with_acc) B.acc[d] = A.acc[i];
@@ -233,7 +235,7 @@ int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, boo
     const int n = (int)c->n_total;
     UpdateArgs U;
     U.dt_half = 0.5f * dt; U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
-    U.continuity = continuity; U.rekey = rekey;
+    U.continuity = continuity; U.rekey = rekey; U.w_rho = c->variable_h ? 0 : 1;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
     if (rekey) SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));
     if (n) SPH_LAUNCH(c, SPH_K_UPDATE, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
@@ -246,7 +248,7 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys);
     if (rc) return rc;
     if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
-                      with_acc ? 1 : 0, c->variable_h ? 0 : 1, c->key, c->rank, c->cell_start);
+                      with_acc ? 1 : 0, (!c->variable_h && with_acc) ? 1 : 0, c->key, c->rank, c->cell_start);
     c->cur ^= 1;
     c->nl_valid = false;                 // recorded neighbour rows index the previous sorted order
     return SPH_OK;
