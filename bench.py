@@ -154,8 +154,9 @@ def aggregate(elapsed_ms: float, units: float, world: int):
 # ---------------------------------------------------------------------------------------------------------
 # reference arm: the oracle on host cores
 # ---------------------------------------------------------------------------------------------------------
-def oracle_steps(wl, steps: int, warmup: int):
-    """Times `steps` oracle PC steps (after the a^0 evaluation and `warmup` steps).  Returns (seconds, pairs)."""
+def oracle_steps(wl, steps: int, warmup: int, budget_s: float = None):
+    """Times `steps` oracle PC steps (after the a^0 evaluation and `warmup` steps); with budget_s it stops after
+    the first step that ends past the budget.  Returns (seconds, pairs, threads, steps done)."""
     from oracle import sph_oracle as O
     st = O.State(wl)
     O.evaluate(wl, st, wl.density_mode)
@@ -164,9 +165,13 @@ def oracle_steps(wl, steps: int, warmup: int):
         O.pc_step(wl, st, wl.dt, wl.density_mode, move=move)
     t0 = time.perf_counter()
     pairs = 0
+    done = 0
     for _ in range(steps):
         pairs += O.pc_step(wl, st, wl.dt, wl.density_mode, move=move)
-    return time.perf_counter() - t0, pairs, O.num_threads()
+        done += 1
+        if budget_s is not None and time.perf_counter() - t0 > budget_s:
+            break
+    return time.perf_counter() - t0, pairs, O.num_threads(), done
 
 
 def run_reference(args):
@@ -174,7 +179,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     wl = make_workload(args.workload, 0, small=True)
-    sec, pairs, cores = oracle_steps(wl, args.steps, args.warmup)
+    sec, pairs, cores, _ = oracle_steps(wl, args.steps, args.warmup)
     val = wl.n_total * args.steps / sec
     sample = f"{wl.name}: {wl.n_total} particles per step (same spacing, h, kernel and parameters as the full workload)"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -384,9 +389,9 @@ def run_ours(args):
     cpu = None
     if not args.no_cpu_baseline:
         wl_small = make_workload(args.workload, 0, small=True)
-        sec, _, cores = oracle_steps(wl_small, args.cpu_steps, 0)
-        cpu = {"value": wl_small.n_total * args.cpu_steps / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{wl_small.name}: {args.cpu_steps} oracle PC steps of {wl_small.n_total} particles "
+        sec, _, cores, done = oracle_steps(wl_small, args.cpu_steps, 0, budget_s=args.cpu_seconds)
+        cpu = {"value": wl_small.n_total * done / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{wl_small.name}: {done} oracle PC steps of {wl_small.n_total} particles "
                          f"(same spacing, h, kernel, parameters) after the a^0 evaluation; {sec:.1f} s"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
@@ -420,7 +425,8 @@ def main():
     ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=10)
-    ap.add_argument("--cpu-steps", type=int, default=96)
+    ap.add_argument("--cpu-steps", type=int, default=1000)
+    ap.add_argument("--cpu-seconds", type=float, default=20.0, help="time budget of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
