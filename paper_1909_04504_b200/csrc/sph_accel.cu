@@ -15,7 +15,7 @@ struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
 template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, bool PEOS>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
 k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
-             int arho_only, NList nl, unsigned long long* __restrict__ counters) {
+             uint32_t arho_only_arrays, NList nl, unsigned long long* __restrict__ counters) {
     __shared__ TileWarpSmem smem[TILE_WARPS];
     TileWarpSmem& ws = smem[threadIdx.x >> 5];
     const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
@@ -43,12 +43,12 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     auto load = [&](uint32_t j) {
         AccelSrc s; s.pj = __ldg(S.posh + j); s.vj = __ldg(S.velm + j); s.aid = 0u;
         s.rj = PEOS ? make_float2(0.0f, 0.0f) : __ldg(S.rp + j);
-        if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
+        if (FILTER) { if (my_mask != pc.all_mask) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS; }   // lanes fed by all arrays skip the gather
         return s;
     };
     bool per = false;                                                   // warp-uniform: some stored batch is a periodic image
     auto compute = [&](const AccelSrc& s, bool has) {
-        if (FILTER) { has = has && ((my_mask >> s.aid) & 1u); fhits += has ? 1u : 0u; }
+        if (FILTER) { has = has && (my_mask == pc.all_mask || ((my_mask >> s.aid) & 1u)); fhits += has ? 1u : 0u; }
         float dx = pi.x - s.pj.x, dy = pi.y - s.pj.y, dz = DIM == 3 ? pi.z - s.pj.z : 0.0f;
         if (per) {
             dx = min_image(dx, Lx, iLx); dy = min_image(dy, Ly, iLy);
@@ -96,7 +96,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     }
     if (active) {
         float4 a = S.acc[i];
-        if (arho_only) a.w = ar;
+        if ((arho_only_arrays >> (meta >> SPH_META_IDX_BITS)) & 1u) a.w = ar;      // ContinuityEquation-only destination array
         else a = make_float4(ax, ay, DIM == 3 ? az : 0.0f, ARHO ? ar : a.w);
         S.acc[i] = a;
         if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
@@ -106,13 +106,13 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
 }
 
 template <int KERNEL, int DIM>
-static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, bool arho_only, bool replay) {
+static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, uint32_t arho_only, bool replay) {
     const int n = (int)c->n_total;
     if (n == 0) return SPH_OK;
     const bool varh = c->variable_h;
     SortedState& S = c->S[c->cur];
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
-    const int ao = arho_only ? 1 : 0;
+    const uint32_t ao = arho_only;
     const bool peos = c->p_is_eos && c->pc.gamma_is_7 && !varh;
 #define LT(VARH, ARHO, FILTER, REPLAY, PEOS) \
         SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PEOS>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
@@ -127,7 +127,9 @@ static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, bool ar
     return SPH_OK;
 }
 
-int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, bool arho_only) {
+// One launch serves every destination array whose mask is non-zero.  arho_only: bit a = array a stores only its
+// continuity sum (ContinuityEquation(dest=solid, sources=[fluid]), Listing 3).
+int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, uint32_t arho_only) {
     bool filter = false, use_list = c->nl_valid && !arho_only;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
@@ -136,7 +138,7 @@ int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, 
     }
     c->last_used_rows = use_list;
     const int k = c->prm.kernel, d = c->grid.dim;
-#define KD(K, D) if (k == K && d == D) return launch_accel_tile_kd<K, D>(c, filter, want_arho || arho_only, arho_only, use_list)
+#define KD(K, D) if (k == K && d == D) return launch_accel_tile_kd<K, D>(c, filter, want_arho || arho_only != 0u, arho_only, use_list)
     KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
     KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
     KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);

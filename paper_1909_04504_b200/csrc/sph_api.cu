@@ -300,7 +300,7 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
     masks[dest] = source_mask;
     int rc = zero_counter(c, CNT_PAIRS_ACCEL); if (rc) return rc;
     rc = zero_counter(c, CNT_CAND_ACCEL); if (rc) return rc;
-    rc = launch_accel(c, masks, arho != nullptr, false); if (rc) return rc;
+    rc = launch_accel(c, masks, arho != nullptr, 0u); if (rc) return rc;
     if (ax || ay || az || arho) { OutPtrs O; memset(&O, 0, sizeof(O)); O.ax = ax; O.ay = ay; O.az = az; O.arho = arho; return emit(c, dest, O, mem); }
     return SPH_OK;
 }
@@ -345,9 +345,24 @@ static int evaluate(sph_ctx* c, bool continuity) {
         fused[a] = same; plain[a] = acc && !same;
         only[a] = a < c->na && continuity && c->tbl_arho[a] != 0 && !same;
     }
-    rc = grouped(c->tbl_accel, fused, [&](const uint32_t* m) { return launch_accel(c, m, true, false); }); if (rc) return rc;
-    rc = grouped(c->tbl_accel, plain, [&](const uint32_t* m) { return launch_accel(c, m, false, false); }); if (rc) return rc;
-    rc = grouped(c->tbl_arho, only, [&](const uint32_t* m) { return launch_accel(c, m, true, true); }); if (rc) return rc;
+    // continuity mode: when no array needs two different source sets, ONE launch serves them all (fluid: momentum +
+    // continuity from {fluid, solid}; solid: continuity only from {fluid}; the per-lane source mask filters)
+    bool one = continuity;
+    for (int a = 0; a < c->na; ++a) if (plain[a] && only[a]) one = false;
+    if (one) {
+        uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 }, ao = 0u; bool any = false;
+        for (int a = 0; a < c->na; ++a) {
+            if (fused[a] || plain[a]) masks[a] = c->tbl_accel[a];
+            else if (only[a]) { masks[a] = c->tbl_arho[a]; ao |= 1u << a; }
+            any = any || masks[a] != 0u;
+        }
+        return any ? launch_accel(c, masks, true, ao) : SPH_OK;
+    }
+    rc = grouped(c->tbl_accel, fused, [&](const uint32_t* m) { return launch_accel(c, m, true, 0u); }); if (rc) return rc;
+    rc = grouped(c->tbl_accel, plain, [&](const uint32_t* m) { return launch_accel(c, m, false, 0u); }); if (rc) return rc;
+    rc = grouped(c->tbl_arho, only, [&](const uint32_t* m) {
+        uint32_t ao = 0u; for (int a = 0; a < c->na; ++a) if (m[a]) ao |= 1u << a;
+        return launch_accel(c, m, true, ao); }); if (rc) return rc;
     return SPH_OK;
 }
 

@@ -85,4 +85,4 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
                           int64_t* total, int mem);
 // sph_density.cu / sph_accel.cu: one launch serves every dest array whose mask is non-zero
 int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record);
-int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, bool arho_only);
+int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, uint32_t arho_only);
