@@ -106,7 +106,10 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     SPH_CUDA_OK(c, cudaMalloc(&c->cell_count, (size_t)(c->max_keys + 2) * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMalloc(&c->cell_start, (size_t)(c->max_keys + 2) * sizeof(uint32_t)));
     const size_t scan_n = (size_t)(c->max_keys > tot ? c->max_keys : tot) + 2;
-    SPH_CUDA_OK(c, cudaMalloc(&c->block_sums, (scan_n / 2048 + 4) * sizeof(uint32_t)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->scan_state, (scan_n / 2048 + 4) * sizeof(unsigned long long)));
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_state, 0, (scan_n / 2048 + 4) * sizeof(unsigned long long), c->stream));
+    SPH_CUDA_OK(c, cudaMalloc(&c->scan_ticket, sizeof(uint32_t)));
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_ticket, 0, sizeof(uint32_t), c->stream));
     SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(float)));
     SPH_CUDA_OK(c, cudaMalloc(&c->counters, CNT_COUNT * sizeof(unsigned long long)));
     SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 2 * sizeof(float)));
@@ -134,7 +137,7 @@ extern "C" int sph_destroy(sph_ctx* c) {
     }
     cudaFree(c->S[0].acc); cudaFree(c->S[1].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
     cudaFree(c->nl.pool); cudaFree(c->nl.head); cudaFree(c->nl.used);
-    cudaFree(c->block_sums); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
+    cudaFree(c->scan_state); cudaFree(c->scan_ticket); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
     for (int k = 0; k < c->prof_cap; ++k) { cudaEventDestroy(c->prof[k].a); cudaEventDestroy(c->prof[k].b); }
     free(c->prof);
     delete c;

@@ -29,7 +29,8 @@ struct sph_ctx {
                                // sph_pc_step it is consumed by k_update before the sort and rewritten after it)
     int cur;
     uint32_t *key, *rank;      // per particle, pre-sort order
-    uint32_t *cell_count, *cell_start, *block_sums;
+    uint32_t *cell_count, *cell_start;
+    unsigned long long* scan_state; uint32_t* scan_ticket; uint32_t scan_epoch;   // k_scan look-back table
     float* staging;            // host<->device staging for SPH_MEM_HOST (10 floats per particle of capacity)
     float* out_tmp;            // device scratch for caller-order outputs (4 floats per particle of capacity)
     unsigned long long* counters;     // device, CNT_COUNT entries

@@ -126,7 +126,7 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
 }
 
 // ------------------------------------------------------------------------------------------------
-// exclusive scan of n uint32 (out has n+1 entries; out[n] = total): reduce / scan of block sums / final.
+// exclusive scan of n uint32 (out has n+1 entries; out[n] = total), one launch.
 // ------------------------------------------------------------------------------------------------
 #define SCAN_T 512
 #define SCAN_ITEMS 4
@@ -151,55 +151,62 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
     return r;
 }
 
+// Single-pass scan with decoupled look-back: tile t publishes its aggregate, then warp 0 sums the aggregates of
+// its predecessors, 32 at a time, back to the nearest tile whose inclusive prefix is already known.  Tiles take
+// their number from a ticket, so every predecessor of a running tile is running or done (no deadlock).  A state
+// word is {epoch-tagged flag, value}; the epoch changes with every scan, so the table is never cleared.
 __global__ void __launch_bounds__(SCAN_T)
-k_scan_reduce(const uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ block_sums) {
-    const long long b0 = (long long)blockIdx.x * SCAN_TILE;
-    uint32_t s = 0;
-#pragma unroll
-    for (int k = 0; k < SCAN_ITEMS; ++k) { long long i = b0 + k * SCAN_T + threadIdx.x; if (i < n) s += in[i]; }
-    __shared__ uint32_t tot;
-    block_exclusive_scan(s, &tot);
+k_scan(const uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int nb,
+       unsigned long long* __restrict__ state, uint32_t* __restrict__ ticket, uint32_t epoch) {
+    __shared__ uint32_t s_tile, s_total, s_prefix;
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
     __syncthreads();
-    if (threadIdx.x == 0) block_sums[blockIdx.x] = tot;
-}
-
-__global__ void __launch_bounds__(SCAN_T)
-k_scan_blocks(uint32_t* __restrict__ block_sums, int nb) {       // single block, in place -> exclusive
-    __shared__ uint32_t carry, tot;
-    if (threadIdx.x == 0) carry = 0;
-    __syncthreads();
-    for (int b0 = 0; b0 < nb; b0 += SCAN_T) {
-        const int i = b0 + threadIdx.x;
-        const uint32_t v = i < nb ? block_sums[i] : 0u;
-        const uint32_t ex = block_exclusive_scan(v, &tot);
-        if (i < nb) block_sums[i] = ex + carry;
-        __syncthreads();
-        if (threadIdx.x == 0) carry += tot;
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) block_sums[nb] = carry;
-}
-
-__global__ void __launch_bounds__(SCAN_T)
-k_scan_final(const uint32_t* __restrict__ in, long long n, const uint32_t* __restrict__ block_sums,
-             uint32_t* __restrict__ out, int nb) {
-    const long long b0 = (long long)blockIdx.x * SCAN_TILE;
-    const long long i0 = b0 + (long long)threadIdx.x * SCAN_ITEMS;
+    const uint32_t tile = s_tile;
+    const long long i0 = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
     uint32_t v[SCAN_ITEMS], s = 0;
 #pragma unroll
     for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (i0 + k < n) ? in[i0 + k] : 0u; s += v[k]; }
-    uint32_t ex = block_exclusive_scan(s, nullptr) + block_sums[blockIdx.x];
+    uint32_t ex = block_exclusive_scan(s, &s_total);
+    __syncthreads();
+    const uint32_t total = s_total;
+    const uint32_t F_AGG = 2u * epoch + 1u, F_INC = 2u * epoch + 2u;
+    volatile unsigned long long* vs = state;
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        uint32_t prefix = 0u;
+        if (tile > 0) {
+            if (lane == 0) vs[tile] = ((unsigned long long)F_AGG << 32) | total;
+            long long p = (long long)tile - 1;                    // look back over tiles p, p-1, ... (lane = distance)
+            for (;;) {
+                const long long q = p - lane;
+                unsigned long long w = 0ull; uint32_t f = F_INC;   // tiles before 0 count as "inclusive, 0"
+                if (q >= 0) { do { w = vs[q]; f = (uint32_t)(w >> 32); } while (f != F_AGG && f != F_INC); }
+                const unsigned inc = __ballot_sync(SPH_FULL_MASK, f == F_INC);
+                const int stop = inc ? __ffs(inc) - 1 : 32;        // nearest tile with a known inclusive prefix
+                uint32_t add = (lane <= stop && q >= 0) ? (uint32_t)w : 0u;
+                for (int o = 16; o > 0; o >>= 1) add += __shfl_xor_sync(SPH_FULL_MASK, add, o);
+                prefix += add;
+                if (inc) break;
+                p -= 32;
+            }
+        }
+        if (lane == 0) {
+            vs[tile] = ((unsigned long long)F_INC << 32) | (prefix + total);
+            s_prefix = prefix;
+            if ((int)tile == nb - 1) { out[n] = prefix + total; *ticket = 0u; }   // last tile: grand total, ticket reset
+        }
+    }
+    __syncthreads();
+    ex += s_prefix;
 #pragma unroll
     for (int k = 0; k < SCAN_ITEMS; ++k) { if (i0 + k < n) out[i0 + k] = ex; ex += v[k]; }
-    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = block_sums[nb];
 }
 
 static int scan_exclusive(sph_ctx* c, const uint32_t* in, uint32_t* out, long long n) {
     const int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
     if (nb == 0) { SPH_CUDA_OK(c, cudaMemsetAsync(out, 0, sizeof(uint32_t), c->stream)); return SPH_OK; }
-    SPH_LAUNCH(c, SPH_K_SCAN, k_scan_reduce, nb, SCAN_T, 0, in, n, c->block_sums);
-    SPH_LAUNCH(c, SPH_K_SCAN, k_scan_blocks, 1, SCAN_T, 0, c->block_sums, nb);
-    SPH_LAUNCH(c, SPH_K_SCAN, k_scan_final, nb, SCAN_T, 0, in, n, c->block_sums, out, nb);
+    c->scan_epoch = c->scan_epoch >= 0x3fffffffu ? 1u : c->scan_epoch + 1u;
+    SPH_LAUNCH(c, SPH_K_SCAN, k_scan, nb, SCAN_T, 0, in, n, out, nb, c->scan_state, c->scan_ticket, c->scan_epoch);
     return SPH_OK;
 }
 
