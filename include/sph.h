@@ -39,7 +39,7 @@ extern "C" {
 #endif
 
 #define SPH_MAX_ARRAYS 4
-#define SPH_ABI_VERSION 3
+#define SPH_ABI_VERSION 4
 
 typedef struct sph_ctx sph_ctx;
 
@@ -65,6 +65,12 @@ enum sph_density_mode {
     SPH_DENSITY_CONTINUITY = 1  /* rho integrated from eq.7 (L126), as the paper's dam break (L142, L369-374) */
 };
 
+enum sph_integrator {
+    SPH_INTEGRATOR_PC = 0,      /* predictor-corrector, eqs. 12-14 (L148-152), R10 (default)             */
+    SPH_INTEGRATOR_EULER = 1    /* forward Euler, the paper's worked example (L335, Fig.2), R22:
+                                   x += dt u ; u += dt a ; rho += dt arho, all from the values of step n        */
+};
+
 enum sph_mem { SPH_MEM_DEVICE = 0, SPH_MEM_HOST = 1 };
 enum sph_array_flags { SPH_ARRAY_DYNAMIC = 0, SPH_ARRAY_FIXED = 1 /* x,u never updated (tank walls, L142) */ };
 
@@ -80,6 +86,10 @@ typedef struct sph_params {
     double alpha, eps;          /* artificial viscosity (R9): Pi = -alpha c0 mu/rhobar, mu = h vr/(r^2+eps h^2) */
     double g[3];                /* body force = initial value of the accumulator (Listing 4) */
     int move;                   /* 1: sph_pc_step applies eq.13 (default); 0: positions frozen (config C5) */
+    double nu, eta;             /* laminar viscosity, eq.10 (L134-136): a_i += sum_j m_j 4 nu/(rho_i+rho_j)
+                                 * (r_ij . grad_i W_ij)/(r_ij^2 + eta h_ij^2) u_ij, in the same pair loop as eq.9.
+                                 * nu = 0 (default): term off.  eta: the paper's regulariser (0.01 is customary) */
+    int integrator;             /* enum sph_integrator: what sph_pc_step steps with */
     /* Tuning knobs of the neighbour search; results do not depend on them (0 = default). */
     int xsub;                   /* x sub-cells per support radius (default 4, 1..16): finer x-interval culling   */
     int nlist_slots;            /* record pool of the pair passes, in rows of 32 words per warp (32 particles) of
@@ -183,7 +193,9 @@ int sph_summation_density(sph_ctx* ctx, int dest, uint32_t source_mask, float* r
 int sph_wcsph_accel(sph_ctx* ctx, int dest, uint32_t source_mask,
                     float* ax, float* ay, float* az, float* arho, int mem);
 
-/* n_steps predictor-corrector steps, eqs. 12-14 (L148-152), R10/R11, on the context's state:
+/* n_steps time steps on the context's state.  sph_params.integrator == SPH_INTEGRATOR_EULER: forward Euler
+ * (see enum sph_integrator), one evaluation per step.  Default: predictor-corrector, eqs. 12-14 (L148-152),
+ * DESIGN.md R10/R11:
  *   [a^0 = F(x^0,u^0) on the first call after a build]
  *   u += dt/2 a ; x += dt u (+ periodic wrap, L443) ; NNPS rebuilt (L443) ; [rho = eq.3] ; EOS ; a = F ; u += dt/2 a
  * density_mode selects eq.3 or the integrated eq.7 (rho stepped like u, on every array).

@@ -16,7 +16,9 @@
 //                         (the paper only says "classic scheme of [36]", L185);
 //                         arho_i += m_j (v_i-v_j).grad_i W_ij             (eq.7; Listing 4)
 //   loop structure        for d_idx: for s_idx in neighbours(d_idx): loop(...)   (Listing 7)
-// The integrator (eqs. 12-14) is per-particle arithmetic and lives in sph_oracle.py.
+//   orc_visc_laminar      a_i += m_j 4 nu/(rho_i+rho_j) (r_ij.grad_i W_ij)/(r^2 + eta h^2) u_ij     (eq.10)
+// The integrators (eqs. 12-14; forward Euler, Fig.2) are per-particle arithmetic and live in
+// sph_oracle.py.
 //
 // Readings: symmetric h_ij = (h_i+h_j)/2 (R3); strict '<' (R4); self pair included (R5);
 // minimum image applied to the difference (R6); grad W := 0 at r = 0 (R18).
@@ -375,6 +377,39 @@ ORC_API void orc_accel(const orc_domain* dom, int kernel, double alpha, double e
         pairs += c;
     }
     if (n_pairs) *n_pairs += pairs;
+}
+
+// Laminar viscosity, eq.10 (L134-136), added to the accelerations when nu != 0:
+//   a_visc,i = sum_j m_j 4 nu / (rho_i + rho_j) * (r_ij . grad_i W_ij) / (|r_ij|^2 + eta h_ij^2) * u_ij
+// (h in the regulariser read as h_ij, R3).  visc_power accumulates u_i . a_visc,i for the dissipation pin.
+ORC_API void orc_visc_laminar(const orc_domain* dom, int kernel, double nu, double eta, int pred32, int method,
+               int64_t nd, const double* xd, const double* yd, const double* zd,
+               const double* ud, const double* vd, const double* wd, const double* hd, const double* rhod,
+               int64_t ns, const double* xs, const double* ys, const double* zs,
+               const double* us, const double* vs, const double* ws,
+               const double* hs, const double* ms, const double* rhos,
+               double* au, double* av, double* aw, double* abs_a, double* visc_power) {
+    double k = orc_support(kernel);
+    Pts D{nd, xd, yd, zd, hd}, S{ns, xs, ys, zs, hs};
+    CellGrid g; if (method) build_grid(g, dom, k, D, S);
+    #pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < nd; ++i) {
+        double sx = 0, sy = 0, sz = 0, sabs = 0;
+        for_neighbors(dom, k, pred32, method, &g, D, i, S, [&](int64_t j) {
+            PairGeom pg = geom64(dom, xd, yd, zd, hd, i, xs, ys, zs, hs, j);
+            if (pg.r == 0.0) return;                               // R18: grad W = 0
+            double dw = orc_dWdr(kernel, dom->dim, pg.r, pg.hij);
+            double rdw = dw * pg.r;                                // r_ij . grad_i W_ij = dW/dr * r
+            double vx = ud[i] - us[j], vy = vd[i] - vs[j];
+            double vz = dom->dim == 3 ? wd[i] - ws[j] : 0.0;
+            double c = ms[j] * 4.0 * nu / (rhod[i] + rhos[j]) * rdw / (pg.r * pg.r + eta * pg.hij * pg.hij);
+            sx += c * vx; sy += c * vy; sz += c * vz;
+            sabs += std::fabs(c) * std::sqrt(vx * vx + vy * vy + vz * vz);
+        });
+        au[i] += sx; av[i] += sy; if (aw) aw[i] += sz;
+        if (abs_a) abs_a[i] += sabs;
+        if (visc_power) visc_power[i] += sx * ud[i] + sy * vd[i] + (dom->dim == 3 ? sz * wd[i] : 0.0);
+    }
 }
 
 ORC_API int orc_num_threads(void) {          // threads the OpenMP loops above actually use (bench cpu_baseline "cores")

@@ -63,6 +63,9 @@ def lib():
         L.orc_accel.restype = None
         L.orc_accel.argtypes = [C.POINTER(_Domain), C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int,
                                 C.c_int64] + [_DP] * 9 + [C.c_int64] + [_DP] * 10 + [_DP] * 7 + [_IP]
+        L.orc_visc_laminar.restype = None
+        L.orc_visc_laminar.argtypes = [C.POINTER(_Domain), C.c_int, C.c_double, C.c_double, C.c_int, C.c_int,
+                                       C.c_int64] + [_DP] * 8 + [C.c_int64] + [_DP] * 9 + [_DP] * 5
         L.orc_num_threads.restype = C.c_int
         L.orc_set_num_threads.argtypes = [C.c_int]
         _lib = L
@@ -180,7 +183,7 @@ def eos(wl, rho: np.ndarray) -> np.ndarray:
 
 
 def accel(wl, st: State, dest: int, sources: Sequence[int], pred32: bool = True, method: str = "cell",
-          gravity: bool = True, alpha: Optional[float] = None, subset=None):
+          gravity: bool = True, alpha: Optional[float] = None, subset=None, nu: Optional[float] = None):
     """eq.8-9 + Pi_ij (+ eq.7): dict(au,av,aw,arho,abs_a,abs_arho,visc_power,n_pairs) for array `dest`.
     The accumulators start at g (Listing 4: gravity is the initial value) and arho at 0 (L402-403)."""
     L = lib(); dom = _domain(wl); kid = KERNEL_ID[wl.kernel]
@@ -199,6 +202,15 @@ def accel(wl, st: State, dest: int, sources: Sequence[int], pred32: bool = True,
                     _p(out["au"]), _p(out["av"]), _p(out["aw"]), _p(out["arho"]),
                     _p(out["abs_a"]), _p(out["abs_arho"]), _p(out["visc_power"]),
                     npairs.ctypes.data_as(_IP))
+    nu_ = float(getattr(wl, "nu", 0.0) if nu is None else nu)
+    out["lam_power"] = np.zeros(nd)
+    if nu_ != 0.0:                                        # laminar viscosity, eq.10 (L134-136)
+        for s in sources:
+            S = st.arrays[s]
+            L.orc_visc_laminar(C.byref(dom), kid, nu_, float(getattr(wl, "eta", 0.01)), int(pred32), _method(method),
+                               nd, *(_p(D[c]) for c in ("x", "y", "z", "u", "v", "w", "h", "rho")),
+                               len(S["x"]), *(_p(S[c]) for c in ("x", "y", "z", "u", "v", "w", "h", "m", "rho")),
+                               _p(out["au"]), _p(out["av"]), _p(out["aw"]), _p(out["abs_a"]), _p(out["lam_power"]))
     out["n_pairs"] = int(npairs[0])
     return out
 
@@ -281,4 +293,31 @@ def pc_step(wl, st: State, dt: float, mode: str, move: bool = True, pred32: bool
                     A[vel] = A[vel] + 0.5 * dt * A[acc]                               # (14)
         if mode == "continuity":
             A["rho"] = A["rho"] + 0.5 * dt * A["arho"]
+    return pairs
+
+
+def euler_step(wl, st: State, dt: float, mode: str, move: bool = True, pred32: bool = False,
+               method: str = "cell") -> int:
+    """One forward-Euler step ("a simple forward Euler integrator", Fig.2; R22):
+         a^n = F(x^n, u^n, rho^n)          (evaluated on the first call, afterwards carried over)
+         x^{n+1} = x^n + dt u^n ; u^{n+1} = u^n + dt a^n ; rho^{n+1} = rho^n + dt arho^n (continuity mode)
+         periodic wrap (L443) ; a^{n+1} = F(x^{n+1}, u^{n+1}, rho^{n+1})
+       Fixed arrays keep x,u."""
+    pairs = 0
+    if not st.have_accel:
+        pairs += evaluate(wl, st, mode, pred32, method)
+    comps = (("u", "au", "x"), ("v", "av", "y"), ("w", "aw", "z"))
+    for A in st.arrays:
+        if not A["fixed"]:
+            for k, (vel, acc, pos) in enumerate(comps):
+                if k >= wl.dim:
+                    continue
+                if move:
+                    A[pos] = A[pos] + dt * A[vel]
+                    if wl.periodic[k]:
+                        A[pos] = _wrap(A[pos], float(wl.lo[k]), float(wl.hi[k]))
+                A[vel] = A[vel] + dt * A[acc]
+        if mode == "continuity":
+            A["rho"] = A["rho"] + dt * A["arho"]
+    pairs += evaluate(wl, st, mode, pred32, method)
     return pairs

@@ -19,6 +19,7 @@ SPH_MAX_ARRAYS = 4
 KERNEL_ID = {"cubic": 0, "quintic": 1, "wendland_c2": 2}
 SUMMATION, CONTINUITY = 0, 1
 MODE_ID = {"summation": SUMMATION, "continuity": CONTINUITY}
+INTEGRATOR_ID = {"pc": 0, "euler": 1}
 MEM_DEVICE, MEM_HOST = 0, 1
 ARRAY_DYNAMIC, ARRAY_FIXED = 0, 1
 
@@ -39,6 +40,7 @@ class sph_domain(C.Structure):
 class sph_params(C.Structure):
     _fields_ = [("kernel", C.c_int), ("rho0", C.c_double), ("c0", C.c_double), ("gamma", C.c_double),
                 ("alpha", C.c_double), ("eps", C.c_double), ("g", C.c_double * 3), ("move", C.c_int),
+                ("nu", C.c_double), ("eta", C.c_double), ("integrator", C.c_int),
                 ("xsub", C.c_int), ("nlist_slots", C.c_int)]
 
 
@@ -140,7 +142,8 @@ class SphContext:
 
     def __init__(self, *, dim: int, lo, hi, periodic, kernel: str, rho0: float, c0: float, gamma: float = 7.0,
                  alpha: float = 0.1, eps: float = 0.01, g=(0.0, 0.0, 0.0), move: bool = True,
-                 capacity: Sequence[int], stream=None, xsub: int = 0, nlist_slots: int = 0):
+                 capacity: Sequence[int], stream=None, xsub: int = 0, nlist_slots: int = 0,
+                 nu: float = 0.0, eta: float = 0.01, integrator: str = "pc"):
         import torch
         if not torch.cuda.is_available():
             raise SphError(-7, "no CUDA device: the SPH path has no CPU fallback")
@@ -151,6 +154,7 @@ class SphContext:
         prm = sph_params(); prm.kernel = KERNEL_ID[kernel]
         prm.rho0, prm.c0, prm.gamma, prm.alpha, prm.eps, prm.move = rho0, c0, gamma, alpha, eps, int(move)
         prm.xsub, prm.nlist_slots = int(xsub), int(nlist_slots)
+        prm.nu, prm.eta, prm.integrator = float(nu), float(eta), INTEGRATOR_ID[integrator]
         for k in range(3):
             dom.lo[k], dom.hi[k], dom.periodic[k] = float(lo[k]), float(hi[k]), int(bool(periodic[k]))
             prm.g[k] = float(g[k])
@@ -171,7 +175,7 @@ class SphContext:
     @classmethod
     def from_workload(cls, wl, stream=None, capacity=None, **over):
         kw = dict(dim=wl.dim, lo=wl.lo, hi=wl.hi, periodic=wl.periodic, kernel=wl.kernel, rho0=wl.rho0, c0=wl.c0,
-                  gamma=wl.gamma, alpha=wl.alpha, eps=wl.eps, g=wl.g,
+                  gamma=wl.gamma, alpha=wl.alpha, eps=wl.eps, g=wl.g, nu=wl.nu, eta=wl.eta, integrator=wl.integrator,
                   capacity=capacity or [a.n for a in wl.arrays], stream=stream)
         kw.update(over)
         return cls(**kw)

@@ -12,7 +12,7 @@
 // L372-374): the same loop, only arho is stored.
 struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
 
-template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, bool PEOS>
+template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, bool PEOS, bool LAMINAR>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
 k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
              uint32_t arho_only_arrays, NList nl, unsigned long long* __restrict__ counters) {
@@ -31,7 +31,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
     const float iLx = 1.0f / g.L[0], iLy = 1.0f / g.L[1], iLz = 1.0f / g.L[2];
     const float sigma = pc.sigma, h_c = pc.h_const, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
-    const float visc = pc.visc, eps = pc.eps;
+    const float visc = pc.visc, eps = pc.eps, nu4 = pc.nu4, eta = pc.eta;
     const float hi = VARH ? pi.w : h_c;
     // PEOS (constant h, gamma = 7, every p is the EOS of its rho): the neighbour's rho rides in velm.w and its
     // p/rho^2 is recomputed, two 16-byte gathers per pair instead of three (the loop is L1-gather bound); the
@@ -81,6 +81,12 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         ax = fmaf(sc, dx, ax); ay = fmaf(sc, dy, ay);
         if (DIM == 3) az = fmaf(sc, dz, az);
         if (ARHO) ar = fmaf(mg, vr, ar);
+        if (LAMINAR) {                                                  // laminar viscosity, eq.10 (launches with nu != 0)
+            // m_j 4nu/(rho_i+rho_j) (r.gradW)/(r^2 + eta h^2) u_ij,  r.gradW = gc r^2
+            const float lam = mg * nu4 * r2 * rcp_approx(fmaf(eta * hij, hij, r2) * (rho_i + rho_j));
+            ax = fmaf(lam, vx, ax); ay = fmaf(lam, vy, ay);
+            if (DIM == 3) az = fmaf(lam, vi.z - s.vj.z, az);
+        }
     };
     const uint32_t idle = in ? (uint32_t)i : 0u;
     auto drain = [&](uint32_t nz, bool shifted) { per = shifted; tile_drain<AccelSrc>(ws, nz, idle, load, compute); };
@@ -114,15 +120,18 @@ static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, uint32_
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
     const uint32_t ao = arho_only;
     const bool peos = c->p_is_eos && c->pc.gamma_is_7 && !varh;
-#define LT(VARH, ARHO, FILTER, REPLAY, PEOS) \
-        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PEOS>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
-#define LT1(VARH, ARHO, FILTER, PEOS) do { if (replay) LT(VARH, ARHO, FILTER, true, PEOS); else LT(VARH, ARHO, FILTER, false, PEOS); } while (0)
+    const bool lam = c->pc.nu4 != 0.0f;
+#define LT(VARH, ARHO, FILTER, REPLAY, PEOS, LAM) \
+        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PEOS, LAM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
+#define LT0(VARH, ARHO, FILTER, REPLAY, PEOS) do { if (lam) LT(VARH, ARHO, FILTER, REPLAY, PEOS, true); else LT(VARH, ARHO, FILTER, REPLAY, PEOS, false); } while (0)
+#define LT1(VARH, ARHO, FILTER, PEOS) do { if (replay) LT0(VARH, ARHO, FILTER, true, PEOS); else LT0(VARH, ARHO, FILTER, false, PEOS); } while (0)
 #define LT2(VARH, ARHO, PEOS) do { if (filter) LT1(VARH, ARHO, true, PEOS); else LT1(VARH, ARHO, false, PEOS); } while (0)
 #define LT3(VARH, PEOS) do { if (want_arho) LT2(VARH, true, PEOS); else LT2(VARH, false, PEOS); } while (0)
     if (varh) LT3(true, false); else if (peos) LT3(false, true); else LT3(false, false);
 #undef LT3
 #undef LT2
 #undef LT1
+#undef LT0
 #undef LT
     return SPH_OK;
 }

@@ -49,6 +49,7 @@ static void set_consts(sph_ctx* c) {
     pc.gamma_is_7 = (P.gamma == 7.0);
     pc.visc = (float)(-2.0 * P.alpha * P.c0);
     pc.eps = (float)P.eps;
+    pc.nu4 = (float)(4.0 * P.nu); pc.eta = (float)P.eta;
     for (int k = 0; k < 3; ++k) pc.g[k] = (float)P.g[k];
     pc.all_mask = (1u << c->na) - 1u;
     pc.h_const = 1.0f; pc.hinv_const = 1.0f; pc.fac_const = 1.0f;
@@ -63,6 +64,8 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     if (params->kernel < 0 || params->kernel > SPH_KERNEL_WENDLAND_C2) return SPH_ERR_BAD_ARG;
     if (!(params->rho0 > 0) || !(params->c0 > 0) || !(params->gamma > 0)) return SPH_ERR_BAD_ARG;
     if (params->xsub < 0 || params->xsub > 16) return SPH_ERR_BAD_ARG;
+    if (params->integrator != SPH_INTEGRATOR_PC && params->integrator != SPH_INTEGRATOR_EULER) return SPH_ERR_BAD_ARG;
+    if (!(params->nu >= 0) || !(params->eta >= 0)) return SPH_ERR_BAD_ARG;
     for (int k = 0; k < domain->dim; ++k) if (!(domain->hi[k] > domain->lo[k])) return SPH_ERR_BAD_ARG;
     int64_t tot = 0;
     for (int a = 0; a < n_arrays; ++a) {
@@ -379,14 +382,16 @@ extern "C" int sph_pc_step(sph_ctx* c, double dt, int n_steps, int density_mode)
     if (!c->have_accel || (cont && !c->have_arho)) {                                             // a^0 = F(x^0, u^0)
         rc = evaluate(c, cont); if (rc) return rc; c->have_accel = true; c->have_arho = cont;
     }
+    const bool euler = c->prm.integrator == SPH_INTEGRATOR_EULER;
     for (int s = 0; s < n_steps; ++s) {
-        rc = nnps_update_key_hist(c, (float)dt, s > 0, true, cont, true); if (rc) return rc;    // (14 of step s-1) + 12 + 13 + key
+        // PC: (14 of step s-1) + 12 + 13 + key.   Euler: x += dt u ; u += dt a ; rho += dt arho ; key.
+        rc = nnps_update_key_hist(c, (float)dt, !euler && s > 0, true, cont, true); if (rc) return rc;
         rc = nnps_sort_from_keys(c, false); if (rc) return rc;                                  // NNPS rebuilt every step (L443)
         rc = evaluate(c, cont); if (rc) return rc;
         c->have_arho = cont;
         c->steps_done++;
     }
-    if (n_steps > 0) { rc = nnps_update_key_hist(c, (float)dt, true, false, cont, false); if (rc) return rc; }   // eq.14
+    if (n_steps > 0 && !euler) { rc = nnps_update_key_hist(c, (float)dt, true, false, cont, false); if (rc) return rc; }   // eq.14
     return SPH_OK;
 }
 

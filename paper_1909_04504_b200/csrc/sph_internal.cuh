@@ -48,6 +48,7 @@ struct PairConsts {
     int   gamma_is_7;
     float visc;                // -2 alpha c0   (Pi = visc * h vr / ((r2 + eps h^2)(rho_i + rho_j)))
     float eps;
+    float nu4, eta;            // laminar viscosity eq.10: 4 nu (0 = term off) and its regulariser
     float g[3];
     uint32_t src_mask[SPH_MAX_ARRAYS];   // per DEST array: source-array bitmask; 0 = not a destination of this launch
     uint32_t all_mask;         // (1 << na) - 1

@@ -73,7 +73,7 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
 // way on EVERY array (the tank particles too, L142) and re-evaluates the EOS (group 1 of Listing 3).
 // ------------------------------------------------------------------------------------------------
 struct UpdateArgs {
-    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho;
+    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho, euler;
     int fixed[SPH_MAX_ARRAYS];
 };
 
@@ -93,12 +93,18 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
             vel.x = fmaf(U.dt_half, a.x, vel.x); vel.y = fmaf(U.dt_half, a.y, vel.y);
             if (g.dim == 3) vel.z = fmaf(U.dt_half, a.z, vel.z);
         }
+        if (U.euler && U.move) {                                        // forward Euler: x^{n+1} = x^n + dt u^n (old u)
+            pos.x = fmaf(U.dt, vel.x, pos.x); pos.y = fmaf(U.dt, vel.y, pos.y);
+            if (g.dim == 3) pos.z = fmaf(U.dt, vel.z, pos.z);
+        }
         if (U.kick1) {
             vel.x = fmaf(U.dt_half, a.x, vel.x); vel.y = fmaf(U.dt_half, a.y, vel.y);   // eq.12
             if (g.dim == 3) vel.z = fmaf(U.dt_half, a.z, vel.z);
             if (U.move) {                                                // eq.13 + periodic wrap
-                pos.x = fmaf(U.dt, vel.x, pos.x); pos.y = fmaf(U.dt, vel.y, pos.y);
-                if (g.dim == 3) pos.z = fmaf(U.dt, vel.z, pos.z);
+                if (!U.euler) {
+                    pos.x = fmaf(U.dt, vel.x, pos.x); pos.y = fmaf(U.dt, vel.y, pos.y);
+                    if (g.dim == 3) pos.z = fmaf(U.dt, vel.z, pos.z);
+                }
                 if (g.per[0]) { if (pos.x >= g.hi[0]) pos.x -= g.L[0]; else if (pos.x < g.lo[0]) pos.x += g.L[0]; }
                 if (g.per[1]) { if (pos.y >= g.hi[1]) pos.y -= g.L[1]; else if (pos.y < g.lo[1]) pos.y += g.L[1]; }
                 if (g.dim == 3 && g.per[2]) { if (pos.z >= g.hi[2]) pos.z -= g.L[2]; else if (pos.z < g.lo[2]) pos.z += g.L[2]; }
@@ -241,7 +247,9 @@ int nnps_key_hist(sph_ctx* c) {
 int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey) {
     const int n = (int)c->n_total;
     UpdateArgs U;
-    U.dt_half = 0.5f * dt; U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
+    U.euler = c->prm.integrator == SPH_INTEGRATOR_EULER ? 1 : 0;
+    U.dt_half = U.euler ? dt : 0.5f * dt;              // Euler: the one kick per step is a full dt
+    U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
     U.continuity = continuity; U.rekey = rekey; U.w_rho = c->variable_h ? 0 : 1;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
     if (rekey) SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));

@@ -73,6 +73,9 @@ class Workload:
     density_sources: Optional[List[List[int]]] = None   # per dest array
     accel_sources: Optional[List[List[int]]] = None      # per dynamic dest array ([] for fixed)
     arho_sources: Optional[List[List[int]]] = None       # continuity mode, per dest array
+    nu: float = 0.0                                      # laminar kinematic viscosity of eq.10 (L134-136); 0 = term off
+    eta: float = 0.01                                    # its regulariser eta (eq.10)
+    integrator: str = "pc"                               # "pc" (eqs. 12-14) or "euler" (L335, Fig.2)
 
     @property
     def n_total(self) -> int:

@@ -103,3 +103,32 @@ def test_record_pool_overflow_falls_back_to_searching(WL):
         for o in (o1, o2):
             scale = np.abs(o0[k]).max()
             assert np.abs(o[k].astype(np.float64) - o0[k]).max() <= 2e-6 * scale, k
+
+
+@pytest.mark.parametrize("name", ["dam2d_euler_laminar", "3d_per_euler_laminar", "3d_varh_pc_laminar"])
+def test_laminar_viscosity_and_euler_steps(O, WL, name):
+    """eq.10 in the pair loop (nu > 0) and the forward-Euler integrator of the paper's worked example (L335,
+    Fig.2): a^0 + two steps on the GPU == the oracle's, from the same state (second step from the GPU's state)."""
+    if name == "dam2d_euler_laminar":
+        wl, mode = WL.dam_break_2d(dx=0.04), "continuity"
+        wl.integrator, wl.nu = "euler", 1.0e-3
+        wl.arrays[0].u[:] = np.random.default_rng(9).uniform(-0.5, 0.5, wl.arrays[0].n).astype(np.float32)
+    elif name == "3d_per_euler_laminar":
+        wl, mode = WL.periodic_box_3d((16, 16, 16), seed=4), "summation"
+        wl.integrator, wl.nu = "euler", 5.0e-3
+    else:
+        wl, mode = WL.random_box(n=4000, dim=3, periodic=True, seed=62, kernel="cubic", variable_h=True), "summation"
+        wl.nu = 2.0e-3
+    step = O.euler_step if wl.integrator == "euler" else O.pc_step
+    ctx, _ = make_ctx(wl)
+    ctx.pc_step(wl.dt, 1, mode)
+    st = O.State(wl)
+    step(wl, st, wl.dt, mode)
+    _compare_state(wl, ctx, st, name + " step1")
+    # the viscous term must be there: the same step with nu = 0 differs by far more than the tolerance
+    nu = wl.nu; wl.nu = 0.0
+    st0 = O.State(wl); step(wl, st0, wl.dt, mode); wl.nu = nu
+    d = np.abs(st0.arrays[0]["u"] - st.arrays[0]["u"]).max() / np.abs(st.arrays[0]["u"]).max()
+    assert d > 20 * TOL, f"nu has no visible effect in this case ({d:.2e})"
+    ctx.synchronize()
+    ctx.close()
