@@ -20,7 +20,13 @@ LIB = os.environ.get("SPH_B200_LIB") or os.path.join(HERE, "libsph_b200.so")
 EXTRA = os.environ.get("SPH_B200_NVCC_FLAGS", "").split()
 OBJ = os.path.join(HERE, "build" if not os.environ.get("SPH_B200_LIB") else
                    "build_" + hashlib.sha256(LIB.encode()).hexdigest()[:8])
-SOURCES = ["sph_api.cu", "sph_nnps.cu", "sph_density.cu", "sph_accel.cu", "sph_probe.cu"]
+# (source, extra defines, object): sph_accel.cu is compiled once per smoothing kernel (its instantiations dominate
+# the build time) and once as the dispatcher
+SOURCES = [("sph_api.cu", [], "sph_api.o"), ("sph_nnps.cu", [], "sph_nnps.o"), ("sph_density.cu", [], "sph_density.o"),
+           ("sph_probe.cu", [], "sph_probe.o"), ("sph_accel.cu", [], "sph_accel.o"),
+           ("sph_accel.cu", ["-DSPH_ACCEL_KERNEL=0"], "sph_accel_k0.o"),
+           ("sph_accel.cu", ["-DSPH_ACCEL_KERNEL=1"], "sph_accel_k1.o"),
+           ("sph_accel.cu", ["-DSPH_ACCEL_KERNEL=2"], "sph_accel_k2.o")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
@@ -39,7 +45,7 @@ def _digest() -> str:
         p = os.path.normpath(os.path.join(CSRC, n))
         if os.path.isfile(p):
             h.update(n.encode()); h.update(open(p, "rb").read())
-    h.update(" ".join(ARCH + FLAGS + EXTRA).encode())
+    h.update(" ".join(ARCH + FLAGS + EXTRA + [repr(SOURCES)]).encode())
     return h.hexdigest()
 
 
@@ -51,9 +57,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = _nvcc()
 
-    def compile_one(src: str) -> str:
-        obj = os.path.join(OBJ, src.replace(".cu", ".o"))
-        cmd = [nvcc, *ARCH, *FLAGS, *EXTRA, "-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
+    def compile_one(item) -> str:
+        src, defs, oname = item
+        obj = os.path.join(OBJ, oname)
+        cmd = [nvcc, *ARCH, *FLAGS, *EXTRA, *defs, "-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]
         r = subprocess.run(cmd, capture_output=True, text=True)

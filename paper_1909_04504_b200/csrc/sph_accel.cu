@@ -10,6 +10,13 @@
 // custom tables).  REPLAY = true: it replays the hit masks recorded by the density pass of the same evaluation
 // and tests nothing.  ARHO_ONLY launches serve ContinuityEquation(dest=solid, sources=[fluid]) (Listing 3
 // L372-374): the same loop, only arho is stored.
+// This file is compiled four times (build.py): once per smoothing kernel with -DSPH_ACCEL_KERNEL=<id> (the kernel
+// template and its launcher launch_accel_k<id>), and once without (the dispatcher launch_accel).
+int launch_accel_k0(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay);
+int launch_accel_k1(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay);
+int launch_accel_k2(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay);
+
+#ifdef SPH_ACCEL_KERNEL
 struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
 
 template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, bool PEOS, bool LAMINAR>
@@ -70,10 +77,10 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         const float vx = vi.x - s.vj.x, vy = vi.y - s.vj.y;
         float vr = fmaf(vy, dy, vx * dx);
         if (DIM == 3) vr = fmaf(vi.z - s.vj.z, dz, vr);
-        // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
         const float mj = VARH ? s.vj.w : s.pj.w;                        // SortedState: constant h keeps m in posh.w
         const float rho_j = PEOS ? s.vj.w : s.rj.x;
         const float pr_j = PEOS ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y;
+        // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
         const float den = fmaf(eps * hij, hij, r2) * (rho_i + rho_j);
         const float Pi = vr < 0.0f ? visc * hij * vr * rcp_approx(den) : 0.0f;
         const float mg = has ? mj * gc : 0.0f;                          // a lane that has run out contributes nothing
@@ -83,7 +90,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         if (ARHO) ar = fmaf(mg, vr, ar);
         if (LAMINAR) {                                                  // laminar viscosity, eq.10 (launches with nu != 0)
             // m_j 4nu/(rho_i+rho_j) (r.gradW)/(r^2 + eta h^2) u_ij,  r.gradW = gc r^2
-            const float lam = mg * nu4 * r2 * rcp_approx(fmaf(eta * hij, hij, r2) * (rho_i + rho_j));
+            const float lam = mg * nu4 * r2 * rcp_approx(fmaxf(fmaf(eta * hij, hij, r2) * (rho_i + rho_j), 1.0e-30f));
             ax = fmaf(lam, vx, ax); ay = fmaf(lam, vy, ay);
             if (DIM == 3) az = fmaf(lam, vi.z - s.vj.z, az);
         }
@@ -136,6 +143,14 @@ static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, uint32_
     return SPH_OK;
 }
 
+#define SPH_CAT2(a, b) a##b
+#define SPH_CAT(a, b) SPH_CAT2(a, b)
+int SPH_CAT(launch_accel_k, SPH_ACCEL_KERNEL)(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay) {
+    return dim == 2 ? launch_accel_tile_kd<SPH_ACCEL_KERNEL, 2>(c, filter, want_arho, arho_only, replay)
+                    : launch_accel_tile_kd<SPH_ACCEL_KERNEL, 3>(c, filter, want_arho, arho_only, replay);
+}
+
+#else
 // One launch serves every destination array whose mask is non-zero.  arho_only: bit a = array a stores only its
 // continuity sum (ContinuityEquation(dest=solid, sources=[fluid]), Listing 3).
 int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, uint32_t arho_only) {
@@ -147,10 +162,11 @@ int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, 
     }
     c->last_used_rows = use_list;
     const int k = c->prm.kernel, d = c->grid.dim;
-#define KD(K, D) if (k == K && d == D) return launch_accel_tile_kd<K, D>(c, filter, want_arho || arho_only != 0u, arho_only, use_list)
-    KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
-    KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
-    KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);
-#undef KD
+    if (d != 2 && d != 3) return sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
+    const bool wa = want_arho || arho_only != 0u;
+    if (k == SPH_KERNEL_CUBIC)       return launch_accel_k0(c, d, filter, wa, arho_only, use_list);
+    if (k == SPH_KERNEL_QUINTIC)     return launch_accel_k1(c, d, filter, wa, arho_only, use_list);
+    if (k == SPH_KERNEL_WENDLAND_C2) return launch_accel_k2(c, d, filter, wa, arho_only, use_list);
     return sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
 }
+#endif

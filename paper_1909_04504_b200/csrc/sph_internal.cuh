@@ -132,10 +132,13 @@ __device__ __forceinline__ float eos_pressure(float rho, float rho0, float B, fl
 
 // p/rho^2 of the Tait EOS with gamma = 7 from rho alone (the momentum pair loop recomputes it per neighbour
 // instead of gathering it): same polynomial as eos_pressure, t formed with a multiplication by 1/rho0.
-__device__ __forceinline__ float eos7_p_over_rho2(float rho, float rho0, float inv_rho0, float B) {
+__device__ __forceinline__ float eos7_p(float rho, float rho0, float inv_rho0, float B) {
     const float t = (rho - rho0) * inv_rho0;
     const float s = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.0f, 7.0f), 21.0f), 35.0f), 35.0f), 21.0f), 7.0f);
-    return B * s * rcp_approx(rho * rho);
+    return B * s;
+}
+__device__ __forceinline__ float eos7_p_over_rho2(float rho, float rho0, float inv_rho0, float B) {
+    return eos7_p(rho, rho0, inv_rho0, B) * rcp_approx(rho * rho);
 }
 
 // Cell coordinate of a position on one axis (clamped; out-of-range on a non-periodic axis is flagged by the caller).
