@@ -114,6 +114,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
     bool ing = false, done = false, seg_shift = false;
     int seg = NSEG;                                   // forces the first group set-up
     uint32_t b0 = 0u, e = 0u;
+    unsigned segs = 0u;                               // non-empty runs of the current group still to stream
     float2 sx = f2(0.0f, 0.0f), sy = sx, sz = sx;
 
     while (!done) {
@@ -135,6 +136,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
                     const int cy = grow % nc1, cz = grow / nc1;
                     const int a = sub_lo - xsub, b = sub_hi + xsub;
                     __syncwarp();
+                    bool nonempty = false;
                     if (lane < NSEG) {                // lane = 9 (oz+1) + 3 (oy+1) + part
                         const int part = lane % 3, oy = (lane / 3) % 3 - 1, oz = DIM == 3 ? lane / 9 - 1 : 0;
                         int y2 = cy + oy, z2 = cz + oz; uint32_t code = 0u; bool ok = true;
@@ -153,11 +155,15 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
                             e_ = __ldg(cell_start + (size_t)(rowbase + (uint32_t)c1 + 1u) * na);
                         }
                         ws.seg_s[lane] = s_; ws.seg_e[lane] = e_; ws.seg_c[lane] = code;
+                        nonempty = s_ < e_;
                     }
+                    segs = __ballot_sync(SPH_FULL_MASK, nonempty);      // runs that hold candidates
                     __syncwarp();
                     seg = -1; b0 = e = 0u;
                     continue;
                 }
+                if (segs == 0u) { seg = NSEG; b0 = e = 0u; continue; }   // group done
+                seg = __ffs(segs) - 1; segs &= segs - 1u;
                 b0 = ws.seg_s[seg]; e = ws.seg_e[seg];
                 const uint32_t code = ws.seg_c[seg];      // image shifts: 1 -> -L (wrapped below), 2 -> +L (wrapped above)
                 seg_shift = code != 0u;
