@@ -87,7 +87,8 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     default_tables(c);
     set_consts(c);
     c->xsub = params->xsub ? params->xsub : 4;
-    if (const char* e = getenv("SPH_XSUB")) { int v = atoi(e); if (v >= 1 && v <= 16) c->xsub = v; }   // tuning override
+    c->xsub_auto = params->xsub == 0;
+    if (const char* e = getenv("SPH_XSUB")) { int v = atoi(e); if (v >= 1 && v <= 16) { c->xsub = v; c->xsub_auto = false; } }   // tuning override
     int nl_slots = params->nlist_slots ? params->nlist_slots : 192;
     if (const char* e = getenv("SPH_NLIST_SLOTS")) { int v = atoi(e); if (v != 0) nl_slots = v; }
     *out = c;                                  // so the caller can read sph_last_error / destroy on failure
@@ -167,6 +168,7 @@ static int size_grid(sph_ctx* c) {
     if (!(cutoff > 0.0)) return sph_fail(c, SPH_ERR_BAD_ARG, "h_max must be positive");
     double scale = 1.0;
     int xsub = c->xsub;
+    if (c->xsub_auto && c->variable_h) xsub = 8;       // variable h: finer x windows pay (reach < cell for small-h groups)
     for (int iter = 0; iter < 64; ++iter) {
         int64_t total = 1; bool ok = true;
         for (int k = 0; k < 3; ++k) {

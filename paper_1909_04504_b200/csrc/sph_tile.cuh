@@ -134,7 +134,15 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
                     const int grow = __shfl_sync(SPH_FULL_MASK, row, first);
                     const int sub_lo = __shfl_sync(SPH_FULL_MASK, sub, first), sub_hi = __shfl_sync(SPH_FULL_MASK, sub, last);
                     const int cy = grow % nc1, cz = grow / nc1;
-                    const int a = sub_lo - xsub, b = sub_hi + xsub;
+                    // x reach in sub-cells: a pair of the group is closer than R = k (h_group_max + h_max) / 2, so
+                    // its sub-cell indices differ by at most floor(R / sub-cell) + 1 (<= xsub: cell >= k h_max)
+                    int nx = xsub;
+                    if (VARH) {
+                        const float hg = __uint_as_float(__reduce_max_sync(SPH_FULL_MASK, ing ? __float_as_uint(pi.w) : 0u));
+                        const float R = pc.kh * (hg + pc.h_const) * 1.0001f;
+                        nx = min(xsub, __float2int_rd(R * g.inv_cell[0]) + 1);
+                    }
+                    const int a = sub_lo - nx, b = sub_hi + nx;
                     __syncwarp();
                     bool nonempty = false;
                     if (lane < NSEG) {                // lane = 9 (oz+1) + 3 (oy+1) + part
