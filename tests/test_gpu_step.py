@@ -132,3 +132,28 @@ def test_laminar_viscosity_and_euler_steps(O, WL, name):
     assert d > 20 * TOL, f"nu has no visible effect in this case ({d:.2e})"
     ctx.synchronize()
     ctx.close()
+
+
+def test_dense_cells_span_several_record_blocks(O, WL):
+    """~100 particles per cell: a warp's candidate stream is > 30 batches, so the mask store is drained and
+    recorded in several blocks per warp and the momentum pass replays a chain of blocks.  Same pairs and the same
+    step as with no record pool, and parity with the oracle."""
+    wl = WL.random_box(n=12000, dim=3, periodic=True, seed=71, kernel="cubic", h_mean=0.1)
+    outs = []
+    for slots in (0, -1):
+        ctx, _ = make_ctx(wl, nlist_slots=slots)
+        ctx.pc_step(wl.dt, 1, "summation")
+        ctx.synchronize()
+        s = ctx.get_stats()
+        outs.append((s, {k: v.cpu().numpy() for k, v in ctx.sync_state(0).items()}))
+        if slots == 0:
+            assert s.used_rows == 1 and s.nlist_fallback_warps == 0
+            assert s.nlist_rows_used > 2 * 32 * ((wl.arrays[0].n + 31) // 32)      # > 2 blocks of 30 per warp
+            st = O.State(wl)
+            O.pc_step(wl, st, wl.dt, "summation")
+            _compare_state(wl, ctx, st, "dense step1")
+        ctx.close()
+    (s0, o0), (s1, o1) = outs
+    assert s0.pairs_density == s0.pairs_accel == s1.pairs_density == s1.pairs_accel
+    for k in ("x", "u", "v", "w", "rho"):
+        assert np.abs(o1[k].astype(np.float64) - o0[k]).max() <= 2e-6 * np.abs(o0[k]).max(), k
