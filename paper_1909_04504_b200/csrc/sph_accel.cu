@@ -20,7 +20,7 @@ int launch_accel_k2(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t a
 struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
 
 template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, bool PEOS, bool LAMINAR>
-__global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
+__global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS_ACCEL)
 k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
              uint32_t arho_only_arrays, NList nl, unsigned long long* __restrict__ counters) {
     __shared__ TileWarpSmem smem[TILE_WARPS];
