@@ -27,7 +27,7 @@
 #define TILE_MIN_BLOCKS 8                 // resident blocks per SM the pair kernels are compiled for (64 registers)
 #endif
 #ifndef TILE_MIN_BLOCKS_ACCEL
-#define TILE_MIN_BLOCKS_ACCEL 7           // the momentum kernel is 3 % faster with 72 registers and 7 blocks (measured, C3)
+#define TILE_MIN_BLOCKS_ACCEL 6           // the momentum kernel is 3-8 % faster with 80 registers and 6 blocks (measured, C3, C4)
 #endif
 #ifndef TILE_MMAX
 #define TILE_MMAX 30                       // masks per warp before a forced drain (<= 30: 30 bases + 2 words = one header row)
