@@ -394,6 +394,28 @@ def run_ours(args):
                "sample": f"{wl_small.name}: {done} oracle PC steps of {wl_small.n_total} particles "
                          f"(same spacing, h, kernel, parameters) after the a^0 evaluation; {sec:.1f} s"}
 
+    # BASELINE.json configs[1] (C2, the 2-D dam break run for its 1,000 steps) beside the headline workload: it is
+    # launch-latency bound at 23,618 particles, so it is reported, not used for the roofline
+    also = None
+    if args.workload == "C3" and not args.no_also:
+        wl2 = make_workload("C2", 0)
+        with torch.cuda.stream(stream):
+            c2 = binding.SphContext.from_workload(wl2, stream=stream)
+            c2.nnps_build(binding.device_arrays(wl2), [a.fixed for a in wl2.arrays])
+            c2.pc_step(wl2.dt, 20, wl2.density_mode)                     # a^0 + warm-up steps
+            c2.synchronize()
+            a2, b2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a2.record(stream); c2.pc_step(wl2.dt, wl2.n_steps, wl2.density_mode); b2.record(stream)
+            torch.cuda.synchronize()
+            c2.synchronize()                                             # raises on out-of-domain / non-finite (no fallback)
+            ms2 = a2.elapsed_time(b2)
+            s2 = c2.get_stats()
+            c2.close()
+        also = {"workload": workload_label("C2"), "steps": wl2.n_steps, "ms_total": ms2, "us_per_step": 1e3 * ms2 / wl2.n_steps,
+                "value": wl2.n_total * wl2.n_steps / (ms2 * 1e-3), "unit": UNIT,
+                "pair_interactions_per_sec": (s2.pairs_density + s2.pairs_accel) * wl2.n_steps / (ms2 * 1e-3),
+                "note": "one sph_pc_step(dt, 1000) call, continuity mode, device-resident, CUDA events; launch-latency bound"}
+
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
@@ -409,7 +431,7 @@ def run_ours(args):
                     "steps": Ke, "what": "sph_nnps_build(host pinned arrays + a^n) + sph_pc_step(dt,1) + sph_sync_state(host) per step"},
             "gpu_launches": int(launches),
             "roofline": roofline, "kernels": kernels, "hbm_kernels": hbm,
-            "cpu_baseline": cpu, "clocks": clocks}
+            "cpu_baseline": cpu, "clocks": clocks, "configs1_dam_break_2d": also}
     print(json.dumps(line), flush=True)
     ctx.close()
     if dist is not None:
@@ -428,6 +450,7 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=1000)
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="time budget of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the C2 (BASELINE configs[1]) side measurement")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -191,7 +191,8 @@ def taylor_green_2d(n: int = 64, seed: int = 0, jitter: float = 0.1, hdx: float 
 
 def dam_break_2d(dx: float = 0.01, n_steps: int = 1000, density_mode: str = CONTINUITY,
                  kernel: str = "quintic", hdx: float = 1.0) -> Workload:
-    """C2. Fluid block 1x2 (cell-centred, 100x200 = 20,000 at dx=0.01) in a 4x4 tank with 3 wall layers."""
+    """C2. Fluid block 1x2 (cell-centred, 100x200 = 20,000 at dx=0.01) in a 4x4 tank with 3 wall layers.
+    dt = 0.125 h/c0 (R24: BASELINE gives no time step for the dam breaks; 0.25 h/c0 is unstable here)."""
     fx, fy = _cell_centred((int(round(1.0 / dx)), int(round(2.0 / dx))), dx, (0.0, 0.0))
     sx, sy = tank_2d_open_top(dx, 4.0, 4.0, 3)
     rho0 = 1000.0
@@ -204,7 +205,7 @@ def dam_break_2d(dx: float = 0.01, n_steps: int = 1000, density_mode: str = CONT
     lo = (-3 * dx - pad, -3 * dx - pad, 0.0)
     hi = (4.0 + 3 * dx + pad, 4.0 + pad, 1.0)
     return Workload(f"C2_dam_break_2d_dx{dx:g}", 2, lo, hi, (False, False, False), kernel,
-                    rho0, float(c0), 7.0, 0.1, 0.01, (0.0, -9.81, 0.0), 0.25 * h / float(c0),
+                    rho0, float(c0), 7.0, 0.1, 0.01, (0.0, -9.81, 0.0), 0.125 * h / float(c0),
                     n_steps, density_mode, [fluid, solid], note="BASELINE.json configs[1]")
 
 
@@ -248,7 +249,7 @@ def dam_break_3d(dx: float = 0.005, n_steps: int = 50, density_mode: str = CONTI
     lo = (-3 * dx - pad, -3 * dx - pad, -3 * dx - pad)
     hi = (1.6 + 3 * dx + pad, 0.6 + 3 * dx + pad, 1.2 + pad)
     return Workload(f"C4_dam_break_3d_dx{dx:g}", 3, lo, hi, (False, False, False), kernel,
-                    rho0, float(c0), 7.0, 0.1, 0.01, (0.0, 0.0, -9.81), 0.25 * h / float(c0),
+                    rho0, float(c0), 7.0, 0.1, 0.01, (0.0, 0.0, -9.81), 0.125 * h / float(c0),
                     n_steps, density_mode, [fluid, solid], note="BASELINE.json configs[3]")
 
 

@@ -132,13 +132,13 @@ def test_c3_full_density_accel_and_counts(O, WL):
 
 def test_c3_full_pc_steps_stay_finite_and_conserve_momentum(WL):
     """bench.py's timed configuration: sph_pc_step on C3.  Total momentum is conserved by the symmetric pair
-    terms (periodic box, no gravity): after 3 steps it equals the initial one to float32 round-off."""
+    terms (periodic box, no gravity): after the config's 100 steps it equals the initial one to float32 round-off."""
     wl = WL.periodic_box_3d((128, 128, 128), seed=1, dx=1.0 / 128)
     ctx, _ = make_ctx(wl)
     A = wl.arrays[0]
     m = A.m.astype(np.float64)
     p0 = np.array([(m * getattr(A, k).astype(np.float64)).sum() for k in ("u", "v", "w")])
-    ctx.pc_step(wl.dt, 3, "summation")
+    ctx.pc_step(wl.dt, wl.n_steps, "summation")
     ctx.synchronize()
     out = ctx.sync_state(0)
     p1 = np.array([(m * out[k].cpu().numpy().astype(np.float64)).sum() for k in ("u", "v", "w")])
@@ -148,7 +148,8 @@ def test_c3_full_pc_steps_stay_finite_and_conserve_momentum(WL):
         x = out[k].cpu().numpy()
         assert np.isfinite(x).all() and x.min() >= 0.0 and x.max() <= 1.0
     s = ctx.get_stats()
-    assert s.steps_done == 3 and s.used_rows == 1
+    assert wl.n_steps == 100 and s.steps_done == 100 and s.used_rows == 1
+    assert np.abs(out["rho"].cpu().numpy() / wl.rho0 - 1.0).max() < 0.2
     ctx.close()
 
 
@@ -209,4 +210,25 @@ def test_c5_full_variable_h(O, WL):
     sub = _sample(wl.arrays[0].n, N_SAMPLE, 132)
     assert np.array_equal(ctx.neighbor_counts(0, 0)[sub], _rows_count(O, wl, st, 0, [0], sub))
     ctx.synchronize()
+    ctx.close()
+
+
+def test_c2_full_run_of_1000_steps_stays_sane(WL):
+    """BASELINE configs[1] as stated: the 2-D dam break for its 1,000 predictor-corrector steps, NNPS rebuilt every
+    step.  No particle leaves the box, nothing non-finite (sph_synchronize raises otherwise), and the weakly
+    compressible density stays within a few per cent of rho0 (R24: with dt = 0.25 h/c0 this run
+    explodes near step 550, in the oracle as well)."""
+    wl = WL.dam_break_2d()
+    ctx, _ = make_ctx(wl)
+    ctx.pc_step(wl.dt, wl.n_steps, "continuity")
+    ctx.synchronize()
+    s = ctx.get_stats()
+    assert s.steps_done == 1000
+    for d in range(2):
+        out = {k: v.cpu().numpy() for k, v in ctx.sync_state(d).items()}
+        assert all(np.isfinite(v).all() for v in out.values())
+        assert np.abs(out["rho"] / wl.rho0 - 1.0).max() < 0.05
+    fluid = ctx.sync_state(0)
+    assert float(fluid["y"].min()) > 0.0 and float(fluid["x"].min()) > 0.0      # nobody went through the walls
+    assert float(fluid["x"].max()) > 1.0                                         # ... and the dam has started to collapse
     ctx.close()
