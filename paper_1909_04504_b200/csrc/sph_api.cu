@@ -124,8 +124,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
         c->nl.pool_rows = (uint32_t)rows;
         SPH_CUDA_OK(c, cudaMalloc(&c->nl.pool, rows * 32 * sizeof(uint32_t)));
         SPH_CUDA_OK(c, cudaMalloc(&c->nl.head, (warps + 2) * sizeof(uint32_t)));
-        SPH_CUDA_OK(c, cudaMalloc(&c->nl.used, sizeof(uint32_t)));
-        SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.used, 0, sizeof(uint32_t), c->stream));
+        c->nl.used = (uint32_t*)(c->counters + CNT_NL_USED);
     }
     SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
     for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMemsetAsync(c->S[b].acc, 0, N * sizeof(float4), c->stream));
@@ -140,7 +139,7 @@ extern "C" int sph_destroy(sph_ctx* c) {
         cudaFree(c->S[b].posh); cudaFree(c->S[b].velm); cudaFree(c->S[b].rp); cudaFree(c->S[b].meta); cudaFree(c->S[b].cell);
     }
     cudaFree(c->S[0].acc); cudaFree(c->S[1].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
-    cudaFree(c->nl.pool); cudaFree(c->nl.head); cudaFree(c->nl.used);
+    cudaFree(c->nl.pool); cudaFree(c->nl.head);
     cudaFree(c->scan_state); cudaFree(c->scan_ticket); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
     for (int k = 0; k < c->prof_cap; ++k) { cudaEventDestroy(c->prof[k].a); cudaEventDestroy(c->prof[k].b); }
     free(c->prof);
@@ -282,8 +281,8 @@ static int emit(sph_ctx* c, int array, OutPtrs O, int mem) {
     return SPH_OK;
 }
 
-static int zero_counter(sph_ctx* c, int which) {
-    SPH_CUDA_OK(c, cudaMemsetAsync(c->counters + which, 0, sizeof(unsigned long long), c->stream));
+static int zero_counters(sph_ctx* c, int first, int last) {       // one memset for counters [first, last]
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->counters + first, 0, (size_t)(last - first + 1) * sizeof(unsigned long long), c->stream));
     return SPH_OK;
 }
 
@@ -293,8 +292,7 @@ extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask,
     if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
     uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
     masks[dest] = source_mask;
-    int rc = zero_counter(c, CNT_PAIRS_DENSITY); if (rc) return rc;
-    rc = zero_counter(c, CNT_CAND_DENSITY); if (rc) return rc;
+    int rc = zero_counters(c, CNT_PAIRS_DENSITY, CNT_NL_USED); if (rc) return rc;
     rc = launch_density(c, masks, true); if (rc) return rc;
     if (rho_out || p_out) { OutPtrs O; memset(&O, 0, sizeof(O)); O.rho = rho_out; O.p = p_out; return emit(c, dest, O, mem); }
     return SPH_OK;
@@ -306,8 +304,7 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
     if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
     uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
     masks[dest] = source_mask;
-    int rc = zero_counter(c, CNT_PAIRS_ACCEL); if (rc) return rc;
-    rc = zero_counter(c, CNT_CAND_ACCEL); if (rc) return rc;
+    int rc = zero_counters(c, CNT_PAIRS_ACCEL, CNT_CAND_ACCEL); if (rc) return rc;
     rc = launch_accel(c, masks, arho != nullptr, 0u); if (rc) return rc;
     if (ax || ay || az || arho) { OutPtrs O; memset(&O, 0, sizeof(O)); O.ax = ax; O.ay = ay; O.az = az; O.arho = arho; return emit(c, dest, O, mem); }
     return SPH_OK;
@@ -317,10 +314,7 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
 // continuity + momentum.  Destinations that share a source mask share a launch.
 static int evaluate(sph_ctx* c, bool continuity) {
     int rc;
-    rc = zero_counter(c, CNT_PAIRS_DENSITY); if (rc) return rc;
-    rc = zero_counter(c, CNT_PAIRS_ACCEL); if (rc) return rc;
-    rc = zero_counter(c, CNT_CAND_DENSITY); if (rc) return rc;
-    rc = zero_counter(c, CNT_CAND_ACCEL); if (rc) return rc;
+    rc = zero_counters(c, CNT_PAIRS_DENSITY, CNT_CAND_ACCEL); if (rc) return rc;
     auto grouped = [&](const uint32_t* tbl, const bool* take, auto&& fn) -> int {
         bool done[SPH_MAX_ARRAYS] = { false, false, false, false };
         for (int a = 0; a < c->na; ++a) {

@@ -3,8 +3,11 @@
 #include "sph_internal.cuh"
 #include <stdio.h>
 
-enum { CNT_OUT_OF_DOMAIN = 0, CNT_NONFINITE = 1, CNT_PAIRS_DENSITY = 2, CNT_PAIRS_ACCEL = 3,
-       CNT_CAND_DENSITY = 4, CNT_OVERFLOW = 5, CNT_CAND_ACCEL = 6, CNT_COUNT = 8 };
+// device counters: [2..5] belong to a density (recording) pass, [6..7] to an acceleration pass, so that one
+// memset clears what a pass (or a whole evaluation: [2..7]) is about to count
+enum { CNT_OUT_OF_DOMAIN = 0, CNT_NONFINITE = 1, CNT_PAIRS_DENSITY = 2, CNT_CAND_DENSITY = 3, CNT_OVERFLOW = 4,
+       CNT_NL_USED = 5 /* low 32 bits: record rows handed out (NList::used) */, CNT_PAIRS_ACCEL = 6, CNT_CAND_ACCEL = 7,
+       CNT_COUNT = 8 };
 
 struct sph_ctx {
     cudaStream_t stream;

@@ -108,8 +108,7 @@ int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record) {
     c->nl_valid = false;
     if (record) {
         SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.head, 0, (size_t)((c->n_total + 31) / 32 + 1) * sizeof(uint32_t), c->stream));
-        SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.used, 0, sizeof(uint32_t), c->stream));
-        SPH_CUDA_OK(c, cudaMemsetAsync(c->counters + CNT_OVERFLOW, 0, sizeof(unsigned long long), c->stream));
+        // nl.used and the overflow counter live in the counter block the caller has just cleared (CNT_NL_USED)
     }
     const int k = c->prm.kernel, d = c->grid.dim;
     int rc = sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
