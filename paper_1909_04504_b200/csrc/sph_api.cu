@@ -260,6 +260,7 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     c->pc.hinv_const = (float)(1.0 / (double)c->h_max);
     c->pc.fac_const = (float)(kernel_sigma(c->prm.kernel, c->dom.dim) / pow((double)c->h_max, c->dom.dim));
     rc = size_grid(c); if (rc) return rc;
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));   // once per build; k_scan re-clears it
     rc = nnps_key_hist(c); if (rc) return rc;
     rc = nnps_sort_from_keys(c, true); if (rc) return rc;
     c->built = true; c->steps_done = 0; c->p_is_eos = !any_p;

@@ -162,8 +162,8 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
 // their number from a ticket, so every predecessor of a running tile is running or done (no deadlock).  A state
 // word is {epoch-tagged flag, value}; the epoch changes with every scan, so the table is never cleared.
 __global__ void __launch_bounds__(SCAN_T)
-k_scan(const uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int nb,
-       unsigned long long* __restrict__ state, uint32_t* __restrict__ ticket, uint32_t epoch) {
+k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int nb,
+       unsigned long long* __restrict__ state, uint32_t* __restrict__ ticket, uint32_t epoch, int zero_in) {
     __shared__ uint32_t s_tile, s_total, s_prefix;
     if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
     __syncthreads();
@@ -172,6 +172,10 @@ k_scan(const uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out,
     uint32_t v[SCAN_ITEMS], s = 0;
 #pragma unroll
     for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (i0 + k < n) ? in[i0 + k] : 0u; s += v[k]; }
+    if (zero_in) {                                                       // the histogram is consumed: leave it cleared for the next step
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) if (i0 + k < n) in[i0 + k] = 0u;
+    }
     uint32_t ex = block_exclusive_scan(s, &s_total);
     __syncthreads();
     const uint32_t total = s_total;
@@ -208,11 +212,11 @@ k_scan(const uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out,
     for (int k = 0; k < SCAN_ITEMS; ++k) { if (i0 + k < n) out[i0 + k] = ex; ex += v[k]; }
 }
 
-static int scan_exclusive(sph_ctx* c, const uint32_t* in, uint32_t* out, long long n) {
+static int scan_exclusive(sph_ctx* c, uint32_t* in, uint32_t* out, long long n, bool zero_in) {
     const int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
     if (nb == 0) { SPH_CUDA_OK(c, cudaMemsetAsync(out, 0, sizeof(uint32_t), c->stream)); return SPH_OK; }
     c->scan_epoch = c->scan_epoch >= 0x3fffffffu ? 1u : c->scan_epoch + 1u;
-    SPH_LAUNCH(c, SPH_K_SCAN, k_scan, nb, SCAN_T, 0, in, n, out, nb, c->scan_state, c->scan_ticket, c->scan_epoch);
+    SPH_LAUNCH(c, SPH_K_SCAN, k_scan, nb, SCAN_T, 0, in, n, out, nb, c->scan_state, c->scan_ticket, c->scan_epoch, zero_in ? 1 : 0);
     return SPH_OK;
 }
 
@@ -238,7 +242,7 @@ k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass,
 
 int nnps_key_hist(sph_ctx* c) {
     const int n = (int)c->n_total;
-    SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));
+    // cell_count is clear here: sph_nnps_build clears it after sizing the grid, every scan leaves it cleared
     if (n) SPH_LAUNCH(c, SPH_K_KEY, k_key_hist, (n + NB - 1) / NB, NB, 0, c->grid, c->S[c->cur], n, c->key, c->rank,
                       c->cell_count, c->counters);
     return SPH_OK;
@@ -252,7 +256,6 @@ int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, boo
     U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
     U.continuity = continuity; U.rekey = rekey; U.w_rho = c->variable_h ? 0 : 1;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
-    if (rekey) SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));
     if (n) SPH_LAUNCH(c, SPH_K_UPDATE, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
                       c->cell_count, c->counters);
     return SPH_OK;
@@ -260,7 +263,7 @@ int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, boo
 
 int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     const int n = (int)c->n_total;
-    int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys);
+    int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys, true);   // leaves cell_count cleared
     if (rc) return rc;
     if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
                       with_acc ? 1 : 0, (!c->variable_h && with_acc) ? 1 : 0, c->key, c->rank, c->cell_start);
@@ -353,7 +356,7 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
     else                  { if (c->variable_h) SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors_tile<3, true, FILL>), tgrid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); \
                             else SPH_LAUNCH(c, SPH_K_NEIGHBORS, (k_neighbors_tile<3, false, FILL>), tgrid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, (uint32_t)dest, (uint32_t)src, counts, off32, IDX); } } while (0)
     if (n) LN(false, (int32_t*)nullptr);
-    int rc = scan_exclusive(c, counts, off32, nd);
+    int rc = scan_exclusive(c, counts, off32, nd, false);
     if (rc) return rc;
     uint32_t tot32 = 0;
     SPH_CUDA_OK(c, cudaMemcpyAsync(&tot32, off32 + nd, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
