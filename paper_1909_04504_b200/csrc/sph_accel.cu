@@ -19,7 +19,7 @@ int launch_accel_k2(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t a
 #ifdef SPH_ACCEL_KERNEL
 struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
 
-template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, bool PEOS, bool LAMINAR>
+template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, int PM, bool LAMINAR>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS_ACCEL)
 k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
              uint32_t arho_only_arrays, NList nl, unsigned long long* __restrict__ counters) {
@@ -40,16 +40,19 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const float sigma = pc.sigma, h_c = pc.h_const, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
     const float visc = pc.visc, eps = pc.eps, nu4 = pc.nu4, eta = pc.eta;
     const float hi = VARH ? pi.w : h_c;
-    // PEOS (constant h, gamma = 7, every p is the EOS of its rho): the neighbour's rho rides in velm.w and its
-    // p/rho^2 is recomputed, two 16-byte gathers per pair instead of three (the loop is L1-gather bound); the
-    // destination's own term is recomputed the same way so that the pair terms stay antisymmetric.
+    // PM: where the neighbour's rho and p/rho^2 come from (the loop is L1-gather bound: fewer gathers pay).
+    //   0  gathered from rp (variable h; or caller-supplied p, gamma != 7 with non-uniform mass): three gathers
+    //   1  constant h, gamma = 7, every p is the EOS of its rho: rho rides in velm.w, p/rho^2 is recomputed (the
+    //      destination's own term too, so that the pair terms stay antisymmetric): two gathers
+    //   2  UM layout (constant h, uniform mass): rho in velm.w, p/rho^2 in posh.w, m = m_const: two gathers
     const float inv_rho0 = 1.0f / pc.rho0, rho0 = pc.rho0, Beos = pc.B;
-    const float rho_i = ri.x, pr_i = PEOS ? eos7_p_over_rho2(ri.x, rho0, inv_rho0, Beos) : ri.y;
+    const float rho_i = ri.x, pr_i = PM == 1 ? eos7_p_over_rho2(ri.x, rho0, inv_rho0, Beos) : ri.y;
+    const float m_const = pc.m_const;
     float ax = pc.g[0], ay = pc.g[1], az = pc.g[2], ar = 0.0f;      // gravity = accumulator init (Listing 4)
     unsigned long long fhits = 0, rhits = 0;                            // FILTER: hits passing the source mask; replayed hits
     auto load = [&](uint32_t j) {
         AccelSrc s; s.pj = __ldg(S.posh + j); s.vj = __ldg(S.velm + j); s.aid = 0u;
-        s.rj = PEOS ? make_float2(0.0f, 0.0f) : __ldg(S.rp + j);
+        s.rj = PM ? make_float2(0.0f, 0.0f) : __ldg(S.rp + j);
         if (FILTER) { if (my_mask != pc.all_mask) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS; }   // lanes fed by all arrays skip the gather
         return s;
     };
@@ -77,9 +80,9 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         const float vx = vi.x - s.vj.x, vy = vi.y - s.vj.y;
         float vr = fmaf(vy, dy, vx * dx);
         if (DIM == 3) vr = fmaf(vi.z - s.vj.z, dz, vr);
-        const float mj = VARH ? s.vj.w : s.pj.w;                        // SortedState: constant h keeps m in posh.w
-        const float rho_j = PEOS ? s.vj.w : s.rj.x;
-        const float pr_j = PEOS ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y;
+        const float mj = VARH ? s.vj.w : (PM == 2 ? m_const : s.pj.w);  // SortedState layouts
+        const float rho_j = PM ? s.vj.w : s.rj.x;
+        const float pr_j = PM == 2 ? s.pj.w : (PM == 1 ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y);
         // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
         const float den = fmaf(eps * hij, hij, r2) * (rho_i + rho_j);
         const float Pi = vr < 0.0f ? visc * hij * vr * rcp_approx(den) : 0.0f;
@@ -126,15 +129,15 @@ static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, uint32_
     SortedState& S = c->S[c->cur];
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
     const uint32_t ao = arho_only;
-    const bool peos = c->p_is_eos && c->pc.gamma_is_7 && !varh;
+    const int pm = varh ? 0 : (c->pc.uniform_m ? 2 : ((c->p_is_eos && c->pc.gamma_is_7) ? 1 : 0));
     const bool lam = c->pc.nu4 != 0.0f;
-#define LT(VARH, ARHO, FILTER, REPLAY, PEOS, LAM) \
-        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PEOS, LAM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
-#define LT0(VARH, ARHO, FILTER, REPLAY, PEOS) do { if (lam) LT(VARH, ARHO, FILTER, REPLAY, PEOS, true); else LT(VARH, ARHO, FILTER, REPLAY, PEOS, false); } while (0)
-#define LT1(VARH, ARHO, FILTER, PEOS) do { if (replay) LT0(VARH, ARHO, FILTER, true, PEOS); else LT0(VARH, ARHO, FILTER, false, PEOS); } while (0)
-#define LT2(VARH, ARHO, PEOS) do { if (filter) LT1(VARH, ARHO, true, PEOS); else LT1(VARH, ARHO, false, PEOS); } while (0)
-#define LT3(VARH, PEOS) do { if (want_arho) LT2(VARH, true, PEOS); else LT2(VARH, false, PEOS); } while (0)
-    if (varh) LT3(true, false); else if (peos) LT3(false, true); else LT3(false, false);
+#define LT(VARH, ARHO, FILTER, REPLAY, PM, LAM) \
+        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PM, LAM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
+#define LT0(VARH, ARHO, FILTER, REPLAY, PM) do { if (lam) LT(VARH, ARHO, FILTER, REPLAY, PM, true); else LT(VARH, ARHO, FILTER, REPLAY, PM, false); } while (0)
+#define LT1(VARH, ARHO, FILTER, PM) do { if (replay) LT0(VARH, ARHO, FILTER, true, PM); else LT0(VARH, ARHO, FILTER, false, PM); } while (0)
+#define LT2(VARH, ARHO, PM) do { if (filter) LT1(VARH, ARHO, true, PM); else LT1(VARH, ARHO, false, PM); } while (0)
+#define LT3(VARH, PM) do { if (want_arho) LT2(VARH, true, PM); else LT2(VARH, false, PM); } while (0)
+    if (varh) LT3(true, 0); else if (pm == 2) LT3(false, 2); else if (pm == 1) LT3(false, 1); else LT3(false, 0);
 #undef LT3
 #undef LT2
 #undef LT1

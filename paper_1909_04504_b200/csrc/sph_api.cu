@@ -116,7 +116,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_ticket, 0, sizeof(uint32_t), c->stream));
     SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(float)));
     SPH_CUDA_OK(c, cudaMalloc(&c->counters, CNT_COUNT * sizeof(unsigned long long)));
-    SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 2 * sizeof(float)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 4 * sizeof(float)));
     if (nl_slots > 0 && tot > 0) {
         const size_t warps = (size_t)(tot + 31) / 32;
         size_t rows = warps * (size_t)nl_slots + 32;
@@ -249,13 +249,15 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
     c->cur = 0;
     int rc = nnps_pack(c, P); if (rc) return rc;
-    int hmm[2] = { 0, 0 };
+    int hmm[4] = { 0, 0, 0, 0 };
     SPH_CUDA_OK(c, cudaMemcpyAsync(hmm, c->hminmax, sizeof(hmm), cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
     if (tot == 0) { c->h_min = c->h_max = 1.0f; }
     else { memcpy(&c->h_min, &hmm[0], 4); memcpy(&c->h_max, &hmm[1], 4); }
     if (!(c->h_max > 0.0f) || !isfinite(c->h_max)) return sph_fail(c, SPH_ERR_BAD_ARG, "smoothing lengths must be positive and finite");
     c->variable_h = (c->h_min != c->h_max);
+    c->pc.uniform_m = (tot > 0 && !c->variable_h && hmm[2] == hmm[3]) ? 1 : 0;
+    memcpy(&c->pc.m_const, &hmm[3], 4);
     c->pc.h_const = c->h_max;
     c->pc.hinv_const = (float)(1.0 / (double)c->h_max);
     c->pc.fac_const = (float)(kernel_sigma(c->prm.kernel, c->dom.dim) / pow((double)c->h_max, c->dom.dim));

@@ -37,7 +37,7 @@ struct sph_ctx {
     float* staging;            // host<->device staging for SPH_MEM_HOST (10 floats per particle of capacity)
     float* out_tmp;            // device scratch for caller-order outputs (4 floats per particle of capacity)
     unsigned long long* counters;     // device, CNT_COUNT entries
-    float* hminmax;            // device, 2 floats (as ordered ints)
+    float* hminmax;            // device, 4 floats (as ordered ints): h min/max, |m| min/max
 
     // neighbour rows recorded by a density launch for the acceleration launch that follows it
     NList nl;                  // nl.pool == nullptr: recording disabled

@@ -6,7 +6,7 @@
 
 struct DensitySrc { float4 pj; float mj; uint32_t aid; };
 
-template <int KERNEL, int DIM, bool VARH, bool FILTER, bool RECORD>
+template <int KERNEL, int DIM, bool VARH, bool FILTER, bool RECORD, bool UM>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
 k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
                NList nl, unsigned long long* __restrict__ counters) {
@@ -27,6 +27,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     const float iLx = 1.0f / g.L[0], iLy = 1.0f / g.L[1], iLz = 1.0f / g.L[2];
     const float sigma = pc.sigma, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
     const float hi = VARH ? pi.w : pc.h_const;
+    const float mfac_c = pc.m_const * pc.fac_const;                     // UM layout: posh.w is p/rho^2, the mass is m_const
     float rho = 0.0f;
     unsigned long long fhits = 0;                                       // FILTER: hits that pass the source mask
     // constant h: posh.w of the sorted state carries the MASS (SortedState), one 16-byte gather per pair
@@ -48,15 +49,14 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         if (DIM == 3) r2 = fmaf(dz, dz, r2);
         const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;
         const float r = r2 * rinv;
-        float hinv, fac, mj;
+        float hinv, mfac;
         if (VARH) {
             hinv = rcp_approx(0.5f * (hi + s.pj.w));
-            fac = sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
-            mj = s.mj;
-        } else { hinv = hinv_c; fac = fac_c; mj = s.pj.w; }
+            mfac = s.mj * sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
+        } else { hinv = hinv_c; mfac = UM ? mfac_c : s.pj.w * fac_c; }
         float f, df;
         kernel_profile<KERNEL, DIM>(r * hinv, f, df);
-        rho = has ? fmaf(mj * fac, f, rho) : rho;
+        rho = has ? fmaf(mfac, f, rho) : rho;
     };
 
     TileState st; st.reset(); st.tests = 0; st.hits = 0;
@@ -74,6 +74,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
         S.rp[i] = make_float2(rho, p / (rho * rho));
         if (!VARH) S.velm[i].w = rho;                                   // constant h: velm.w carries rho (SortedState)
+        if (UM) S.posh[i].w = p / (rho * rho);                          // UM layout: posh.w carries p/rho^2
         if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
     const unsigned long long h = warp_sum_u64(FILTER ? fhits : st.hits), t = warp_sum_u64(st.tests);
@@ -86,11 +87,11 @@ static int launch_density_tile_kd(sph_ctx* c, bool filter, bool record) {
     if (n == 0) return SPH_OK;
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
     SortedState& S = c->S[c->cur];
-#define LD(VARH, FILTER, RECORD) \
-        SPH_LAUNCH(c, SPH_K_DENSITY, (k_density_tile<KERNEL, DIM, VARH, FILTER, RECORD>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters)
-#define LD2(VARH, FILTER) do { if (record) LD(VARH, FILTER, true); else LD(VARH, FILTER, false); } while (0)
-#define LD3(VARH) do { if (filter) LD2(VARH, true); else LD2(VARH, false); } while (0)
-    if (c->variable_h) LD3(true); else LD3(false);
+#define LD(VARH, FILTER, RECORD, UM) \
+        SPH_LAUNCH(c, SPH_K_DENSITY, (k_density_tile<KERNEL, DIM, VARH, FILTER, RECORD, UM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters)
+#define LD2(VARH, FILTER, UM) do { if (record) LD(VARH, FILTER, true, UM); else LD(VARH, FILTER, false, UM); } while (0)
+#define LD3(VARH, UM) do { if (filter) LD2(VARH, true, UM); else LD2(VARH, false, UM); } while (0)
+    if (c->variable_h) LD3(true, false); else if (c->pc.uniform_m) LD3(false, true); else LD3(false, false);
 #undef LD3
 #undef LD2
 #undef LD

@@ -48,6 +48,7 @@ struct PairConsts {
     int   gamma_is_7;
     float visc;                // -2 alpha c0   (Pi = visc * h vr / ((r2 + eps h^2)(rho_i + rho_j)))
     float eps;
+    float m_const; int uniform_m;   // constant h and every particle of every array has the same mass: the UM layout
     float nu4, eta;            // laminar viscosity eq.10: 4 nu (0 = term off) and its regulariser
     float g[3];
     uint32_t src_mask[SPH_MAX_ARRAYS];   // per DEST array: source-array bitmask; 0 = not a destination of this launch
@@ -57,10 +58,13 @@ struct PairConsts {
 // Cell-sorted particle state (struct of float4 groups: one 16-B vector load per candidate test).
 struct SortedState {
     float4* posh;              // x, y, z, h          | constant h (h_min == h_max; the kernels then take h from
-    float4* velm;              // u, v, w, m          | PairConsts): after the sort posh = (x, y, z, M) and velm =
-                               //                     | (u, v, w, RHO), so that the density pair loop gathers ONE
-                               //                     | 16-byte word per neighbour and the momentum pair loop TWO
-                               //                     | (p/rho^2 is recomputed from rho when p is the EOS of rho)
+    float4* velm;              // u, v, w, m          | PairConsts): after the sort velm = (u, v, w, RHO) and posh =
+                               //                     | (x, y, z, M), so that the density pair loop gathers ONE 16-byte
+                               //                     | word per neighbour and the momentum pair loop TWO (p/rho^2 is
+                               //                     | recomputed from rho when p is the EOS of rho).  UM layout (all
+                               //                     | masses equal too, PairConsts::uniform_m): posh = (x, y, z,
+                               //                     | P/RHO^2) and the mass is the constant m_const: two gathers, no
+                               //                     | recomputation.
     float2* rp;                // rho, p / rho^2   (p itself is returned as (p/rho^2) * rho^2)
     float4* acc;               // ax, ay, az, arho
     uint32_t* meta;            // (array << 28) | original index

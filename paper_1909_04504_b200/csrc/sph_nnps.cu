@@ -27,7 +27,7 @@ __device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, bool& o
 __global__ void __launch_bounds__(NB)
 k_pack(PackArgs A, SortedState S, int n, PairConsts pc, int* __restrict__ hminmax) {
     const int gidx = blockIdx.x * NB + threadIdx.x;
-    float hmin = 3.0e38f, hmax = 0.0f;
+    float hmin = 3.0e38f, hmax = 0.0f, mmin = 3.0e38f, mmax = 0.0f;
     if (gidx < n) {
         int a = 0;
         while (a + 1 < A.na && gidx >= A.base[a + 1]) ++a;
@@ -43,14 +43,19 @@ k_pack(PackArgs A, SortedState S, int n, PairConsts pc, int* __restrict__ hminma
         S.acc[gidx] = make_float4(s.ax ? s.ax[i] : 0.0f, s.ay ? s.ay[i] : 0.0f, s.az ? s.az[i] : 0.0f,
                                   s.arho ? s.arho[i] : 0.0f);
         hmin = hmax = h;
+        mmin = mmax = fabsf(s.m ? s.m[i] : 0.0f);
     }
     for (int o = 16; o > 0; o >>= 1) {
         hmin = fminf(hmin, __shfl_xor_sync(SPH_FULL_MASK, hmin, o));
         hmax = fmaxf(hmax, __shfl_xor_sync(SPH_FULL_MASK, hmax, o));
+        mmin = fminf(mmin, __shfl_xor_sync(SPH_FULL_MASK, mmin, o));
+        mmax = fmaxf(mmax, __shfl_xor_sync(SPH_FULL_MASK, mmax, o));
     }
     if ((threadIdx.x & 31) == 0 && hmax > 0.0f) {      // positive floats order like their bit patterns
         atomicMin(&hminmax[0], __float_as_int(hmin));
         atomicMax(&hminmax[1], __float_as_int(hmax));
+        atomicMin(&hminmax[2], __float_as_int(mmin));          // |m|: uniform mass is detected for the UM state layout
+        atomicMax(&hminmax[3], __float_as_int(mmax));
     }
 }
 
@@ -73,7 +78,7 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
 // way on EVERY array (the tank particles too, L142) and re-evaluates the EOS (group 1 of Listing 3).
 // ------------------------------------------------------------------------------------------------
 struct UpdateArgs {
-    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho, euler;
+    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho, w_prr, euler;
     int fixed[SPH_MAX_ARRAYS];
 };
 
@@ -120,6 +125,7 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
         S.rp[i] = make_float2(rho, p / (rho * rho));
         if (U.w_rho) S.velm[i].w = rho;         // constant h: velm.w of the sorted state carries rho (SortedState)
+        if (U.w_prr) S.posh[i].w = p / (rho * rho);   // ... and, with uniform mass, posh.w carries p/rho^2
     }
     if (U.rekey) {
         bool oob;
@@ -231,7 +237,8 @@ k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass,
     float4 p = A.posh[i];
     float4 v = A.velm[i];
     const float2 r = A.rp[i];
-    if (w_mass) { p.w = v.w; v.w = r.x; }       // constant h, first sort after the pack: posh.w <- m, velm.w <- rho (SortedState)
+    // constant h, first sort after the pack (SortedState): velm.w <- rho; posh.w <- m, or <- p/rho^2 when the mass is uniform
+    if (w_mass) { p.w = w_mass == 2 ? r.y : v.w; v.w = r.x; }
     B.posh[d] = p;
     B.velm[d] = v;
     B.rp[d] = r;
@@ -254,7 +261,7 @@ int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, boo
     U.euler = c->prm.integrator == SPH_INTEGRATOR_EULER ? 1 : 0;
     U.dt_half = U.euler ? dt : 0.5f * dt;              // Euler: the one kick per step is a full dt
     U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
-    U.continuity = continuity; U.rekey = rekey; U.w_rho = c->variable_h ? 0 : 1;
+    U.continuity = continuity; U.rekey = rekey; U.w_rho = c->variable_h ? 0 : 1; U.w_prr = (!c->variable_h && c->pc.uniform_m) ? 1 : 0;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
     if (n) SPH_LAUNCH(c, SPH_K_UPDATE, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
                       c->cell_count, c->counters);
@@ -266,7 +273,7 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys, true);   // leaves cell_count cleared
     if (rc) return rc;
     if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
-                      with_acc ? 1 : 0, (!c->variable_h && with_acc) ? 1 : 0, c->key, c->rank, c->cell_start);
+                      with_acc ? 1 : 0, (!c->variable_h && with_acc) ? (c->pc.uniform_m ? 2 : 1) : 0, c->key, c->rank, c->cell_start);
     c->cur ^= 1;
     c->nl_valid = false;                 // recorded neighbour rows index the previous sorted order
     return SPH_OK;
@@ -385,7 +392,7 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
 // ------------------------------------------------------------------------------------------------
 int nnps_pack(sph_ctx* c, const PackArgs& A) {
     const int n = (int)c->n_total;
-    const int init[2] = { 0x7f7fffff, 0 };
+    const int init[4] = { 0x7f7fffff, 0, 0x7f7fffff, 0 };
     SPH_CUDA_OK(c, cudaMemcpyAsync(c->hminmax, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
     if (n) SPH_LAUNCH(c, SPH_K_PACK, k_pack, (n + NB - 1) / NB, NB, 0, A, c->S[c->cur], n, c->pc, (int*)c->hminmax);
     return SPH_OK;
