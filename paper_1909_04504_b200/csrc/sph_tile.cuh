@@ -281,7 +281,7 @@ struct TileRecorder {
         __syncwarp();
         uint32_t* hdr = nl.pool + (size_t)blk * 32;
         hdr[lane] = lane == 0 ? 0u : (lane == 1 ? ((uint32_t)M | (shifted ? 0x100u : 0u)) : ws.base[lane - 2]);
-        for (int m = 0; m < M; ++m) hdr[(size_t)(m + 1) * 32 + lane] = ws.mask[m][lane];
+        for (int m = 0; m < M; ++m) __stcs(hdr + (size_t)(m + 1) * 32 + lane, ws.mask[m][lane]);   // streaming: keep the state in L2
         if (lane == 0) { if (prev_hdr) nl.pool[(size_t)prev_hdr * 32] = blk; else nl.head[warp_id] = blk; }
         prev_hdr = blk;
     }
