@@ -3,13 +3,15 @@
 // with Monaghan artificial viscosity Pi_ij (R9; the paper only names "the classic scheme", L185)
 // and, in the same pair loop ("no inter-dependencies and may be computed together", L337), the continuity
 // right-hand side eq.7 (L126; Listing 4):   arho_i = sum_j m_j (v_i - v_j) . grad_i W_ij.
-// Gravity is the initial value of the accumulator (Listing 4).
+// Gravity is the initial value of the accumulator (Listing 4).  With sph_params.nu > 0 the laminar
+// viscosity of eq.10 (L134-136) is added in the same loop (LAMINAR instantiations).
 #include "sph_tile.cuh"
 
 // One kernel, two modes (sph_tile.cuh).  REPLAY = false: the warp tests its own candidates (continuity mode,
 // custom tables).  REPLAY = true: it replays the hit masks recorded by the density pass of the same evaluation
-// and tests nothing.  ARHO_ONLY launches serve ContinuityEquation(dest=solid, sources=[fluid]) (Listing 3
-// L372-374): the same loop, only arho is stored.
+// and tests nothing (a warp whose record did not fit the pool searches).  Destination arrays named in
+// arho_only_arrays serve ContinuityEquation(dest=solid, sources=[fluid]) (Listing 3): the same loop,
+// only arho is stored; they share the launch with the momentum destinations.
 // This file is compiled four times (build.py): once per smoothing kernel with -DSPH_ACCEL_KERNEL=<id> (the kernel
 // template and its launcher launch_accel_k<id>), and once without (the dispatcher launch_accel).
 int launch_accel_k0(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay);
