@@ -252,7 +252,11 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     int hmm[4] = { 0, 0, 0, 0 };
     SPH_CUDA_OK(c, cudaMemcpyAsync(hmm, c->hminmax, sizeof(hmm), cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
-    if (tot == 0) { c->h_min = c->h_max = 1.0f; }
+    if (tot == 0) {                            // no particles at all: any grid will do; size it so that a periodic box gets its >= 3 cells
+        double minL = 1.0e300;
+        for (int k = 0; k < c->dom.dim; ++k) minL = fmin(minL, c->dom.hi[k] - c->dom.lo[k]);
+        c->h_min = c->h_max = (float)(minL / (4.0 * kernel_support(c->prm.kernel)));
+    }
     else { memcpy(&c->h_min, &hmm[0], 4); memcpy(&c->h_max, &hmm[1], 4); }
     if (!(c->h_max > 0.0f) || !isfinite(c->h_max)) return sph_fail(c, SPH_ERR_BAD_ARG, "smoothing lengths must be positive and finite");
     c->variable_h = (c->h_min != c->h_max);
