@@ -101,7 +101,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         }
     };
     const uint32_t idle = in ? (uint32_t)i : 0u;
-    auto drain = [&](uint32_t nz, bool shifted) { per = shifted; tile_drain<AccelSrc>(ws, nz, idle, load, compute); };
+    auto drain = [&](uint32_t nz, bool shifted) { per = shifted; tile_drain<AccelSrc, (REPLAY ? TILE_DRAIN_DEPTH_REPLAY : 2)>(ws, nz, idle, load, compute); };
 
     TileState st; st.reset(); st.tests = 0; st.hits = 0;
     const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;

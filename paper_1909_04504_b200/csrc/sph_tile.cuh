@@ -29,6 +29,9 @@
 #ifndef TILE_MIN_BLOCKS_ACCEL
 #define TILE_MIN_BLOCKS_ACCEL 6           // the momentum kernel is 3-8 % faster with 80 registers and 6 blocks (measured, C3, C4)
 #endif
+#ifndef TILE_DRAIN_DEPTH_REPLAY
+#define TILE_DRAIN_DEPTH_REPLAY 3         // hits in flight in the replaying momentum kernel (-4 % on C3; the searching kernels lose with 3)
+#endif
 #ifndef TILE_MMAX
 #define TILE_MMAX 30                       // masks per warp before a forced drain (<= 30: 30 bases + 2 words = one header row)
 #endif
@@ -233,7 +236,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
 // state does not fit L1) overlaps the arithmetic.  A lane that has run out keeps executing with has = false and
 // the harmless index `idle` (its own particle) until the slowest lane of the warp is done; compute(src, has)
 // must contribute nothing when has is false.
-template <class Src, class Load, class Compute>
+template <class Src, int DEPTH = 2, class Load, class Compute>
 __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
     const int lane = threadIdx.x & 31;
     __syncwarp();
@@ -248,14 +251,29 @@ __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32
         cur &= cur - 1u;                        // stays 0 when it is 0
         return j;
     };
-    Src A, B; bool hasA, hasB;
-    A = load(pop(hasA));
-    for (;;) {
-        B = load(pop(hasB));
-        compute(A, hasA);
+    if (DEPTH == 3) {                               // three hits in flight (the momentum loop has the registers for it)
+        Src A, B, C; bool hasA, hasB, hasC;
         A = load(pop(hasA));
-        compute(B, hasB);
-        if (!__any_sync(SPH_FULL_MASK, hasA)) break;
+        B = load(pop(hasB));
+        for (;;) {
+            C = load(pop(hasC));
+            compute(A, hasA);
+            A = load(pop(hasA));
+            compute(B, hasB);
+            B = load(pop(hasB));
+            compute(C, hasC);
+            if (!__any_sync(SPH_FULL_MASK, hasA)) break;      // has is monotone: no A means no B either
+        }
+    } else {
+        Src A, B; bool hasA, hasB;
+        A = load(pop(hasA));
+        for (;;) {
+            B = load(pop(hasB));
+            compute(A, hasA);
+            A = load(pop(hasA));
+            compute(B, hasB);
+            if (!__any_sync(SPH_FULL_MASK, hasA)) break;
+        }
     }
     __syncwarp();
 }
