@@ -65,7 +65,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     auto drain = [&]() {
         if (RECORD) rec.append(ws, st.M, st.shifted, warp_id, counters);
         per = st.shifted;
-        tile_drain<DensitySrc>(ws, st.nz, idle, load, compute);
+        tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY>(ws, st.nz, idle, load, compute);
         st.reset();
     };
     tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st, drain);

@@ -32,6 +32,9 @@
 #ifndef TILE_DRAIN_DEPTH_REPLAY
 #define TILE_DRAIN_DEPTH_REPLAY 3         // hits in flight in the replaying momentum kernel (-4 % on C3; the searching kernels lose with 3)
 #endif
+#ifndef TILE_DRAIN_DEPTH_DENSITY
+#define TILE_DRAIN_DEPTH_DENSITY 3         // hits in flight in the density drain (3: -2 % on C3; 4 is no better)
+#endif
 #ifndef TILE_MMAX
 #define TILE_MMAX 30                       // masks per warp before a forced drain (<= 30: 30 bases + 2 words = one header row)
 #endif
@@ -231,7 +234,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
 }
 
 // Every lane pops its own hits of the stored batches in order (nz: the lane's non-empty masks) and evaluates
-// them.  Branch-free and software-pipelined: two hits are in flight, the source data of the next hit is
+// them.  Branch-free and software-pipelined: DEPTH hits are in flight, the source data of a later hit is
 // gathered (Src = load(sorted index)) before the current one is computed, so the gather latency (L2: the sorted
 // state does not fit L1) overlaps the arithmetic.  A lane that has run out keeps executing with has = false and
 // the harmless index `idle` (its own particle) until the slowest lane of the warp is done; compute(src, has)
@@ -251,29 +254,17 @@ __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32
         cur &= cur - 1u;                        // stays 0 when it is 0
         return j;
     };
-    if (DEPTH == 3) {                               // three hits in flight (the momentum loop has the registers for it)
-        Src A, B, C; bool hasA, hasB, hasC;
-        A = load(pop(hasA));
-        B = load(pop(hasB));
-        for (;;) {
-            C = load(pop(hasC));
-            compute(A, hasA);
-            A = load(pop(hasA));
-            compute(B, hasB);
-            B = load(pop(hasB));
-            compute(C, hasC);
-            if (!__any_sync(SPH_FULL_MASK, hasA)) break;      // has is monotone: no A means no B either
+    Src R[DEPTH]; bool H[DEPTH];                    // DEPTH hits in flight; fully unrolled, so R and H live in registers
+#pragma unroll
+    for (int d = 0; d + 1 < DEPTH; ++d) R[d] = load(pop(H[d]));
+    for (;;) {
+#pragma unroll
+        for (int d = 0; d < DEPTH; ++d) {
+            const int nx = (d + DEPTH - 1) % DEPTH;
+            R[nx] = load(pop(H[nx]));               // gather for a later hit ...
+            compute(R[d], H[d]);                    // ... while this one is evaluated
         }
-    } else {
-        Src A, B; bool hasA, hasB;
-        A = load(pop(hasA));
-        for (;;) {
-            B = load(pop(hasB));
-            compute(A, hasA);
-            A = load(pop(hasA));
-            compute(B, hasB);
-            if (!__any_sync(SPH_FULL_MASK, hasA)) break;
-        }
+        if (!__any_sync(SPH_FULL_MASK, H[0])) break;   // pops are in order: no pending hit 0 means no pending hit at all
     }
     __syncwarp();
 }
