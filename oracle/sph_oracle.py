@@ -1,13 +1,16 @@
 """ORACLE -- TEST INFRASTRUCTURE, NOT THE PRODUCT.  (see the header of sph_oracle.cpp)
 
 ctypes wrapper over oracle/sph_oracle.cpp plus the parts of the path that are per-particle numpy
-one-liners: the group ordering of PAPER.md Listing 3 (L363-378) and the predictor-corrector
-integrator, eqs. 12-14 (L148-152).  Everything is float64.  This module imports nothing from the
+one-liners: the group ordering of PAPER.md Listing 3 (L363-378), the predictor-corrector
+integrator, eqs. 12-14 (L148-152), and the forward-Euler integrator of the paper's worked example
+(L335, Fig.2; R22).  Everything is float64.  Pins: tests/test_oracle_*.py.  PARITY UNPINNED
+(DESIGN.md section 2): the choice of the artificial-viscosity form and its constants, the h_ij
+convention, how rho is stepped, the order inside the Euler step, the physical fidelity of the dam breaks.  This module imports nothing from the
 product package and the product imports nothing from here.
 
 Duck-typed inputs: a "workload" is any object with attributes
   dim, lo, hi, periodic, kernel ('cubic'|'quintic'|'wendland_c2'), rho0, c0, gamma, alpha, eps, g,
-  arrays (each with x,y,z,u,v,w,h,m,rho and .fixed), density_sources, accel_sources, arho_sources.
+  [nu, eta: laminar viscosity eq.10], arrays (each with x,y,z,u,v,w,h,m,rho and .fixed), density_sources, accel_sources, arho_sources.
 """
 from __future__ import annotations
 
