@@ -167,7 +167,7 @@ static int size_grid(sph_ctx* c) {
     if (!(cutoff > 0.0)) return sph_fail(c, SPH_ERR_BAD_ARG, "h_max must be positive");
     double scale = 1.0;
     int xsub = c->xsub;
-    if (c->xsub_auto && c->variable_h) xsub = 8;       // variable h: finer x windows pay (reach < cell for small-h groups)
+    if (c->xsub_auto && c->variable_h) xsub = 16;      // variable h: finer x windows pay (reach < cell for small-h groups)
     for (int iter = 0; iter < 64; ++iter) {
         int64_t total = 1; bool ok = true;
         for (int k = 0; k < 3; ++k) {
