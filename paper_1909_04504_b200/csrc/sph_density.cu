@@ -73,6 +73,9 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     if (active) {
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
         S.rp[i] = make_float2(rho, p / (rho * rho));
+        // The .w stores below touch words that NO thread of this launch reads (constant h: the tests and the drain
+        // use x,y,z of posh and, without UM, its .w = m, which is not written), so concurrent 16-byte gathers of the
+        // same record by other warps see unchanged x,y,z whichever version of .w they get.
         if (!VARH) S.velm[i].w = rho;                                   // constant h: velm.w carries rho (SortedState)
         if (UM) S.posh[i].w = p / (rho * rho);                          // UM layout: posh.w carries p/rho^2
         if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
