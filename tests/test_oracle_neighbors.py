@@ -158,3 +158,17 @@ def test_block_generator_matches_paper_listing(WL):
     assert x.min() == pytest.approx(-1.9) and x.max() == pytest.approx(-0.9)
     wl = WL.dam_break_2d()
     assert [a.n for a in wl.arrays] == [20000, 3618]
+
+
+def test_neighbour_relation_is_symmetric(O, WL):
+    """The predicate r_ij < k (h_i + h_j)/2 is symmetric in i and j (R3): j in N(i) <=> i in N(j), also
+    with variable h and across the periodic seam."""
+    for dim in (2, 3):
+        wl = WL.random_box(n=900, dim=dim, periodic=True, seed=41 + dim, variable_h=True)
+        A = wl.arrays[0]
+        f = {c: getattr(A, c) for c in "xyzh"}
+        for pred32 in (True, False):
+            off, idx = O.neighbors(wl, f, f, pred32=pred32, method="cell")
+            pairs = {(i, int(j)) for i in range(A.n) for j in idx[off[i]:off[i + 1]]}
+            assert all((j, i) in pairs for (i, j) in pairs)
+            assert all((i, i) in pairs for i in range(A.n))          # self pair included (R5)

@@ -103,3 +103,35 @@ def test_no_move_option(O, WL):
     st = O.State(wl); x0 = st.arrays[0]["x"].copy(); u0 = st.arrays[0]["u"].copy()
     O.pc_step(wl, st, wl.dt, "summation", move=False)
     assert np.array_equal(st.arrays[0]["x"], x0) and not np.array_equal(st.arrays[0]["u"], u0)
+
+
+def test_taylor_green_run_follows_the_analytic_decay_trend(O, WL):
+    """north_star pin: the 2-D Taylor-Green state decays like exp(b t), b = -8 pi^2 nu.  With
+    Monaghan's viscosity the continuum-limit nu of the scheme is alpha h c0 / 8 (all pairs; R9), so the
+    kinetic energy of a run of the C1 state must fall like exp(2 b t) with b near -8 pi^2 alpha h c0 / 8 = -0.20/s.
+    The first 0.1 s is an acoustic transient (rho starts uniform: O(Mach^2) = 1e-2 sloshing), so the rate is
+    fitted over t in [0.1, 0.6]: 1,200 steps of the oracle (4 s)."""
+    wl = WL.taylor_green_2d()
+    st = O.State(wl)
+    m = st.arrays[0]["m"]
+    n = 1200
+    ke = np.zeros(n + 1)
+    for s in range(n + 1):
+        A = st.arrays[0]
+        ke[s] = 0.5 * float((m * (A["u"] ** 2 + A["v"] ** 2)).sum())
+        if s < n:
+            O.pc_step(wl, st, wl.dt, "summation")
+    t = np.arange(n + 1) * wl.dt
+    sel = t >= 0.1
+    b = np.polyfit(t[sel], np.log(ke[sel] / ke[0]), 1)[0] / 2.0
+    h = float(wl.arrays[0].h[0])
+    b_ref = -8.0 * np.pi ** 2 * wl.alpha * h * wl.c0 / 8.0
+    assert 0.6 * abs(b_ref) <= -b <= 1.5 * abs(b_ref), (b, b_ref)
+    assert ke[-1] < 0.85 * ke[0] and np.all(ke[sel] < 1.001 * ke[np.argmax(sel)])      # it decays, monotonically on the fit window
+    # the flow stays a Taylor-Green vortex: the velocities still point along the analytic field (L649-652) at the
+    # particles' current positions
+    A = st.arrays[0]
+    ua = -np.cos(2 * np.pi * A["x"]) * np.sin(2 * np.pi * A["y"])
+    va = np.sin(2 * np.pi * A["x"]) * np.cos(2 * np.pi * A["y"])
+    corr = float((A["u"] * ua + A["v"] * va).sum() / np.sqrt((A["u"] ** 2 + A["v"] ** 2).sum() * (ua ** 2 + va ** 2).sum()))
+    assert corr > 0.95
