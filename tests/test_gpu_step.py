@@ -157,3 +157,38 @@ def test_dense_cells_span_several_record_blocks(O, WL):
     assert s0.pairs_density == s0.pairs_accel == s1.pairs_density == s1.pairs_accel
     for k in ("x", "u", "v", "w", "rho"):
         assert np.abs(o1[k].astype(np.float64) - o0[k]).max() <= 2e-6 * np.abs(o0[k]).max(), k
+
+
+def test_taylor_green_run_decays_like_the_oracle(O, WL):
+    """Multi-step behaviour (trajectories are not gated element-wise, R15): 1,200 steps of C1 on the GPU
+    lose kinetic energy at the same fitted rate as the fp64 oracle's run, which is pinned to the analytic
+    Taylor-Green decay (test_oracle_step.py)."""
+    wl = WL.taylor_green_2d()
+    m = wl.arrays[0].m.astype(np.float64)
+    n, every = 1200, 50
+
+    def fit(ke):
+        t = np.arange(len(ke)) * every * wl.dt
+        sel = t >= 0.1
+        return np.polyfit(t[sel], np.log(ke[sel] / ke[0]), 1)[0] / 2.0
+
+    ctx, _ = make_ctx(wl)
+    ke_g = []
+    for s in range(n // every + 1):
+        out = ctx.sync_state(0, fields=("u", "v"))
+        ke_g.append(0.5 * float((m * (out["u"].cpu().numpy().astype(np.float64) ** 2 + out["v"].cpu().numpy().astype(np.float64) ** 2)).sum()))
+        if s < n // every:
+            ctx.pc_step(wl.dt, every, "summation")
+    ctx.synchronize()
+    ctx.close()
+    st = O.State(wl)
+    ke_o = []
+    for s in range(n + 1):
+        if s % every == 0:
+            A = st.arrays[0]
+            ke_o.append(0.5 * float((m * (A["u"] ** 2 + A["v"] ** 2)).sum()))
+        if s < n:
+            O.pc_step(wl, st, wl.dt, "summation")
+    bg, bo = fit(np.array(ke_g)), fit(np.array(ke_o))
+    assert abs(bg - bo) <= 0.05 * abs(bo), (bg, bo)
+    assert abs(ke_g[-1] / ke_g[0] - ke_o[-1] / ke_o[0]) < 5e-3
