@@ -91,7 +91,7 @@ typedef struct sph_params {
                                  * nu = 0 (default): term off.  eta: the paper's regulariser (0.01 is customary) */
     int integrator;             /* enum sph_integrator: what sph_pc_step steps with */
     /* Tuning knobs of the neighbour search; results do not depend on them (0 = default). */
-    int xsub;                   /* x sub-cells per support radius (1..16; default 0 = 4, or 16 when h varies)      */
+    int xsub;                   /* x sub-cells per support radius (1..16; default 0 = 6, or 16 when h varies)      */
     int nlist_slots;            /* record pool of the pair passes, in rows of 32 words per warp (32 particles) of
                                  * capacity (default 192, i.e. 768 B per particle of capacity; < 0: no pool, every
                                  * pair pass searches).  The summation-density pass records one 32-bit hit mask

@@ -86,7 +86,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     c->cap_total = tot;
     default_tables(c);
     set_consts(c);
-    c->xsub = params->xsub ? params->xsub : 4;
+    c->xsub = params->xsub ? params->xsub : 6;
     c->xsub_auto = params->xsub == 0;
     if (const char* e = getenv("SPH_XSUB")) { int v = atoi(e); if (v >= 1 && v <= 16) { c->xsub = v; c->xsub_auto = false; } }   // tuning override
     int nl_slots = params->nlist_slots ? params->nlist_slots : 192;

@@ -44,7 +44,7 @@ struct sph_ctx {
     bool nl_valid;             // rows match the current sort and the masks below
     uint32_t nl_mask[SPH_MAX_ARRAYS];   // per dest array: the source mask the rows were recorded with (0 = none)
     bool last_used_rows;       // the last acceleration launch replayed recorded rows
-    bool xsub_auto;            // xsub was not given: 4, or 16 when h varies
+    bool xsub_auto;            // xsub was not given: 6, or 16 when h varies
     int xsub;                  // x sub-cells per support radius requested (GridDesc::xsub is what the grid got)
 
     int64_t launches, steps_done;
