@@ -5,8 +5,11 @@ one-liners: the group ordering of PAPER.md Listing 3 (L363-378), the predictor-c
 integrator, eqs. 12-14 (L148-152), and the forward-Euler integrator of the paper's worked example
 (L335, Fig.2; R22).  Everything is float64.  Pins: tests/test_oracle_*.py.  PARITY UNPINNED
 (DESIGN.md section 2): the choice of the artificial-viscosity form and its constants, the h_ij
-convention, how rho is stepped, the order inside the Euler step, the physical fidelity of the dam breaks.  This module imports nothing from the
-product package and the product imports nothing from here.
+convention, the READING that rho is stepped like u (R11) and the order inside the Euler step (R22) -- the paper
+prints no value to hold those choices to -- and the physical fidelity of the dam breaks.  The IMPLEMENTATION of
+the chosen readings is pinned: both integrators have a step written out bit-equal by hand in the tests (PC:
+test_single_step_is_eqs_12_to_14, test_continuity_mode_step_written_out; Euler: test_oracle_laminar.py).
+This module imports nothing from the product package and the product imports nothing from here.
 
 Duck-typed inputs: a "workload" is any object with attributes
   dim, lo, hi, periodic, kernel ('cubic'|'quintic'|'wendland_c2'), rho0, c0, gamma, alpha, eps, g,

@@ -98,6 +98,67 @@ def test_fixed_arrays_and_continuity_mode(O, WL):
     assert np.abs(F["rho"] / wl.rho0 - 1).max() < 0.02        # weakly compressible
 
 
+def test_continuity_mode_step_written_out(O, WL):
+    """Continuity-mode predictor-corrector step written out by hand around the oracle's own F (eqs. 12-14
+    L148-152 for u, x; L142 "the continuity equation is solved on the tank particles too"; R11: rho is
+    stepped like u):   rho^{n+1/2} = rho^n + dt/2 arho^n ;  F evaluated at (x^{n+1}, u^{n+1/2}, rho^{n+1/2}) ;
+    rho^{n+1} = rho^{n+1/2} + dt/2 arho^{n+1}, on BOTH arrays, bit-equal.  A full-dt kick, a dropped kick or a
+    kick with the wrong arho fails this."""
+    wl = WL.dam_break_2d(dx=0.05)
+    rng = np.random.default_rng(11)
+    wl.arrays[0].u[:] = rng.uniform(-0.3, 0.3, wl.arrays[0].n).astype(np.float32)
+    wl.arrays[0].v[:] = rng.uniform(-0.3, 0.3, wl.arrays[0].n).astype(np.float32)
+    dt = wl.dt
+    st = O.State(wl)
+    O.evaluate(wl, st, "continuity")                       # a^n, arho^n
+    s0 = st.copy()
+    O.pc_step(wl, st, dt, "continuity")
+    # the half-step state, by hand
+    mid = s0.copy()
+    F0, S0 = s0.arrays
+    Fm, Sm = mid.arrays
+    Fm["u"] = F0["u"] + 0.5 * dt * F0["au"]; Fm["v"] = F0["v"] + 0.5 * dt * F0["av"]          # (12)
+    Fm["x"] = F0["x"] + dt * Fm["u"]; Fm["y"] = F0["y"] + dt * Fm["v"]                         # (13)
+    Fm["rho"] = F0["rho"] + 0.5 * dt * F0["arho"]
+    Sm["rho"] = S0["rho"] + 0.5 * dt * S0["arho"]
+    O.evaluate(wl, mid, "continuity")                      # a^{n+1}, arho^{n+1} from (x^{n+1}, u^{n+1/2}, rho^{n+1/2})
+    F1, S1 = st.arrays
+    assert np.array_equal(F1["x"], Fm["x"]) and np.array_equal(F1["y"], Fm["y"])
+    assert np.array_equal(F1["u"], Fm["u"] + 0.5 * dt * Fm["au"])                              # (14)
+    assert np.array_equal(F1["v"], Fm["v"] + 0.5 * dt * Fm["av"])
+    assert np.array_equal(F1["rho"], Fm["rho"] + 0.5 * dt * Fm["arho"])
+    assert np.array_equal(S1["rho"], Sm["rho"] + 0.5 * dt * Sm["arho"])
+    assert np.array_equal(S1["x"], S0["x"]) and np.array_equal(S1["u"], S0["u"])               # fixed array (L142)
+    # the kicks are not degenerate: both halves move rho, and differently (so a doubled first kick is told apart)
+    k1 = 0.5 * dt * F0["arho"]; k2 = 0.5 * dt * Fm["arho"]
+    assert np.abs(k1).max() > 1e-9 * wl.rho0 and np.abs(k2 - k1).max() > 1e-3 * np.abs(k1).max()
+    assert np.abs(0.5 * dt * S0["arho"]).max() > 1e-9 * wl.rho0
+    # p of the result is the EOS of the rho the evaluation saw (group order L364-378): rho^{n+1/2}
+    assert np.array_equal(F1["p"], O.eos(wl, Fm["rho"])) and np.array_equal(S1["p"], O.eos(wl, Sm["rho"]))
+
+
+def test_continuity_mode_rho_follows_the_closed_form_of_a_uniform_compression(O, WL):
+    """A pin with a value the mathematics fixes: particles on a periodic lattice with the velocity field u = -c (x - 1/2)
+    frozen in time (fixed array: x,u never change) have a constant arho = rho div-free term  sum_j m_j u_ij . grad W
+    ~ +c rho0 (eq.7, tr A = -c), so n continuity steps give rho_n = rho_0 + n dt arho exactly (two half kicks
+    per step = one full kick), and arho is within the kernel-sum error of c rho0 d."""
+    wl = WL.lattice((16, 16), 2, 1.3, "cubic")
+    A = wl.arrays[0]
+    c = 0.7
+    A.u[:] = (-c * (A.x - 0.5)).astype(np.float32); A.v[:] = (-c * (A.y - 0.5)).astype(np.float32)
+    A.fixed = True
+    wl.arho_sources = [[0]]
+    st = O.State(wl)
+    O.evaluate(wl, st, "continuity")
+    arho0 = st.arrays[0]["arho"].copy(); rho0 = st.arrays[0]["rho"].copy()
+    n = 4
+    for _ in range(n):
+        O.pc_step(wl, st, wl.dt, "continuity")
+    assert np.allclose(st.arrays[0]["rho"], rho0 + n * wl.dt * arho0, rtol=0, atol=1e-12 * wl.rho0)
+    inner = (np.abs(A.x - 0.5) < 0.2) & (np.abs(A.y - 0.5) < 0.2)
+    assert np.allclose(arho0[inner], 2 * c * wl.rho0, rtol=2e-2)     # measured 1.06 % at h = 1.3 dx
+
+
 def test_no_move_option(O, WL):
     wl = WL.random_box(n=300, dim=3, periodic=True, seed=43, variable_h=True)
     st = O.State(wl); x0 = st.arrays[0]["x"].copy(); u0 = st.arrays[0]["u"].copy()
