@@ -39,7 +39,7 @@ extern "C" {
 #endif
 
 #define SPH_MAX_ARRAYS 4
-#define SPH_ABI_VERSION 4
+#define SPH_ABI_VERSION 5
 
 typedef struct sph_ctx sph_ctx;
 
@@ -91,7 +91,10 @@ typedef struct sph_params {
                                  * nu = 0 (default): term off.  eta: the paper's regulariser (0.01 is customary) */
     int integrator;             /* enum sph_integrator: what sph_pc_step steps with */
     /* Tuning knobs of the neighbour search; results do not depend on them (0 = default). */
-    int xsub;                   /* x sub-cells per support radius (1..16; default 0 = 6, or 16 when h varies)      */
+    int xsub;                   /* x sub-cells per support radius (1..16; default 0 = 6, or 4 when h varies)       */
+    int levels;                 /* variable h: number of h classes, each with its own cell grid (PAPER.md L158-160,
+                                 * L171: one grid sized by h_max "becomes inefficient"); 0 = as many as keep the h ratio
+                                 * of a class <= ~1.6 (at most 8); 1 = the paper's single grid sized by h_max      */
     int nlist_slots;            /* record pool of the pair passes, in rows of 32 words per warp (32 particles) of
                                  * capacity (default 192, i.e. 768 B per particle of capacity; < 0: no pool, every
                                  * pair pass searches).  The summation-density pass records one 32-bit hit mask
@@ -118,12 +121,12 @@ typedef struct sph_array {      /* one named particle array (L316) */
 } sph_array;
 
 typedef struct sph_stats {
-    int32_t n_cells[3];         /* grid dimensions */
+    int32_t n_cells[3];         /* grid dimensions of the coarsest level (cells >= k h_max; n_cells[0] counts x sub-cells) */
     double cell_size[3];
     int64_t n_particles;        /* all arrays */
-    int64_t pairs_density;      /* (i,j) pairs passing the predicate in the last density pass(es), self pairs included */
+    int64_t pairs_density;      /* (i,j) pairs passing the exact predicate in the last density pass(es), self pairs included */
     int64_t pairs_accel;        /* same for the last acceleration pass(es) */
-    int64_t candidates;         /* predicate evaluations of the last density + acceleration passes */
+    int64_t candidates;         /* candidates streamed through the filter in the last density + acceleration passes */
     int64_t candidates_density, candidates_accel;
     int64_t kernel_launches;    /* CUDA kernels launched by this context since sph_create */
     int64_t steps_done;         /* predictor-corrector steps since the last sph_nnps_build */
@@ -133,6 +136,8 @@ typedef struct sph_stats {
     int32_t used_rows;          /* 1 if the last acceleration pass replayed the hit masks recorded by the density pass */
     int64_t nlist_rows_used, nlist_rows_capacity;   /* record pool occupancy after the last recording pass */
     int64_t nlist_fallback_warps;                   /* warps whose masks did not fit the pool in that pass (they search again) */
+    int32_t n_levels;           /* h classes / level grids of the current build (1 when h is constant) */
+    int64_t n_keys;             /* entries of the shared cell table (all levels x arrays) */
 } sph_stats;
 
 /* Per-kernel device timing (CUDA events on the context stream around every launch), for the roofline report. */

@@ -41,7 +41,7 @@ class sph_params(C.Structure):
     _fields_ = [("kernel", C.c_int), ("rho0", C.c_double), ("c0", C.c_double), ("gamma", C.c_double),
                 ("alpha", C.c_double), ("eps", C.c_double), ("g", C.c_double * 3), ("move", C.c_int),
                 ("nu", C.c_double), ("eta", C.c_double), ("integrator", C.c_int),
-                ("xsub", C.c_int), ("nlist_slots", C.c_int)]
+                ("xsub", C.c_int), ("levels", C.c_int), ("nlist_slots", C.c_int)]
 
 
 class sph_array(C.Structure):
@@ -56,7 +56,7 @@ class sph_stats(C.Structure):
                 ("kernel_launches", C.c_int64), ("steps_done", C.c_int64), ("variable_h", C.c_int32),
                 ("h_max", C.c_float), ("xsub", C.c_int32), ("used_rows", C.c_int32),
                 ("nlist_rows_used", C.c_int64), ("nlist_rows_capacity", C.c_int64),
-                ("nlist_fallback_warps", C.c_int64)]
+                ("nlist_fallback_warps", C.c_int64), ("n_levels", C.c_int32), ("n_keys", C.c_int64)]
 
 
 class sph_profile(C.Structure):
@@ -142,7 +142,7 @@ class SphContext:
 
     def __init__(self, *, dim: int, lo, hi, periodic, kernel: str, rho0: float, c0: float, gamma: float = 7.0,
                  alpha: float = 0.1, eps: float = 0.01, g=(0.0, 0.0, 0.0), move: bool = True,
-                 capacity: Sequence[int], stream=None, xsub: int = 0, nlist_slots: int = 0,
+                 capacity: Sequence[int], stream=None, xsub: int = 0, nlist_slots: int = 0, levels: int = 0,
                  nu: float = 0.0, eta: float = 0.01, integrator: str = "pc"):
         import torch
         if not torch.cuda.is_available():
@@ -153,7 +153,7 @@ class SphContext:
         dom = sph_domain(); dom.dim = int(dim)
         prm = sph_params(); prm.kernel = KERNEL_ID[kernel]
         prm.rho0, prm.c0, prm.gamma, prm.alpha, prm.eps, prm.move = rho0, c0, gamma, alpha, eps, int(move)
-        prm.xsub, prm.nlist_slots = int(xsub), int(nlist_slots)
+        prm.xsub, prm.nlist_slots, prm.levels = int(xsub), int(nlist_slots), int(levels)
         prm.nu, prm.eta, prm.integrator = float(nu), float(eta), INTEGRATOR_ID[integrator]
         for k in range(3):
             dom.lo[k], dom.hi[k], dom.periodic[k] = float(lo[k]), float(hi[k]), int(bool(periodic[k]))

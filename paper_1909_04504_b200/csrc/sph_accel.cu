@@ -14,9 +14,9 @@
 // only arho is stored; they share the launch with the momentum destinations.
 // This file is compiled four times (build.py): once per smoothing kernel with -DSPH_ACCEL_KERNEL=<id> (the kernel
 // template and its launcher launch_accel_k<id>), and once without (the dispatcher launch_accel).
-int launch_accel_k0(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay);
-int launch_accel_k1(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay);
-int launch_accel_k2(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay);
+int launch_accel_k0(sph_ctx* c, int dim, bool filter, bool want_arho, const AccelRoles& roles, bool replay);
+int launch_accel_k1(sph_ctx* c, int dim, bool filter, bool want_arho, const AccelRoles& roles, bool replay);
+int launch_accel_k2(sph_ctx* c, int dim, bool filter, bool want_arho, const AccelRoles& roles, bool replay);
 
 #ifdef SPH_ACCEL_KERNEL
 struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
@@ -24,7 +24,7 @@ struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
 template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, int PM, bool LAMINAR>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS_ACCEL)
 k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
-             uint32_t arho_only_arrays, NList nl, unsigned long long* __restrict__ counters) {
+             AccelRoles roles, NList nl, unsigned long long* __restrict__ counters) {
     __shared__ TileWarpSmem smem[TILE_WARPS];
     TileWarpSmem& ws = smem[threadIdx.x >> 5];
     const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
@@ -32,42 +32,53 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const bool in = i < n;
     uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1), vi = make_float4(0, 0, 0, 0);
     float2 ri = make_float2(1, 0);
-    if (in) { meta = S.meta[i]; pi = S.posh[i]; vi = S.velm[i]; ri = S.rp[i]; ci = S.cell[i]; }
-    const uint32_t my_mask = in ? pc.src_mask[meta >> SPH_META_IDX_BITS] : 0u;
+    if (in) { meta = S.meta[i]; pi = __ldg(S.posh + i); vi = __ldg(S.velm + i); ri = __ldg(S.rp + i); ci = S.cell[i]; }
+    const uint32_t aid_i = meta >> SPH_META_IDX_BITS;
+    const uint32_t my_mask = in ? pc.src_mask[aid_i] : 0u;
     const bool active = my_mask != 0u;
+    // arrays that are no destination of any launch of this evaluation: their accelerations are zero (the sort does
+    // not carry acc along, so what lies in their rows belongs to other particles)
+    if (in && !active && (((roles.zero_xyz | roles.zero_w) >> aid_i) & 1u)) {
+        float4 a = S.acc[i];
+        if ((roles.zero_xyz >> aid_i) & 1u) { a.x = 0.0f; a.y = 0.0f; a.z = 0.0f; }
+        if ((roles.zero_w >> aid_i) & 1u) a.w = 0.0f;
+        S.acc[i] = a;
+    }
     if (!__any_sync(SPH_FULL_MASK, active)) return;
 
     const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
-    const float iLx = 1.0f / g.L[0], iLy = 1.0f / g.L[1], iLz = 1.0f / g.L[2];
-    const float sigma = pc.sigma, h_c = pc.h_const, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
+    const float sigma = pc.sigma, h_c = pc.h_const, hinv_c = pc.hinv_const, fac_c = pc.fac_const, kh = pc.kh;
     const float visc = pc.visc, eps = pc.eps, nu4 = pc.nu4, eta = pc.eta;
     const float hi = VARH ? pi.w : h_c;
+    const float cut2c = pair_cut2(kh, h_c, h_c);
     // PM: where the neighbour's rho and p/rho^2 come from (the loop is L1-gather bound: fewer gathers pay).
-    //   0  gathered from rp (variable h; or caller-supplied p, gamma != 7 with non-uniform mass): three gathers
-    //   1  constant h, gamma = 7, every p is the EOS of its rho: rho rides in velm.w, p/rho^2 is recomputed (the
-    //      destination's own term too, so that the pair terms stay antisymmetric): two gathers
+    //   0  gathered from rp (caller-supplied p, gamma != 7 ...): three gathers
+    //   1  gamma = 7, every p is the EOS of its rho, and velm.w carries rho (constant h, or variable h with uniform
+    //      mass): p/rho^2 is recomputed (the destination's own term too, so that the pair terms stay antisymmetric):
+    //      two gathers
     //   2  UM layout (constant h, uniform mass): rho in velm.w, p/rho^2 in posh.w, m = m_const: two gathers
     const float inv_rho0 = 1.0f / pc.rho0, rho0 = pc.rho0, Beos = pc.B;
     const float rho_i = ri.x, pr_i = PM == 1 ? eos7_p_over_rho2(ri.x, rho0, inv_rho0, Beos) : ri.y;
     const float m_const = pc.m_const;
     float ax = pc.g[0], ay = pc.g[1], az = pc.g[2], ar = 0.0f;      // gravity = accumulator init (Listing 4)
-    unsigned long long fhits = 0, rhits = 0;                            // FILTER: hits passing the source mask; replayed hits
+    unsigned nhits = 0;                                                 // pairs that pass the exact predicate (and the source mask)
     auto load = [&](uint32_t j) {
         AccelSrc s; s.pj = __ldg(S.posh + j); s.vj = __ldg(S.velm + j); s.aid = 0u;
         s.rj = PM ? make_float2(0.0f, 0.0f) : __ldg(S.rp + j);
         if (FILTER) { if (my_mask != pc.all_mask) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS; }   // lanes fed by all arrays skip the gather
         return s;
     };
-    bool per = false;                                                   // warp-uniform: some stored batch is a periodic image
-    auto compute = [&](const AccelSrc& s, bool has) {
-        if (FILTER) { has = has && (my_mask == pc.all_mask || ((my_mask >> s.aid) & 1u)); fhits += has ? 1u : 0u; }
-        float dx = pi.x - s.pj.x, dy = pi.y - s.pj.y, dz = DIM == 3 ? pi.z - s.pj.z : 0.0f;
-        if (per) {
-            dx = min_image(dx, Lx, iLx); dy = min_image(dy, Ly, iLy);
-            if (DIM == 3) dz = min_image(dz, Lz, iLz);
+    auto compute = [&](const AccelSrc& s, bool has, uint32_t code, auto per) {
+        // the exact predicate of DESIGN.md R7 on the candidate the tensor-core filter let through
+        float dx = __fsub_rn(pi.x, s.pj.x), dy = __fsub_rn(pi.y, s.pj.y), dz = DIM == 3 ? __fsub_rn(pi.z, s.pj.z) : 0.0f;
+        if (decltype(per)::value) {
+            dx = __fsub_rn(dx, img_shift(code, 0, Lx)); dy = __fsub_rn(dy, img_shift(code, 1, Ly));
+            if (DIM == 3) dz = __fsub_rn(dz, img_shift(code, 2, Lz));
         }
-        float r2 = fmaf(dy, dy, dx * dx);
-        if (DIM == 3) r2 = fmaf(dz, dz, r2);
+        const float r2 = pair_r2(dx, dy, dz);
+        has = has && r2 < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);
+        if (FILTER) has = has && (my_mask == pc.all_mask || ((my_mask >> s.aid) & 1u));
+        nhits += has ? 1u : 0u;
         const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;       // grad W := 0 at r = 0 (R18): rinv = 0
         const float r = r2 * rinv;
         float hij, hinv, fac;
@@ -82,7 +93,8 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         const float vx = vi.x - s.vj.x, vy = vi.y - s.vj.y;
         float vr = fmaf(vy, dy, vx * dx);
         if (DIM == 3) vr = fmaf(vi.z - s.vj.z, dz, vr);
-        const float mj = VARH ? s.vj.w : (PM == 2 ? m_const : s.pj.w);  // SortedState layouts
+        // SortedState layouts: where m, rho and p/rho^2 of the neighbour ride
+        const float mj = PM == 2 ? m_const : (VARH ? (PM == 1 ? m_const : s.vj.w) : s.pj.w);
         const float rho_j = PM ? s.vj.w : s.rj.x;
         const float pr_j = PM == 2 ? s.pj.w : (PM == 1 ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y);
         // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
@@ -101,45 +113,50 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         }
     };
     const uint32_t idle = in ? (uint32_t)i : 0u;
-    auto drain = [&](uint32_t nz, bool shifted) { per = shifted; tile_drain<AccelSrc, (REPLAY ? TILE_DRAIN_DEPTH_REPLAY : 2)>(ws, nz, idle, load, compute); };
+    constexpr int DEPTH = REPLAY ? TILE_DRAIN_DEPTH_REPLAY : 2;
+    auto drain = [&](uint32_t nz, bool shifted) {
+        if (shifted) tile_drain<AccelSrc, DEPTH, true>(ws, nz, idle, load, compute);
+        else         tile_drain<AccelSrc, DEPTH, false>(ws, nz, idle, load, compute);
+    };
 
-    TileState st; st.reset(); st.tests = 0; st.hits = 0;
+    TileState st; st.reset(); st.tests = 0;
     const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
     if (head != SPH_NL_NONE) {
-        tile_replay(nl, head, ws, active, rhits, drain);
+        tile_replay(nl, head, ws, active, drain);
     } else {                                    // no record (or one that did not fit the pool): search
-        const int row = in ? (int)(ci / (uint32_t)g.nc[0]) : -1;
-        const int sub = in ? (int)(ci % (uint32_t)g.nc[0]) : 0;
-        tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
+        tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
     }
     if (active) {
-        float4 a = S.acc[i];
-        if ((arho_only_arrays >> (meta >> SPH_META_IDX_BITS)) & 1u) a.w = ar;      // ContinuityEquation-only destination array
-        else a = make_float4(ax, ay, DIM == 3 ? az : 0.0f, ARHO ? ar : a.w);
+        float4 a;
+        if ((roles.arho_only >> aid_i) & 1u) {                          // ContinuityEquation-only destination array
+            a = ((roles.keep_xyz >> aid_i) & 1u) ? S.acc[i] : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            a.w = ar;
+        } else a = make_float4(ax, ay, DIM == 3 ? az : 0.0f, ARHO ? ar : 0.0f);
         S.acc[i] = a;
         if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
-    const unsigned long long h = warp_sum_u64(FILTER ? fhits : st.hits + rhits), t = warp_sum_u64(st.tests);
+    const unsigned long long h = warp_sum_u64(nhits), t = warp_sum_u64(st.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); if (t) atomicAdd(&counters[CNT_CAND_ACCEL], t); }
 }
 
 template <int KERNEL, int DIM>
-static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, uint32_t arho_only, bool replay) {
+static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, const AccelRoles& roles, bool replay) {
     const int n = (int)c->n_total;
     if (n == 0) return SPH_OK;
     const bool varh = c->variable_h;
     SortedState& S = c->S[c->cur];
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
-    const uint32_t ao = arho_only;
-    const int pm = varh ? 0 : (c->pc.uniform_m ? 2 : ((c->p_is_eos && c->pc.gamma_is_7) ? 1 : 0));
+    // velm.w carries rho when h is constant or every mass is equal (SortedState)
+    const bool eos7 = c->p_is_eos && c->pc.gamma_is_7;
+    const int pm = varh ? (c->pc.varh_um ? 1 : 0) : (c->pc.uniform_m ? 2 : (eos7 ? 1 : 0));
     const bool lam = c->pc.nu4 != 0.0f;
 #define LT(VARH, ARHO, FILTER, REPLAY, PM, LAM) \
-        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PM, LAM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, ao, c->nl, c->counters)
+        SPH_LAUNCH(c, (REPLAY ? SPH_K_ACCEL_LIST : SPH_K_ACCEL), (k_accel_tile<KERNEL, DIM, VARH, ARHO, FILTER, REPLAY, PM, LAM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, roles, c->nl, c->counters)
 #define LT0(VARH, ARHO, FILTER, REPLAY, PM) do { if (lam) LT(VARH, ARHO, FILTER, REPLAY, PM, true); else LT(VARH, ARHO, FILTER, REPLAY, PM, false); } while (0)
 #define LT1(VARH, ARHO, FILTER, PM) do { if (replay) LT0(VARH, ARHO, FILTER, true, PM); else LT0(VARH, ARHO, FILTER, false, PM); } while (0)
 #define LT2(VARH, ARHO, PM) do { if (filter) LT1(VARH, ARHO, true, PM); else LT1(VARH, ARHO, false, PM); } while (0)
 #define LT3(VARH, PM) do { if (want_arho) LT2(VARH, true, PM); else LT2(VARH, false, PM); } while (0)
-    if (varh) LT3(true, 0); else if (pm == 2) LT3(false, 2); else if (pm == 1) LT3(false, 1); else LT3(false, 0);
+    if (varh) { if (pm == 1) LT3(true, 1); else LT3(true, 0); } else if (pm == 2) LT3(false, 2); else if (pm == 1) LT3(false, 1); else LT3(false, 0);
 #undef LT3
 #undef LT2
 #undef LT1
@@ -150,16 +167,16 @@ static int launch_accel_tile_kd(sph_ctx* c, bool filter, bool want_arho, uint32_
 
 #define SPH_CAT2(a, b) a##b
 #define SPH_CAT(a, b) SPH_CAT2(a, b)
-int SPH_CAT(launch_accel_k, SPH_ACCEL_KERNEL)(sph_ctx* c, int dim, bool filter, bool want_arho, uint32_t arho_only, bool replay) {
-    return dim == 2 ? launch_accel_tile_kd<SPH_ACCEL_KERNEL, 2>(c, filter, want_arho, arho_only, replay)
-                    : launch_accel_tile_kd<SPH_ACCEL_KERNEL, 3>(c, filter, want_arho, arho_only, replay);
+int SPH_CAT(launch_accel_k, SPH_ACCEL_KERNEL)(sph_ctx* c, int dim, bool filter, bool want_arho, const AccelRoles& roles, bool replay) {
+    return dim == 2 ? launch_accel_tile_kd<SPH_ACCEL_KERNEL, 2>(c, filter, want_arho, roles, replay)
+                    : launch_accel_tile_kd<SPH_ACCEL_KERNEL, 3>(c, filter, want_arho, roles, replay);
 }
 
 #else
-// One launch serves every destination array whose mask is non-zero.  arho_only: bit a = array a stores only its
-// continuity sum (ContinuityEquation(dest=solid, sources=[fluid]), Listing 3).
-int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, uint32_t arho_only) {
-    bool filter = false, use_list = c->nl_valid && !arho_only;
+// One launch serves every destination array whose mask is non-zero.  roles.arho_only: bit a = array a stores only
+// its continuity sum (ContinuityEquation(dest=solid, sources=[fluid]), Listing 3).
+int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, const AccelRoles& roles) {
+    bool filter = false, use_list = c->nl_valid && !roles.arho_only;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
         if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) filter = true;
@@ -168,10 +185,10 @@ int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, 
     c->last_used_rows = use_list;
     const int k = c->prm.kernel, d = c->grid.dim;
     if (d != 2 && d != 3) return sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
-    const bool wa = want_arho || arho_only != 0u;
-    if (k == SPH_KERNEL_CUBIC)       return launch_accel_k0(c, d, filter, wa, arho_only, use_list);
-    if (k == SPH_KERNEL_QUINTIC)     return launch_accel_k1(c, d, filter, wa, arho_only, use_list);
-    if (k == SPH_KERNEL_WENDLAND_C2) return launch_accel_k2(c, d, filter, wa, arho_only, use_list);
+    const bool wa = want_arho || roles.arho_only != 0u;
+    if (k == SPH_KERNEL_CUBIC)       return launch_accel_k0(c, d, filter, wa, roles, use_list);
+    if (k == SPH_KERNEL_QUINTIC)     return launch_accel_k1(c, d, filter, wa, roles, use_list);
+    if (k == SPH_KERNEL_WENDLAND_C2) return launch_accel_k2(c, d, filter, wa, roles, use_list);
     return sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
 }
 #endif

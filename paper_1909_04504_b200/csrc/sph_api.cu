@@ -64,6 +64,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     if (params->kernel < 0 || params->kernel > SPH_KERNEL_WENDLAND_C2) return SPH_ERR_BAD_ARG;
     if (!(params->rho0 > 0) || !(params->c0 > 0) || !(params->gamma > 0)) return SPH_ERR_BAD_ARG;
     if (params->xsub < 0 || params->xsub > 16) return SPH_ERR_BAD_ARG;
+    if (params->levels < 0 || params->levels > SPH_MAX_LEVELS) return SPH_ERR_BAD_ARG;
     if (params->integrator != SPH_INTEGRATOR_PC && params->integrator != SPH_INTEGRATOR_EULER) return SPH_ERR_BAD_ARG;
     if (!(params->nu >= 0) || !(params->eta >= 0)) return SPH_ERR_BAD_ARG;
     for (int k = 0; k < domain->dim; ++k) if (!(domain->hi[k] > domain->lo[k])) return SPH_ERR_BAD_ARG;
@@ -88,15 +89,13 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     set_consts(c);
     c->xsub = params->xsub ? params->xsub : 6;
     c->xsub_auto = params->xsub == 0;
-    if (const char* e = getenv("SPH_XSUB")) { int v = atoi(e); if (v >= 1 && v <= 16) { c->xsub = v; c->xsub_auto = false; } }   // tuning override
-    int nl_slots = params->nlist_slots ? params->nlist_slots : 192;
-    if (const char* e = getenv("SPH_NLIST_SLOTS")) { int v = atoi(e); if (v != 0) nl_slots = v; }
+    const int nl_slots = params->nlist_slots ? params->nlist_slots : 192;
     *out = c;                                  // so the caller can read sph_last_error / destroy on failure
     SPH_CUDA_OK(c, cudaGetDevice(&c->device));
     SPH_CUDA_OK(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
 
     const size_t N = (size_t)tot + 1;
-    c->max_keys = 8 * tot + 65536; if (c->max_keys > ((int64_t)1 << 26)) c->max_keys = (int64_t)1 << 26;
+    c->max_keys = 8 * tot + 65536; if (c->max_keys > ((int64_t)1 << 27)) c->max_keys = (int64_t)1 << 27;
     for (int b = 0; b < 2; ++b) {
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].posh, N * sizeof(float4)));
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].velm, N * sizeof(float4)));
@@ -158,49 +157,69 @@ extern "C" int sph_set_tables(sph_ctx* c, const uint32_t* density_src, const uin
     return SPH_OK;
 }
 
-// cell >= k*h_max (L158-160) with a margin that absorbs the float rounding of the cell coordinate.
+// Level grids.  One level when h is constant: cell >= k*h_max (L158-160) with a margin that absorbs the float
+// rounding of the cell coordinate.  When h varies the particles are binned into geometric h classes (ratio <= ~1.6
+// per level) and every level gets its own grid with cell >= k * (largest h of the level): the paper's remedy for
+// "cells become too large" (L158-160, L171) without giving up the sort-by-cell-key structure.
 static int size_grid(sph_ctx* c) {
     GridDesc& g = c->grid;
     memset(&g, 0, sizeof(g));
     g.dim = c->dom.dim; g.na = c->na;
-    const double cutoff = kernel_support(c->prm.kernel) * (double)c->h_max;
-    if (!(cutoff > 0.0)) return sph_fail(c, SPH_ERR_BAD_ARG, "h_max must be positive");
-    double scale = 1.0;
+    const double ksup = kernel_support(c->prm.kernel);
+    if (!((double)c->h_max > 0.0)) return sph_fail(c, SPH_ERR_BAD_ARG, "h_max must be positive");
+    double big = 0.0;
+    for (int k = 0; k < 3; ++k) {
+        g.per[k] = (k < g.dim) ? (c->dom.periodic[k] != 0) : 0;
+        g.lo[k] = (float)c->dom.lo[k]; g.hi[k] = (float)c->dom.hi[k];
+        g.L[k] = (float)(c->dom.hi[k] - c->dom.lo[k]);
+        if (k < g.dim) big = fmax(big, fmax(fmax(fabs(c->dom.lo[k]), fabs(c->dom.hi[k])), c->dom.hi[k] - c->dom.lo[k]));
+    }
+    g.uabs = (float)(1.1920929e-7 * big);
+    const double ratio = (double)c->h_max / (double)c->h_min;
+    int nlev = 1;
+    if (c->variable_h) {
+        nlev = c->prm.levels > 0 ? c->prm.levels : (int)ceil(log(ratio) / log(1.6) - 1.0e-9);
+        nlev = nlev < 1 ? 1 : (nlev > SPH_MAX_LEVELS ? SPH_MAX_LEVELS : nlev);
+    }
     int xsub = c->xsub;
-    if (c->xsub_auto && c->variable_h) xsub = 16;      // variable h: finer x windows pay (reach < cell for small-h groups)
-    for (int iter = 0; iter < 64; ++iter) {
-        int64_t total = 1; bool ok = true;
-        for (int k = 0; k < 3; ++k) {
-            g.per[k] = (k < g.dim) ? (c->dom.periodic[k] != 0) : 0;
-            const double L = (k < g.dim) ? c->dom.hi[k] - c->dom.lo[k] : 1.0;
-            int n = 1;
-            if (k < g.dim) {
-                double est = L / (cutoff * scale);
-                double margin = 1.0e-3 + 4.0e-7 * est;
-                double nd = floor(L / (cutoff * scale * (1.0 + margin)));
-                if (nd > 1.0e6) nd = 1.0e6;
-                n = nd < 1.0 ? 1 : (int)nd;
-                if (g.per[k] && n < 3) {
-                    if (scale > 1.0) ok = false;      // cannot coarsen further
-                    else return sph_fail(c, SPH_ERR_BAD_ARG, "a periodic axis needs at least 3 cells of size k*h_max");
+    if (c->xsub_auto && c->variable_h) xsub = 4;
+    double scale = 1.0;
+    for (int iter = 0; iter < 96; ++iter) {
+        int64_t total = 0; bool ok = true;
+        for (int l = 0; l < nlev && ok; ++l) {
+            LevelDesc& Lv = g.lev[l];
+            // every h of level l is <= hmax_l (float thresholds; level_of_h uses the same comparisons on both sides)
+            Lv.hmax = (l == nlev - 1) ? c->h_max : (float)((double)c->h_min * pow(ratio, (l + 1.0) / nlev));
+            if (l == nlev - 1 || Lv.hmax > c->h_max) Lv.hmax = c->h_max;
+            const double cutoff = ksup * (double)Lv.hmax;
+            int64_t cells = 1;
+            for (int k = 0; k < 3; ++k) {
+                const double L = (k < g.dim) ? c->dom.hi[k] - c->dom.lo[k] : 1.0;
+                int n = 1;
+                if (k < g.dim) {
+                    const double est = L / (cutoff * scale);
+                    const double margin = 1.0e-3 + 4.0e-7 * est;
+                    double nd = floor(L / (cutoff * scale * (1.0 + margin)));
+                    if (nd > 1.0e6) nd = 1.0e6;
+                    n = nd < 1.0 ? 1 : (int)nd;
+                    if (g.per[k] && n < 3) {
+                        if (scale > 1.0) { ok = false; break; }      // cannot coarsen further
+                        return sph_fail(c, SPH_ERR_BAD_ARG, "a periodic axis needs at least 3 cells of size k*h_max");
+                    }
                 }
+                if (k == 0) n *= xsub;
+                Lv.nc[k] = n;
+                Lv.inv_cell[k] = (float)(n / L);
+                cells *= n;
             }
-            if (k == 0) n *= xsub;
-            g.nc[k] = n;
-            g.lo[k] = (float)c->dom.lo[k]; g.hi[k] = (float)c->dom.hi[k];
-            g.L[k] = (float)(c->dom.hi[k] - c->dom.lo[k]);
-            g.inv_cell[k] = (float)(n / L);
-            g.cell[k] = (float)(L / n);
-            // culling margin: 1e-3 cell + 8 ulp of the largest coordinate (rounding of positions, cell
-            // coordinates and slab bounds; the bounds only have to be conservative)
-            const double big = fmax(fmax(fabs(c->dom.lo[k]), fabs(c->dom.hi[k])), L);
-            g.marg[k] = (float)(1.0e-3 * (L / n) + 8.0 * 1.1920929e-7 * big + 4.0e-7 * L);
-            total *= n;
+            Lv.xsub = xsub;
+            Lv.base = (uint32_t)total;
+            total += cells;
+            if (total > ((int64_t)1 << 30)) ok = false;
         }
-        g.xsub = xsub;
-        if (!ok) return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
-        if (total * c->na <= c->max_keys) { c->n_keys = total * c->na; return SPH_OK; }
-        if (xsub > 1) xsub /= 2; else scale *= 1.26;
+        g.nlev = nlev;
+        if (ok && total * c->na <= c->max_keys) { c->n_keys = total * c->na; return SPH_OK; }
+        if (xsub > 1) xsub /= 2; else if (nlev > 1) --nlev; else scale *= 1.26;
     }
     return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
 }
@@ -260,7 +279,9 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     else { memcpy(&c->h_min, &hmm[0], 4); memcpy(&c->h_max, &hmm[1], 4); }
     if (!(c->h_max > 0.0f) || !isfinite(c->h_max)) return sph_fail(c, SPH_ERR_BAD_ARG, "smoothing lengths must be positive and finite");
     c->variable_h = (c->h_min != c->h_max);
+    c->p_is_eos = !any_p;
     c->pc.uniform_m = (tot > 0 && !c->variable_h && hmm[2] == hmm[3]) ? 1 : 0;
+    c->pc.varh_um = (tot > 0 && c->variable_h && hmm[2] == hmm[3] && c->p_is_eos && c->pc.gamma_is_7) ? 1 : 0;
     memcpy(&c->pc.m_const, &hmm[3], 4);
     c->pc.h_const = c->h_max;
     c->pc.hinv_const = (float)(1.0 / (double)c->h_max);
@@ -269,7 +290,7 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));   // once per build; k_scan re-clears it
     rc = nnps_key_hist(c); if (rc) return rc;
     rc = nnps_sort_from_keys(c, true); if (rc) return rc;
-    c->built = true; c->steps_done = 0; c->p_is_eos = !any_p;
+    c->built = true; c->steps_done = 0;
     c->have_accel = all_acc && tot > 0; c->have_arho = all_arho && tot > 0;     // restart from caller-supplied a^n
     return SPH_OK;
 }
@@ -312,7 +333,8 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
     uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
     masks[dest] = source_mask;
     int rc = zero_counters(c, CNT_PAIRS_ACCEL, CNT_CAND_ACCEL); if (rc) return rc;
-    rc = launch_accel(c, masks, arho != nullptr, 0u); if (rc) return rc;
+    const AccelRoles roles = { 0u, 0u, 0u, 0u };
+    rc = launch_accel(c, masks, arho != nullptr, roles); if (rc) return rc;
     if (ax || ay || az || arho) { OutPtrs O; memset(&O, 0, sizeof(O)); O.ax = ax; O.ay = ay; O.az = az; O.arho = arho; return emit(c, dest, O, mem); }
     return SPH_OK;
 }
@@ -348,12 +370,25 @@ static int evaluate(sph_ctx* c, bool continuity) {
         if (rc) return rc;
     }
     bool fused[SPH_MAX_ARRAYS], plain[SPH_MAX_ARRAYS], only[SPH_MAX_ARRAYS];
+    // arrays whose acc.xyz / acc.w NO launch of this evaluation computes get zeros from the first launch (the sort
+    // does not carry acc along: what lies in their rows belongs to other particles)
+    AccelRoles first = { 0u, 0u, 0u, 0u };
+    uint32_t keep = 0u;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         const bool acc = a < c->na && c->tbl_accel[a] != 0;
         const bool same = acc && continuity && c->tbl_arho[a] == c->tbl_accel[a];
         fused[a] = same; plain[a] = acc && !same;
         only[a] = a < c->na && continuity && c->tbl_arho[a] != 0 && !same;
+        if (a < c->na && !acc) first.zero_xyz |= 1u << a;
+        if (a < c->na && !(continuity && c->tbl_arho[a] != 0)) first.zero_w |= 1u << a;
+        if (plain[a]) keep |= 1u << a;
     }
+    bool launched = false;
+    auto accel = [&](const uint32_t* m, bool want_arho, uint32_t arho_only, bool after_plain) -> int {
+        AccelRoles r = { arho_only, after_plain ? (arho_only & keep) : 0u, launched ? 0u : first.zero_xyz, launched ? 0u : first.zero_w };
+        launched = true;
+        return launch_accel(c, m, want_arho, r);
+    };
     // continuity mode: when no array needs two different source sets, ONE launch serves them all (fluid: momentum +
     // continuity from {fluid, solid}; solid: continuity only from {fluid}; the per-lane source mask filters)
     bool one = continuity;
@@ -365,13 +400,16 @@ static int evaluate(sph_ctx* c, bool continuity) {
             else if (only[a]) { masks[a] = c->tbl_arho[a]; ao |= 1u << a; }
             any = any || masks[a] != 0u;
         }
-        return any ? launch_accel(c, masks, true, ao) : SPH_OK;
+        if (any) { rc = accel(masks, true, ao, false); if (rc) return rc; }
+    } else {
+        rc = grouped(c->tbl_accel, fused, [&](const uint32_t* m) { return accel(m, true, 0u, false); }); if (rc) return rc;
+        rc = grouped(c->tbl_accel, plain, [&](const uint32_t* m) { return accel(m, false, 0u, false); }); if (rc) return rc;
+        rc = grouped(c->tbl_arho, only, [&](const uint32_t* m) {
+            uint32_t ao = 0u; for (int a = 0; a < c->na; ++a) if (m[a]) ao |= 1u << a;
+            return accel(m, true, ao, true); }); if (rc) return rc;
     }
-    rc = grouped(c->tbl_accel, fused, [&](const uint32_t* m) { return launch_accel(c, m, true, 0u); }); if (rc) return rc;
-    rc = grouped(c->tbl_accel, plain, [&](const uint32_t* m) { return launch_accel(c, m, false, 0u); }); if (rc) return rc;
-    rc = grouped(c->tbl_arho, only, [&](const uint32_t* m) {
-        uint32_t ao = 0u; for (int a = 0; a < c->na; ++a) if (m[a]) ao |= 1u << a;
-        return launch_accel(c, m, true, ao); }); if (rc) return rc;
+    if (!launched && c->n_total > 0)      // no momentum / continuity destination at all: every acceleration is zero
+        SPH_CUDA_OK(c, cudaMemsetAsync(c->S[c->cur].acc, 0, (size_t)c->n_total * sizeof(float4), c->stream));
     return SPH_OK;
 }
 
@@ -445,10 +483,13 @@ extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
     unsigned long long h[CNT_COUNT];
     int rc = read_counters(c, h); if (rc) return rc;
     memset(out, 0, sizeof(*out));
+    const LevelDesc& top = c->grid.lev[c->grid.nlev > 0 ? c->grid.nlev - 1 : 0];    // the coarsest level: cells >= k h_max
     for (int k = 0; k < 3; ++k) {
-        out->n_cells[k] = c->grid.nc[k];
-        out->cell_size[k] = c->grid.nc[k] ? (c->dom.hi[k] - c->dom.lo[k]) / c->grid.nc[k] : 0.0;
+        out->n_cells[k] = top.nc[k];
+        out->cell_size[k] = top.nc[k] ? (c->dom.hi[k] - c->dom.lo[k]) / top.nc[k] : 0.0;
     }
+    out->n_levels = c->grid.nlev;
+    out->n_keys = c->n_keys;
     out->n_particles = c->n_total;
     out->pairs_density = (int64_t)h[CNT_PAIRS_DENSITY];
     out->pairs_accel = (int64_t)h[CNT_PAIRS_ACCEL];
@@ -459,7 +500,7 @@ extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->steps_done = c->steps_done;
     out->variable_h = c->variable_h ? 1 : 0;
     out->h_max = c->h_max;
-    out->xsub = c->grid.xsub;
+    out->xsub = top.xsub;
     out->used_rows = c->last_used_rows ? 1 : 0;
     out->nlist_rows_capacity = c->nl.pool_rows;
     out->nlist_fallback_warps = (int64_t)h[CNT_OVERFLOW];

@@ -35,7 +35,6 @@ struct sph_ctx {
     uint32_t *cell_count, *cell_start;
     unsigned long long* scan_state; uint32_t* scan_ticket; uint32_t scan_epoch;   // k_scan look-back table
     float* staging;            // host<->device staging for SPH_MEM_HOST (10 floats per particle of capacity)
-    float* out_tmp;            // device scratch for caller-order outputs (4 floats per particle of capacity)
     unsigned long long* counters;     // device, CNT_COUNT entries
     float* hminmax;            // device, 4 floats (as ordered ints): h min/max, |m| min/max
 
@@ -90,4 +89,10 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
                           int64_t* total, int mem);
 // sph_density.cu / sph_accel.cu: one launch serves every dest array whose mask is non-zero
 int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record);
-int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, uint32_t arho_only);
+// what a momentum launch stores for which array (bitmasks over arrays)
+struct AccelRoles {
+    uint32_t arho_only;        // destination arrays that store only their continuity sum (acc.w)
+    uint32_t keep_xyz;         // ... of those, arrays whose acc.xyz an earlier launch of this evaluation computed (kept); the others get 0
+    uint32_t zero_xyz, zero_w; // arrays that are NO destination of this launch and whose acc.xyz / acc.w no launch of the evaluation computes: zeroed
+};
+int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, const AccelRoles& roles);

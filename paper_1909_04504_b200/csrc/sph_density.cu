@@ -16,71 +16,69 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     const int warp_id = i >> 5;
     const bool in = i < n;
     uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
-    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; }
+    if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = ld_state(S.posh + i); }
     const uint32_t my_mask = in ? pc.src_mask[meta >> SPH_META_IDX_BITS] : 0u;
     const bool active = my_mask != 0u;
     if (!__any_sync(SPH_FULL_MASK, active)) return;
-    const int row = in ? (int)(ci / (uint32_t)g.nc[0]) : -1;
-    const int sub = in ? (int)(ci % (uint32_t)g.nc[0]) : 0;
 
     const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
-    const float iLx = 1.0f / g.L[0], iLy = 1.0f / g.L[1], iLz = 1.0f / g.L[2];
-    const float sigma = pc.sigma, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
+    const float sigma = pc.sigma, hinv_c = pc.hinv_const, fac_c = pc.fac_const, kh = pc.kh;
     const float hi = VARH ? pi.w : pc.h_const;
+    const float cut2c = pair_cut2(kh, pc.h_const, pc.h_const);
     const float mfac_c = pc.m_const * pc.fac_const;                     // UM layout: posh.w is p/rho^2, the mass is m_const
     float rho = 0.0f;
-    unsigned long long fhits = 0;                                       // FILTER: hits that pass the source mask
-    // constant h: posh.w of the sorted state carries the MASS (SortedState), one 16-byte gather per pair
+    unsigned nhits = 0;                                                 // pairs that pass the exact predicate (and the source mask)
+    // constant h: posh.w of the sorted state carries the MASS (SortedState), one 16-byte gather per pair.  Plain
+    // loads: the epilogue of this launch rewrites .w words of posh / velm that other warps' gathers cover (x, y, z
+    // never change and the .w they return is not used then).
     auto load = [&](uint32_t j) {
-        DensitySrc s; s.pj = __ldg(S.posh + j); s.mj = 0.0f; s.aid = 0u;
-        if (VARH) s.mj = __ldg(&S.velm[j].w);
+        DensitySrc s; s.pj = ld_state(S.posh + j); s.mj = 0.0f; s.aid = 0u;
+        if (VARH && !UM) s.mj = ld_state(&S.velm[j].w);            // VU layout (variable h, uniform mass): m = m_const
         if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
         return s;
     };
-    bool per = false;                                                   // warp-uniform: some stored batch is a periodic image
-    auto compute = [&](const DensitySrc& s, bool has) {
-        if (FILTER) { has = has && ((my_mask >> s.aid) & 1u); fhits += has ? 1u : 0u; }
-        float dx = pi.x - s.pj.x, dy = pi.y - s.pj.y, dz = DIM == 3 ? pi.z - s.pj.z : 0.0f;
-        if (per) {
-            dx = min_image(dx, Lx, iLx); dy = min_image(dy, Ly, iLy);
-            if (DIM == 3) dz = min_image(dz, Lz, iLz);
+    auto compute = [&](const DensitySrc& s, bool has, uint32_t code, auto per) {
+        // the exact predicate of DESIGN.md R7 on the candidate the tensor-core filter let through
+        float dx = __fsub_rn(pi.x, s.pj.x), dy = __fsub_rn(pi.y, s.pj.y), dz = DIM == 3 ? __fsub_rn(pi.z, s.pj.z) : 0.0f;
+        if (decltype(per)::value) {
+            dx = __fsub_rn(dx, img_shift(code, 0, Lx)); dy = __fsub_rn(dy, img_shift(code, 1, Ly));
+            if (DIM == 3) dz = __fsub_rn(dz, img_shift(code, 2, Lz));
         }
-        float r2 = fmaf(dy, dy, dx * dx);
-        if (DIM == 3) r2 = fmaf(dz, dz, r2);
+        const float r2 = pair_r2(dx, dy, dz);
+        has = has && r2 < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);
+        if (FILTER) has = has && ((my_mask >> s.aid) & 1u);
+        nhits += has ? 1u : 0u;
         const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;
         const float r = r2 * rinv;
         float hinv, mfac;
         if (VARH) {
             hinv = rcp_approx(0.5f * (hi + s.pj.w));
-            mfac = s.mj * sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
+            mfac = (UM ? pc.m_const : s.mj) * sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
         } else { hinv = hinv_c; mfac = UM ? mfac_c : s.pj.w * fac_c; }
         float f, df;
         kernel_profile<KERNEL, DIM>(r * hinv, f, df);
         rho = has ? fmaf(mfac, f, rho) : rho;
     };
 
-    TileState st; st.reset(); st.tests = 0; st.hits = 0;
+    TileState st; st.reset(); st.tests = 0;
     const uint32_t idle = in ? (uint32_t)i : 0u;
     TileRecorder rec; rec.init(nl); if (!RECORD) rec.ok = false;
     auto drain = [&]() {
         if (RECORD) rec.append(ws, st.M, st.shifted, warp_id, counters);
-        per = st.shifted;
-        tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY>(ws, st.nz, idle, load, compute);
+        if (st.shifted) tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, true>(ws, st.nz, idle, load, compute);
+        else            tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, false>(ws, st.nz, idle, load, compute);
         st.reset();
     };
-    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st, drain);
+    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, drain);
 
     if (active) {
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
         S.rp[i] = make_float2(rho, p / (rho * rho));
-        // The .w stores below touch words that NO thread of this launch reads (constant h: the tests and the drain
-        // use x,y,z of posh and, without UM, its .w = m, which is not written), so concurrent 16-byte gathers of the
-        // same record by other warps see unchanged x,y,z whichever version of .w they get.
-        if (!VARH) S.velm[i].w = rho;                                   // constant h: velm.w carries rho (SortedState)
-        if (UM) S.posh[i].w = p / (rho * rho);                          // UM layout: posh.w carries p/rho^2
+        if (!VARH || UM) S.velm[i].w = rho;                             // constant h, or VU layout: velm.w carries rho (SortedState)
+        if (UM && !VARH) S.posh[i].w = p / (rho * rho);                 // UM layout: posh.w carries p/rho^2
         if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
-    const unsigned long long h = warp_sum_u64(FILTER ? fhits : st.hits), t = warp_sum_u64(st.tests);
+    const unsigned long long h = warp_sum_u64(nhits), t = warp_sum_u64(st.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CAND_DENSITY], t); }
 }
 
@@ -94,7 +92,7 @@ static int launch_density_tile_kd(sph_ctx* c, bool filter, bool record) {
         SPH_LAUNCH(c, SPH_K_DENSITY, (k_density_tile<KERNEL, DIM, VARH, FILTER, RECORD, UM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters)
 #define LD2(VARH, FILTER, UM) do { if (record) LD(VARH, FILTER, true, UM); else LD(VARH, FILTER, false, UM); } while (0)
 #define LD3(VARH, UM) do { if (filter) LD2(VARH, true, UM); else LD2(VARH, false, UM); } while (0)
-    if (c->variable_h) LD3(true, false); else if (c->pc.uniform_m) LD3(false, true); else LD3(false, false);
+    if (c->variable_h) { if (c->pc.varh_um) LD3(true, true); else LD3(true, false); } else if (c->pc.uniform_m) LD3(false, true); else LD3(false, false);
 #undef LD3
 #undef LD2
 #undef LD

@@ -8,22 +8,36 @@
 #define SPH_META_IDX_BITS 28u                    // meta = (array id << 28) | original index
 #define SPH_META_IDX_MASK ((1u << SPH_META_IDX_BITS) - 1u)
 
-// Uniform cell grid (cells of size >= the support radius; 3^d neighbouring boxes).
-// y and z cells are >= the support radius; every such cell is split into `xsub` sub-cells along x (x is the
+// Cell grid (cells of size >= the support radius; L158-160, L171: one grid sized by h_max "becomes
+// inefficient" when h varies).  Particles are binned by h into `nlev` LEVELS (geometric h classes; one level when h
+// is constant); level l has its own uniform grid with cells >= k * hmax_l, all levels share ONE cell table and ONE
+// sorted order (key = (level base + linear cell) * na + array, level-major).  In every level grid the y and z cells
+// are >= the support radius of the level and every such cell is split into `xsub` sub-cells along x (x is the
 // fastest key digit, so a stencil row is one contiguous run and an x-interval of it is a contiguous sub-run).
-struct GridDesc {
-    int dim;
+#define SPH_MAX_LEVELS 8
+struct LevelDesc {
     int nc[3];                 // cells per axis (nc[2] = 1 in 2-D); nc[0] counts the x SUB-cells
     int xsub;                  // x sub-cells per support radius
-    int per[3];                // periodic per axis
+    uint32_t base;             // first cell of this level in the shared cell table (in cells; times na = key)
+    float inv_cell[3];         // 1 / cell size (x: sub-cell)
+    float hmax;                // every particle binned into this level has h <= hmax
+};
+struct GridDesc {
+    int dim;
     int na;                    // particle arrays merged into the grid: key = cell * na + array
+    int nlev;                  // levels in use (1 when h is constant)
+    int per[3];                // periodic per axis
     float lo[3];               // domain origin
-    float inv_cell[3];         // 1 / cell size
     float L[3];                // (float)(hi - lo): the period used by the neighbour predicate (R7)
     float hi[3];
-    float cell[3];             // cell size per axis (x: sub-cell size)
-    float marg[3];             // absolute safety margin of the conservative culling bounds
+    float uabs;                // 2^-23 * largest coordinate magnitude: absolute rounding unit of positions
+    LevelDesc lev[SPH_MAX_LEVELS];
 };
+__host__ __device__ inline int level_of_h(const GridDesc& g, float h) {
+    int l = 0;
+    while (l + 1 < g.nlev && h > g.lev[l].hmax) ++l;
+    return l;
+}
 
 // Neighbour rows recorded by the density pass and replayed by the acceleration pass.
 // The pool is an array of ROWS of 32 words (one word per lane of the warp that owns the row).  A warp appends
@@ -49,6 +63,7 @@ struct PairConsts {
     float visc;                // -2 alpha c0   (Pi = visc * h vr / ((r2 + eps h^2)(rho_i + rho_j)))
     float eps;
     float m_const; int uniform_m;   // constant h and every particle of every array has the same mass: the UM layout
+    int varh_um;               // variable h, uniform mass, gamma = 7 and p = EOS(rho): the VU layout (velm.w = rho, m = m_const)
     float nu4, eta;            // laminar viscosity eq.10: 4 nu (0 = term off) and its regulariser
     float g[3];
     uint32_t src_mask[SPH_MAX_ARRAYS];   // per DEST array: source-array bitmask; 0 = not a destination of this launch
@@ -64,7 +79,10 @@ struct SortedState {
                                //                     | recomputed from rho when p is the EOS of rho).  UM layout (all
                                //                     | masses equal too, PairConsts::uniform_m): posh = (x, y, z,
                                //                     | P/RHO^2) and the mass is the constant m_const: two gathers, no
-                               //                     | recomputation.
+                               //                     | recomputation.  VU layout (VARIABLE h, all masses equal, p is
+                               //                     | the gamma = 7 EOS of rho; PairConsts::varh_um): posh = (x, y, z,
+                               //                     | h), velm = (u, v, w, RHO), mass = m_const: the density loop gathers
+                               //                     | one word per neighbour, the momentum loop two.
     float2* rp;                // rho, p / rho^2   (p itself is returned as (p/rho^2) * rho^2)
     float4* acc;               // ax, ay, az, arho
     uint32_t* meta;            // (array << 28) | original index

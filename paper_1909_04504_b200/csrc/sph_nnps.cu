@@ -9,7 +9,8 @@
 // ------------------------------------------------------------------------------------------------
 // cell of a position (a1).  Linear key, x fastest, so the 3 x-adjacent cells of a stencil row are one run.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, bool& oob) {
+__device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, int level, bool& oob) {
+    const LevelDesc& Lv = g.lev[level];
     int c[3]; const float x[3] = { p.x, p.y, p.z };
     oob = false;
 #pragma unroll
@@ -17,10 +18,10 @@ __device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, bool& o
         if (a < g.dim) {
             if (!(x[a] >= g.lo[a] && x[a] <= g.hi[a])) oob = true;   // also catches NaN; periodic axes too:
                                                                       // the caller's positions must lie in the box
-            c[a] = cell_coord(x[a], g.lo[a], g.inv_cell[a], g.nc[a]);
+            c[a] = cell_coord(x[a], g.lo[a], Lv.inv_cell[a], Lv.nc[a]);
         } else c[a] = 0;
     }
-    return (uint32_t)((c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0]);
+    return Lv.base + (uint32_t)((c[2] * Lv.nc[1] + c[1]) * Lv.nc[0] + c[0]);
 }
 
 // Loads the caller's SoA arrays into the (not yet sorted) float4 groups and reduces h_min / h_max.
@@ -65,7 +66,8 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
     bool oob;
-    const uint32_t cell = cell_of(g, S.posh[i], oob);
+    const float4 p = S.posh[i];                                       // posh.w is still h here (k_pack; the layouts change at the sort)
+    const uint32_t cell = cell_of(g, p, level_of_h(g, p.w), oob);
     const uint32_t k = cell * (uint32_t)g.na + (S.meta[i] >> SPH_META_IDX_BITS);
     key[i] = k;
     rank[i] = atomicAdd(&cell_count[k], 1u);
@@ -129,7 +131,7 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
     }
     if (U.rekey) {
         bool oob;
-        const uint32_t cell = cell_of(g, pos, oob);
+        const uint32_t cell = cell_of(g, pos, g.nlev > 1 ? level_of_h(g, pos.w) : 0, oob);   // several levels only when h varies: posh.w = h
         const uint32_t k = cell * (uint32_t)g.na + aid;
         key[i] = k;
         rank[i] = atomicAdd(&cell_count[k], 1u);
@@ -237,8 +239,9 @@ k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass,
     float4 p = A.posh[i];
     float4 v = A.velm[i];
     const float2 r = A.rp[i];
-    // constant h, first sort after the pack (SortedState): velm.w <- rho; posh.w <- m, or <- p/rho^2 when the mass is uniform
-    if (w_mass) { p.w = w_mass == 2 ? r.y : v.w; v.w = r.x; }
+    // first sort after the pack (SortedState).  constant h: velm.w <- rho; posh.w <- m, or <- p/rho^2 when the mass is uniform
+    if (w_mass == 3) v.w = r.x;                                      // VU layout (variable h): velm.w <- rho, posh.w stays h
+    else if (w_mass) { p.w = w_mass == 2 ? r.y : v.w; v.w = r.x; }
     B.posh[d] = p;
     B.velm[d] = v;
     B.rp[d] = r;
@@ -261,7 +264,7 @@ int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, boo
     U.euler = c->prm.integrator == SPH_INTEGRATOR_EULER ? 1 : 0;
     U.dt_half = U.euler ? dt : 0.5f * dt;              // Euler: the one kick per step is a full dt
     U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
-    U.continuity = continuity; U.rekey = rekey; U.w_rho = c->variable_h ? 0 : 1; U.w_prr = (!c->variable_h && c->pc.uniform_m) ? 1 : 0;
+    U.continuity = continuity; U.rekey = rekey; U.w_rho = (!c->variable_h || c->pc.varh_um) ? 1 : 0; U.w_prr = (!c->variable_h && c->pc.uniform_m) ? 1 : 0;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
     if (n) SPH_LAUNCH(c, SPH_K_UPDATE, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
                       c->cell_count, c->counters);
@@ -273,7 +276,7 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys, true);   // leaves cell_count cleared
     if (rc) return rc;
     if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
-                      with_acc ? 1 : 0, (!c->variable_h && with_acc) ? (c->pc.uniform_m ? 2 : 1) : 0, c->key, c->rank, c->cell_start);
+                      with_acc ? 1 : 0, !with_acc ? 0 : (c->variable_h ? (c->pc.varh_um ? 3 : 0) : (c->pc.uniform_m ? 2 : 1)), c->key, c->rank, c->cell_start);
     c->cur ^= 1;
     c->nl_valid = false;                 // recorded neighbour rows index the previous sorted order
     return SPH_OK;
@@ -307,6 +310,8 @@ int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O) {
 // ------------------------------------------------------------------------------------------------
 // neighbour-list export (verification): the same warp-tile walker and predicate code as the pair kernels.
 // ------------------------------------------------------------------------------------------------
+struct NbSrc { float4 pj; uint32_t meta; };
+
 template <int DIM, bool VARH, bool FILL>
 __global__ void __launch_bounds__(TILE_BLOCK)
 k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
@@ -321,20 +326,28 @@ k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __res
     const bool active = in && (meta >> SPH_META_IDX_BITS) == dest;
     if (!__any_sync(SPH_FULL_MASK, active)) return;
     const uint32_t o = meta & SPH_META_IDX_MASK;
-    const int row = in ? (int)(ci / (uint32_t)g.nc[0]) : -1;
-    const int sub = in ? (int)(ci % (uint32_t)g.nc[0]) : 0;
+    const float hi = VARH ? pi.w : pc.h_const, kh = pc.kh;
+    const float cut2c = pair_cut2(kh, pc.h_const, pc.h_const);
     uint32_t cnt = 0;
     int32_t* out = FILL ? indices + (active ? offsets[o] : 0u) : nullptr;
-    auto load = [&](uint32_t j) { return __ldg(S.meta + j); };
-    auto compute = [&](const uint32_t& m, bool has) {
-        if (!has || (m >> SPH_META_IDX_BITS) != src) return;
-        if (FILL) out[cnt] = (int32_t)(m & SPH_META_IDX_MASK);
+    auto load = [&](uint32_t j) { NbSrc s; s.pj = __ldg(S.posh + j); s.meta = __ldg(S.meta + j); return s; };
+    auto compute = [&](const NbSrc& s, bool has, uint32_t code, auto per) {
+        float dx = __fsub_rn(pi.x, s.pj.x), dy = __fsub_rn(pi.y, s.pj.y), dz = DIM == 3 ? __fsub_rn(pi.z, s.pj.z) : 0.0f;
+        if (decltype(per)::value) {
+            dx = __fsub_rn(dx, img_shift(code, 0, g.L[0])); dy = __fsub_rn(dy, img_shift(code, 1, g.L[1]));
+            if (DIM == 3) dz = __fsub_rn(dz, img_shift(code, 2, g.L[2]));
+        }
+        has = has && pair_r2(dx, dy, dz) < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);     // the exact predicate R7
+        if (!has || (s.meta >> SPH_META_IDX_BITS) != src) return;
+        if (FILL) out[cnt] = (int32_t)(s.meta & SPH_META_IDX_MASK);
         ++cnt;
     };
-    TileState st; st.reset(); st.tests = 0; st.hits = 0;
+    TileState st; st.reset(); st.tests = 0;
     const uint32_t idle = in ? (uint32_t)i : 0u;
-    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, pi, row, sub, ws, st,
-                         [&]() { tile_drain<uint32_t>(ws, st.nz, idle, load, compute); st.reset(); });
+    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, [&]() {
+        if (st.shifted) tile_drain<NbSrc, 2, true>(ws, st.nz, idle, load, compute);
+        else            tile_drain<NbSrc, 2, false>(ws, st.nz, idle, load, compute);
+        st.reset(); });
     if (!active) return;
     if (!FILL) counts[o] = cnt;
     else {                                              // rows ascending (insertion sort; rows are short)

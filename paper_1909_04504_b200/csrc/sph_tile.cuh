@@ -1,22 +1,32 @@
-// Warp-tile pair machinery: candidate tests, hit masks, drain, mask records.
+// Warp-tile pair machinery: candidate walk, tensor-core filter, hit masks, drain,
+// mask records.
 //
-// Mapping.  A warp owns 32 consecutive particles of the CELL-SORTED order (x sub-cell fastest), i.e. a short
-// tube along x inside one stencil row (Fig.1).  For each of the 3^(d-1) neighbouring rows the
-// warp's candidates are ONE contiguous run of the sorted order: the sub-cells [sub_lo - xsub, sub_hi + xsub]
-// (a coarse cell = xsub sub-cells >= the support radius, so nothing closer than the cut-off lies outside).
+// Mapping.  A warp owns 32 consecutive particles of the CELL-SORTED order (level-major, x sub-cell fastest), i.e.
+// a short tube along x inside one stencil row of its level grid (Fig.1).  Lanes of one level and
+// row without a wide x gap form a GROUP.  For every group and every level b of the grid (one level when h is
+// constant; PAPER.md L158-160, L171 for variable h) the candidates are the cells of level b that meet the
+// group's bounding box grown by the reach R = k (h_group_max + h_max,b) / 2: a (rows in y) x (rows in z) set of
+// stencil rows, each ONE contiguous run of the sorted order (+ the images across a periodic seam as separate runs
+// with their shift code).  32 lanes look the runs up in parallel, one flat loop streams them 32 candidates at a
+// time; the next batch is prefetched into registers while the current one is tested.
 //
-// Phase 1 (tests).  The run is read once, coalesced, 32 candidates at a time, and staged as SoA in shared
-// memory; every lane then tests ITS particle against the SAME candidate, read as a shared-memory broadcast
-// (no divergent loads, no bank conflicts), four candidates per step with packed f32x2 arithmetic (FADD2 /
-// FMUL2 / FFMA2, sm_100).  The arithmetic is the bit-specified predicate of DESIGN.md R7; rounding of the
-// packed forms is the same round-to-nearest as the scalar forms.  The result is one 32-bit hit mask per lane
-// and batch, stored to shared memory (mask[m][lane]) with the batch's first sorted index (base[m]).
-// Phase 2 (evaluation).  When the mask store is full, and once at the end, the warp drains it: every lane pops
-// its own hits in order and runs the expensive body (kernel, EOS terms, viscosity) on them, so the body runs
-// at mean/max neighbour-count lane utilisation instead of the hit rate of the tests.
-// Records.  A recording pass also copies the masks and bases (not the hit indices: 4 B per 32 tests instead of
-// 4 B per hit) to the record pool; the acceleration pass of the same evaluation replays them (tile_replay)
-// and tests nothing.
+// Phase 1 (filter).  The 32 x 32 squared distances of a batch are a small dense contraction,
+//     s_ij = |x_i - x_j|^2 - cut_ij^2 = n_i + n_j - 2 x_i . x_j - 2 kh^2 h_i h_j ,   n = |x|^2 - kh^2 h^2 ,
+// so it runs on the tensor cores: 8 mma.sync.m16n8k8 (tf32 operands, fp32 accumulators) per batch, operands
+// [-2x, -2y, -2z, -2 kh^2 h, n_hi, n_lo, 1, 1] . [x, y, z, h, 1, 1, n_hi, n_lo] in coordinates relative to the
+// group's centre, rounded to tf32 (n split into two tf32 words).  tf32 cannot decide the bit-specified predicate
+// of DESIGN.md R7, so the tensor-core result is only a CONSERVATIVE filter: a margin that bounds the rounding
+// (derived in DESIGN.md "Tensor-core filter") is subtracted on the candidate side, the sign bits of the
+// accumulators are collected with one funnel shift each, and a 4 x 4 byte transpose inside every quad gives each
+// lane the 32-bit mask of ITS particle for the batch: a superset of its neighbours (+ ~4 %).
+// Phase 2 (evaluation).  When the mask store is full, and once at the end, the warp drains it: every lane pops its
+// own candidates in order, applies the EXACT float predicate R7 (image-specific shift, fl(x_i - x_j), fma chain,
+// r2 < cut2) and runs the expensive body (kernel, EOS terms, viscosity) on the true neighbours, so the body runs at
+// mean/max neighbour-count lane utilisation instead of the hit rate of the tests.  Set membership is therefore
+// decided by exactly the expression the oracle uses; the filter only has to have no false negatives.
+// Records.  A recording pass also copies the masks, bases and shift codes (not the hit indices: 4 B per 32 tests
+// instead of 4 B per hit) to the record pool; the acceleration pass of the same evaluation replays them
+// (tile_replay), applies the same exact predicate and walks nothing.
 #pragma once
 #include "sph_ctx.cuh"
 #include <type_traits>
@@ -27,262 +37,342 @@
 #define TILE_MIN_BLOCKS 8                 // resident blocks per SM the pair kernels are compiled for (64 registers)
 #endif
 #ifndef TILE_MIN_BLOCKS_ACCEL
-#define TILE_MIN_BLOCKS_ACCEL 6           // the momentum kernel is 3-8 % faster with 80 registers and 6 blocks (measured, C3, C4)
+#define TILE_MIN_BLOCKS_ACCEL 6           // the momentum kernel is faster with 80 registers and 6 blocks (measured, C3, C4)
 #endif
 #ifndef TILE_DRAIN_DEPTH_REPLAY
-#define TILE_DRAIN_DEPTH_REPLAY 3         // hits in flight in the replaying momentum kernel (-4 % on C3; the searching kernels lose with 3)
+#define TILE_DRAIN_DEPTH_REPLAY 3         // hits in flight in the replaying momentum kernel
 #endif
 #ifndef TILE_DRAIN_DEPTH_DENSITY
-#define TILE_DRAIN_DEPTH_DENSITY 3         // hits in flight in the density drain (3: -2 % on C3; 4 is no better)
+#define TILE_DRAIN_DEPTH_DENSITY 3        // hits in flight in the density drain
 #endif
 #ifndef TILE_MMAX
-#define TILE_MMAX 30                       // masks per warp before a forced drain (<= 30: 30 bases + 2 words = one header row)
+#define TILE_MMAX 24                      // masks per warp before a forced drain (<= 30: 30 bases + 2 words = one header row)
 #endif
 
 struct __align__(16) TileWarpSmem {
-    float x[32], y[32], z[32], h[32];      // one staged batch of candidates, SoA
-    uint32_t mask[TILE_MMAX][32];          // hit masks, [batch][lane]
+    union {
+        float2 G[4][34];                   // B operands of one batch: G[t][c] = (feature t, feature t+4) of staged candidate c
+        float Af[32 * 9];                  // A operands of a group while the quads exchange them (stride 9: conflict-free)
+    };
+    uint32_t mask[TILE_MMAX][32];          // candidate masks, [batch][lane]
     uint32_t base[32];                     // first sorted index of every batch
-    uint32_t seg_s[32], seg_e[32], seg_c[32];   // candidate runs of the current group: [s, e) and image-shift code
+    uint32_t bcode[32];                    // image-shift code of every batch (2 bits per axis: 1 -> -L, 2 -> +L)
+    uint32_t seg_s[32], seg_e[32], seg_c[32];   // candidate runs of the current pass: [s, e) and image-shift code
 };
 
 struct TileState {
     int M;                                 // masks stored since the last drain (warp-uniform)
-    uint32_t nz;                           // bit m: this lane's mask m has hits
+    uint32_t nz;                           // bit m: this lane's mask m is not empty
     bool shifted;                          // some stored batch came from a periodic image (warp-uniform)
-    unsigned long long tests;              // predicate evaluations of this lane's particle
-    unsigned long long hits;               // predicate hits of this lane's particle
+    unsigned long long tests;              // candidates streamed for this lane's particle
     __device__ __forceinline__ void reset() { M = 0; nz = 0u; shifted = false; }
 };
 
-__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
-__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, f2(-b.x, -b.y)); }
+// plain (coherent) loads of the sorted state: the density pass rewrites .w words of records that other warps gather
+template <class T> __device__ __forceinline__ T ld_state(const T* p) { return *p; }
 
-// Predicate of DESIGN.md R7 for 4 staged candidates c..c+3 against this lane's particle: bit k of the result
-// is the hit of candidate c+k.   d = fl(fl(x_i - x_j) - shift);  r2 = fma(dz,dz,fma(dy,dy,fl(dx*dx)));
-// cut = fl(kh * fl(h_i + h_j));  hit <=> r2 < fl(cut*cut).
-template <int DIM, bool VARH, bool SHIFT>
-__device__ __forceinline__ uint32_t tile_test4(const TileWarpSmem& ws, int c, float2 xi, float2 yi, float2 zi,
-                                               float2 sx, float2 sy, float2 sz, float2 cut2c, float2 kh2, float2 hi2) {
-    const float4 X = *reinterpret_cast<const float4*>(ws.x + c);
-    const float4 Y = *reinterpret_cast<const float4*>(ws.y + c);
-    float2 dxa = sub2(xi, f2(X.x, X.y)), dxb = sub2(xi, f2(X.z, X.w));
-    float2 dya = sub2(yi, f2(Y.x, Y.y)), dyb = sub2(yi, f2(Y.z, Y.w));
-    if (SHIFT) { dxa = sub2(dxa, sx); dxb = sub2(dxb, sx); dya = sub2(dya, sy); dyb = sub2(dyb, sy); }
-    float2 ra = __ffma2_rn(dya, dya, __fmul2_rn(dxa, dxa));
-    float2 rb = __ffma2_rn(dyb, dyb, __fmul2_rn(dxb, dxb));
-    if (DIM == 3) {
-        const float4 Z = *reinterpret_cast<const float4*>(ws.z + c);
-        float2 dza = sub2(zi, f2(Z.x, Z.y)), dzb = sub2(zi, f2(Z.z, Z.w));
-        if (SHIFT) { dza = sub2(dza, sz); dzb = sub2(dzb, sz); }
-        ra = __ffma2_rn(dza, dza, ra); rb = __ffma2_rn(dzb, dzb, rb);
-    }
-    float2 ca = cut2c, cb = cut2c;
-    if (VARH) {
-        const float4 H = *reinterpret_cast<const float4*>(ws.h + c);
-        const float2 ta = __fmul2_rn(kh2, __fadd2_rn(hi2, f2(H.x, H.y)));
-        const float2 tb = __fmul2_rn(kh2, __fadd2_rn(hi2, f2(H.z, H.w)));
-        ca = __fmul2_rn(ta, ta); cb = __fmul2_rn(tb, tb);
-    }
-    uint32_t m = 0;
-    if (ra.x < ca.x) m |= 1u;
-    if (ra.y < ca.y) m |= 2u;
-    if (rb.x < cb.x) m |= 4u;
-    if (rb.y < cb.y) m |= 8u;
-    return m;
+__device__ __forceinline__ float tf32r(float x) {           // round to tf32 (10 explicit mantissa bits), half away from zero
+    return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+}
+__device__ __forceinline__ uint32_t f2ord(float x) {         // order-preserving float -> uint
+    const uint32_t b = __float_as_uint(x);
+    return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(uint32_t o) {
+    return __uint_as_float(o ^ (((o >> 31) - 1u) | 0x80000000u));
+}
+__device__ __forceinline__ float warp_min_f(float v) { return ord2f(__reduce_min_sync(SPH_FULL_MASK, f2ord(v))); }
+__device__ __forceinline__ float warp_max_f(float v) { return ord2f(__reduce_max_sync(SPH_FULL_MASK, f2ord(v))); }
+
+// minimum-image shift of a batch on one axis from its code: d = fl(x_i - x_j) - shift (R7)
+__device__ __forceinline__ float img_shift(uint32_t code, int axis, float L) {
+    const uint32_t c = (code >> (2 * axis)) & 3u;
+    return c == 1u ? -L : (c == 2u ? L : 0.0f);
+}
+
+// D = A (16 x 8, tf32, row) * B (8 x 8, tf32, col), fp32 accumulators starting from zero
+__device__ __forceinline__ void mma_tf32_16x8x8(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
+        : "=f"(c[0]), "=f"(c[1]), "=f"(c[2]), "=f"(c[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1), "f"(0.0f));
 }
 
 // Walks every candidate run of the warp's 32 particles.  `drain()` is called (warp-uniformly, from ONE site)
 // whenever the mask store holds TILE_MMAX batches, and once at the end; it must consume the masks and call
-// st.reset().  All 32 lanes must call this.
-//   row = cell / nc0 (the stencil row of the particle), sub = cell % nc0 (its x sub-cell), -1 / 0 for lanes
-//   past the end of the sorted order.
-// Structure: for every GROUP of lanes (below) the 3^(d-1) x 3 candidate runs (stencil row x {inside the box,
-// image across the low x seam, image across the high x seam}) are looked up by 27 lanes in parallel and
-// written to a small table; one flat loop then streams the runs batch by batch.
+// st.reset().  All 32 lanes must call this.   in: the lane holds a particle; active: it is a destination of this
+// launch; pi = (x, y, z, h); ci = its cell id (level base + linear cell).
 template <int DIM, bool VARH, class Drain>
 __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& pc,
-                                          const float4* __restrict__ posh, const uint32_t* __restrict__ cell_start,
-                                          bool active, float4 pi, int row, int sub,
+                                          const float4* posh, const uint32_t* __restrict__ cell_start,
+                                          bool active, bool in, float4 pi, uint32_t ci,
                                           TileWarpSmem& ws, TileState& st, Drain&& drain) {
-    const int lane = threadIdx.x & 31;
-    const int nc0 = g.nc[0], nc1 = g.nc[1], nc2 = g.nc[2], na = g.na, xsub = g.xsub;
-    const float2 xi = f2(pi.x, pi.x), yi = f2(pi.y, pi.y), zi = f2(pi.z, pi.z);
-    const float2 kh2 = f2(pc.kh, pc.kh), hi2 = f2(pi.w, pi.w);
-    const float cc = pair_cut2(pc.kh, pc.h_const, pc.h_const);
-    const float2 cut2c = f2(cc, cc);
-    constexpr int NSEG = (DIM == 3 ? 27 : 9);
+    const int lane = threadIdx.x & 31, gq = lane >> 2, tq = lane & 3;
+    const int na = g.na, nlev = VARH ? g.nlev : 1;
+    const float khsq = pc.kh * pc.kh;
+    const float cut2c = pair_cut2(pc.kh, pc.h_const, pc.h_const);
 
-    // groups: maximal lane ranges of one stencil row without an x gap wider than two coarse cells (a wider
-    // gap means the windows of its two sides are disjoint, so splitting there saves tests)
+    // own cell -> (level, stencil row, x sub-cell); groups: maximal lane ranges of one level and row without an x
+    // gap wider than two coarse cells (a wider gap means the windows of its two sides are disjoint)
+    int lvl = 0;
+    if (VARH) { while (lvl + 1 < nlev && ci >= g.lev[lvl + 1].base) ++lvl; }
+    const uint32_t rel = ci - g.lev[lvl].base;
+    const uint32_t nc0_own = (uint32_t)g.lev[lvl].nc[0];
+    int row = in ? (int)(rel / nc0_own) : -1;
+    const int sub = in ? (int)(rel % nc0_own) : 0;
+    const int gap = 2 * g.lev[lvl].xsub;
+    if (VARH) row = in ? row * SPH_MAX_LEVELS + lvl : -1;                 // rows of different levels never compare equal
     const int prow = __shfl_up_sync(SPH_FULL_MASK, row, 1), psub = __shfl_up_sync(SPH_FULL_MASK, sub, 1);
-    const bool brk = lane == 0 || row != prow || sub - psub > 2 * xsub;
+    const bool brk = lane == 0 || row != prow || sub - psub > gap;
     const unsigned brkmask = __ballot_sync(SPH_FULL_MASK, brk);
     unsigned remaining = __ballot_sync(SPH_FULL_MASK, active);
 
-    bool ing = false, done = false, seg_shift = false;
-    int seg = NSEG;                                   // forces the first group set-up
-    uint32_t b0 = 0u, e = 0u;
-    unsigned segs = 0u;                               // non-empty runs of the current group still to stream
-    float2 sx = f2(0.0f, 0.0f), sy = sx, sz = sx;
+    // per-thread constants of the mask transpose and of the B-operand fetch
+    const uint32_t selA = ((uint32_t)tq << (4 * tq)) | ((uint32_t)(4 + tq) << (4 * (tq ^ 1)));
+    const uint32_t selB = ((uint32_t)tq << (4 * (tq ^ 2))) | ((uint32_t)(4 + tq) << (4 * (tq ^ 3)));
+    const uint32_t selC = ((uint32_t)tq << (4 * tq)) | ((uint32_t)(tq ^ 1) << (4 * (tq ^ 1))) |
+                          ((uint32_t)(4 + (tq ^ 2)) << (4 * (tq ^ 2))) | ((uint32_t)(4 + (tq ^ 3)) << (4 * (tq ^ 3)));
+    const int cidx = 8 * (gq >> 1) + 7 - (gq & 1);           // column g of N-tile nt holds staged candidate cidx - 2 nt
 
-    while (!done) {
-        while (st.M < TILE_MMAX) {
-            if (b0 >= e) {
-                if (++seg >= NSEG) {                  // next group
-                    if (!remaining) { done = true; break; }
-                    const int leader = __ffs(remaining) - 1;
-                    const int gs = 31 - __clz(brkmask & (0xffffffffu >> (31 - leader)));      // start of the leader's range
-                    const unsigned above = leader < 31 ? (brkmask & (0xffffffffu << (leader + 1))) : 0u;
-                    const int ge = above ? __ffs(above) - 1 : 32;                               // one past its end
-                    const unsigned range = (ge == 32 ? 0xffffffffu : ((1u << ge) - 1u)) & (0xffffffffu << gs);
-                    const unsigned gmask = remaining & range;
-                    remaining &= ~gmask;
-                    ing = (gmask >> lane) & 1u;
-                    const int first = __ffs(gmask) - 1, last = 31 - __clz(gmask);
-                    const int grow = __shfl_sync(SPH_FULL_MASK, row, first);
-                    const int sub_lo = __shfl_sync(SPH_FULL_MASK, sub, first), sub_hi = __shfl_sync(SPH_FULL_MASK, sub, last);
-                    const int cy = grow % nc1, cz = grow / nc1;
-                    // x reach in sub-cells: a pair of the group is closer than R = k (h_group_max + h_max) / 2, so
-                    // its sub-cell indices differ by at most floor(R / sub-cell) + 1 (<= xsub: cell >= k h_max)
-                    int nx = xsub;
-                    if (VARH) {
-                        const float hg = __uint_as_float(__reduce_max_sync(SPH_FULL_MASK, ing ? __float_as_uint(pi.w) : 0u));
-                        const float R = pc.kh * (hg + pc.h_const) * 1.0001f;
-                        nx = min(xsub, __float2int_rd(R * g.inv_cell[0]) + 1);
-                    }
-                    const int a = sub_lo - nx, b = sub_hi + nx;
-                    __syncwarp();
-                    bool nonempty = false;
-                    if (lane < NSEG) {                // lane = 9 (oz+1) + 3 (oy+1) + part
-                        const int part = lane % 3, oy = (lane / 3) % 3 - 1, oz = DIM == 3 ? lane / 9 - 1 : 0;
-                        int y2 = cy + oy, z2 = cz + oz; uint32_t code = 0u; bool ok = true;
-                        if (y2 < 0)         { if (g.per[1]) { y2 += nc1; code |= 1u << 2; } else ok = false; }
-                        else if (y2 >= nc1) { if (g.per[1]) { y2 -= nc1; code |= 2u << 2; } else ok = false; }
-                        if (z2 < 0)         { if (g.per[2]) { z2 += nc2; code |= 1u << 4; } else ok = false; }
-                        else if (z2 >= nc2) { if (g.per[2]) { z2 -= nc2; code |= 2u << 4; } else ok = false; }
-                        int c0, c1;
-                        if (part == 0)      { c0 = max(a, 0); c1 = min(b, nc0 - 1); }
-                        else if (part == 1) { c0 = a + nc0; c1 = nc0 - 1; code |= 1u; ok = ok && g.per[0] && a < 0; }
-                        else                { c0 = 0; c1 = b - nc0; code |= 2u; ok = ok && g.per[0] && b >= nc0; }
-                        uint32_t s_ = 0u, e_ = 0u;
-                        if (ok) {
-                            const uint32_t rowbase = (uint32_t)((z2 * nc1 + y2) * nc0);
-                            s_ = __ldg(cell_start + (size_t)(rowbase + (uint32_t)c0) * na);
-                            e_ = __ldg(cell_start + (size_t)(rowbase + (uint32_t)c1 + 1u) * na);
-                        }
-                        ws.seg_s[lane] = s_; ws.seg_e[lane] = e_; ws.seg_c[lane] = code;
-                        nonempty = s_ < e_;
-                    }
-                    segs = __ballot_sync(SPH_FULL_MASK, nonempty);      // runs that hold candidates
-                    __syncwarp();
-                    seg = -1; b0 = e = 0u;
-                    continue;
+    // ---- group state (warp-uniform unless noted)
+    bool grp = false, ing = false /* per lane */;
+    float xmin = 0, xmax = 0, ymin = 0, ymax = 0, zmin = 0, zmax = 0, hg = pc.h_const, ox = 0, oy = 0, oz = 0, exm = 0;
+    uint32_t A0[4] = {0, 0, 0, 0}, A1[4] = {0, 0, 0, 0};      // per lane: A operands (rows of the quad's four particles)
+    // ---- level state
+    int b = 0, pass = 0, npass = 0, entries = 0, nparts = 1, ny = 1, x0 = 0, x1 = 0, y0 = 0, z0 = 0;
+    bool lowpart = false, highpart = false;
+    float margin = 0.0f, inv_ny = 1.0f;
+    // ---- run / batch state
+    unsigned segs = 0u;
+    bool have = false;
+    uint32_t nb0 = 0u, ne = 0u, ncode = 0u;
+    float4 pjn = make_float4(0, 0, 0, 0);
+
+    auto load_batch = [&](uint32_t bb, uint32_t ee) -> float4 {
+        const uint32_t j = bb + (uint32_t)lane;
+        return j < ee ? ld_state(posh + j) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    };
+    auto pop_run = [&]() -> bool {
+        if (!segs) return false;
+        const int k = __ffs(segs) - 1; segs &= segs - 1u;
+        nb0 = ws.seg_s[k]; ne = ws.seg_e[k]; ncode = ws.seg_c[k];
+        return true;
+    };
+
+    auto setup_group = [&]() {
+        const int leader = __ffs(remaining) - 1;
+        const int gs = 31 - __clz(brkmask & (0xffffffffu >> (31 - leader)));      // start of the leader's range
+        const unsigned above = leader < 31 ? (brkmask & (0xffffffffu << (leader + 1))) : 0u;
+        const int ge = above ? __ffs(above) - 1 : 32;                               // one past its end
+        const unsigned range = (ge == 32 ? 0xffffffffu : ((1u << ge) - 1u)) & (0xffffffffu << gs);
+        const unsigned gmask = remaining & range;
+        remaining &= ~gmask;
+        ing = (gmask >> lane) & 1u;
+        const float big = 3.0e38f;
+        xmin = warp_min_f(ing ? pi.x : big); xmax = warp_max_f(ing ? pi.x : -big);
+        ymin = warp_min_f(ing ? pi.y : big); ymax = warp_max_f(ing ? pi.y : -big);
+        if (DIM == 3) { zmin = warp_min_f(ing ? pi.z : big); zmax = warp_max_f(ing ? pi.z : -big); }
+        if (VARH) hg = __uint_as_float(__reduce_max_sync(SPH_FULL_MASK, ing ? __float_as_uint(pi.w) : 0u));
+        ox = 0.5f * (xmin + xmax); oy = 0.5f * (ymin + ymax); oz = DIM == 3 ? 0.5f * (zmin + zmax) : 0.0f;
+        exm = 0.5f * fmaxf(fmaxf(xmax - xmin, ymax - ymin), DIM == 3 ? zmax - zmin : 0.0f);
+        // A operands of this lane's particle: [-2x, -2y, -2z, -2 kh^2 h, n_hi, n_lo, 1, 1], n = |x|^2 - kh^2 h^2
+        const float xt = tf32r(pi.x - ox), yt = tf32r(pi.y - oy), zt = DIM == 3 ? tf32r(pi.z - oz) : 0.0f;
+        const float ht = VARH ? tf32r(pi.w) : 0.0f;
+        const float n = fmaf(zt, zt, fmaf(yt, yt, xt * xt)) - khsq * ht * ht;
+        const float nh = tf32r(n), nl = tf32r(n - nh);
+        __syncwarp();                                          // G (aliased) is no longer read
+        float* af = ws.Af + lane * 9;
+        af[0] = -2.0f * xt; af[1] = -2.0f * yt; af[2] = -2.0f * zt; af[3] = tf32r(-2.0f * khsq * ht);
+        af[4] = nh; af[5] = nl; af[6] = 1.0f; af[7] = 1.0f;
+        __syncwarp();
+        const float* q = ws.Af + (4 * gq) * 9 + tq;             // rows of the quad's particles 0..3, features tq and tq + 4
+        A0[0] = __float_as_uint(q[0]);      A0[1] = __float_as_uint(q[9]);       A0[2] = __float_as_uint(q[4]);      A0[3] = __float_as_uint(q[13]);
+        A1[0] = __float_as_uint(q[18]);     A1[1] = __float_as_uint(q[27]);      A1[2] = __float_as_uint(q[22]);     A1[3] = __float_as_uint(q[31]);
+        __syncwarp();
+    };
+
+    // candidate cells of level b: the level's cells that meet the group's bounding box grown by the reach R
+    auto setup_level = [&]() {
+        const LevelDesc& Lv = g.lev[b];
+        const float R = pc.kh * (hg + (VARH ? Lv.hmax : pc.h_const)) * 1.0001f + 16.0f * g.uabs;
+        const float X = exm + R;                               // bound of every tile-local coordinate that matters
+        margin = (R * X + R * R) * (1.0f / 128.0f) + X * X * (1.0f / 32768.0f) + 64.0f * g.uabs * (R + X);
+        const int n0 = Lv.nc[0], n1 = Lv.nc[1], n2 = Lv.nc[2];
+        const float e0 = 1.0e-3f + 4.8e-7f * (float)n0, e1 = 1.0e-3f + 4.8e-7f * (float)n1, e2 = 1.0e-3f + 4.8e-7f * (float)n2;
+        x0 = __float2int_rd((xmin - R - g.lo[0]) * Lv.inv_cell[0] - e0); x1 = __float2int_rd((xmax + R - g.lo[0]) * Lv.inv_cell[0] + e0);
+        y0 = __float2int_rd((ymin - R - g.lo[1]) * Lv.inv_cell[1] - e1);
+        int y1 = __float2int_rd((ymax + R - g.lo[1]) * Lv.inv_cell[1] + e1);
+        int z1 = 0; z0 = 0;
+        if (DIM == 3) { z0 = __float2int_rd((zmin - R - g.lo[2]) * Lv.inv_cell[2] - e2); z1 = __float2int_rd((zmax + R - g.lo[2]) * Lv.inv_cell[2] + e2); }
+        if (!g.per[0]) { x0 = max(x0, 0); x1 = min(x1, n0 - 1); } else { x0 = max(x0, -n0); x1 = min(x1, 2 * n0 - 1); }
+        if (!g.per[1]) { y0 = max(y0, 0); y1 = min(y1, n1 - 1); } else { y0 = max(y0, -n1); y1 = min(y1, 2 * n1 - 1); }
+        if (DIM == 3) { if (!g.per[2]) { z0 = max(z0, 0); z1 = min(z1, n2 - 1); } else { z0 = max(z0, -n2); z1 = min(z1, 2 * n2 - 1); } }
+        lowpart = g.per[0] && x0 < 0; highpart = g.per[0] && x1 >= n0;
+        nparts = 1 + (lowpart ? 1 : 0) + (highpart ? 1 : 0);
+        ny = y1 - y0 + 1;
+        const int nzr = z1 - z0 + 1;
+        entries = (ny > 0 && nzr > 0 && x1 >= x0) ? ny * nzr * nparts : 0;
+        npass = (entries + 31) >> 5;
+        inv_ny = 1.0f / (float)max(ny, 1);
+    };
+
+    // 32 lanes look up 32 (row, x part) entries of the current level: [s, e) of the sorted order + shift code
+    auto setup_pass = [&]() {
+        const LevelDesc& Lv = g.lev[b];
+        const int n0 = Lv.nc[0], n1 = Lv.nc[1], n2 = Lv.nc[2];
+        const int ent = pass * 32 + lane;
+        bool nonempty = false;
+        uint32_t s_ = 0u, e_ = 0u, code = 0u;
+        if (ent < entries) {
+            int r = ent, part = 0;
+            if (nparts == 2) { r = ent >> 1; part = ent & 1; } else if (nparts == 3) { r = ent / 3; part = ent - 3 * r; }
+            const int kind = part == 0 ? 0 : (part == 1 ? (lowpart ? 1 : 2) : 2);
+            const int rz = (int)(((float)r + 0.5f) * inv_ny);
+            int iy = y0 + (r - rz * ny), iz = z0 + rz;
+            if (iy < 0) { iy += n1; code |= 1u << 2; } else if (iy >= n1) { iy -= n1; code |= 2u << 2; }
+            if (iz < 0) { iz += n2; code |= 1u << 4; } else if (iz >= n2) { iz -= n2; code |= 2u << 4; }
+            int c0, c1;
+            if (kind == 0)      { c0 = max(x0, 0); c1 = min(x1, n0 - 1); }
+            else if (kind == 1) { c0 = max(x0 + n0, 0); c1 = n0 - 1; code |= 1u; }
+            else                { c0 = 0; c1 = min(x1 - n0, n0 - 1); code |= 2u; }
+            const uint32_t rowbase = Lv.base + (uint32_t)((iz * n1 + iy) * n0);
+            s_ = __ldg(cell_start + (size_t)(rowbase + (uint32_t)c0) * na);
+            e_ = __ldg(cell_start + (size_t)(rowbase + (uint32_t)c1 + 1u) * na);
+            nonempty = s_ < e_;
+        }
+        __syncwarp();
+        ws.seg_s[lane] = s_; ws.seg_e[lane] = e_; ws.seg_c[lane] = code;
+        segs = __ballot_sync(SPH_FULL_MASK, nonempty);          // runs that hold candidates
+        __syncwarp();
+    };
+
+    // one batch of <= 32 candidates [cb0, min(cb0 + 32, ce)) against the warp's 32 particles
+    auto process = [&](uint32_t cb0, uint32_t ce, uint32_t ccode, float4 pj) {
+        const bool valid = cb0 + (uint32_t)lane < ce;
+        float xr = pj.x, yr = pj.y, zr = pj.z;
+        if (ccode) {                                            // the image of the candidate next to the group: x_j + shift
+            xr += img_shift(ccode, 0, g.L[0]); yr += img_shift(ccode, 1, g.L[1]);
+            if (DIM == 3) zr += img_shift(ccode, 2, g.L[2]);
+            st.shifted = true;
+        }
+        const float xt = tf32r(xr - ox), yt = tf32r(yr - oy), zt = DIM == 3 ? tf32r(zr - oz) : 0.0f;
+        const float ht = VARH ? tf32r(pj.w) : 0.0f;
+        float n = fmaf(zt, zt, fmaf(yt, yt, xt * xt)) - (VARH ? khsq * ht * ht : cut2c) - margin;
+        n = valid ? n : 1.0e30f;                                // padding never passes
+        const float nh = tf32r(n), nl = tf32r(n - nh);
+        __syncwarp();                                           // readers of the previous batch are done
+        ws.G[0][lane] = make_float2(xt, 1.0f); ws.G[1][lane] = make_float2(yt, 1.0f);
+        ws.G[2][lane] = make_float2(zt, nh);   ws.G[3][lane] = make_float2(ht, nl);
+        __syncwarp();
+        uint32_t pm0 = 0u, pm1 = 0u, pm2 = 0u, pm3 = 0u;        // sign bits of the quad's particles 0..3 (this thread's columns)
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) {
+            const float2 bf = ws.G[tq][cidx - 2 * nt];
+            float c0[4], c1[4];
+            mma_tf32_16x8x8(c0, A0, __float_as_uint(bf.x), __float_as_uint(bf.y));
+            mma_tf32_16x8x8(c1, A1, __float_as_uint(bf.x), __float_as_uint(bf.y));
+            pm0 = __funnelshift_l(__float_as_uint(c0[0]), pm0, 1); pm0 = __funnelshift_l(__float_as_uint(c0[1]), pm0, 1);
+            pm1 = __funnelshift_l(__float_as_uint(c0[2]), pm1, 1); pm1 = __funnelshift_l(__float_as_uint(c0[3]), pm1, 1);
+            pm2 = __funnelshift_l(__float_as_uint(c1[0]), pm2, 1); pm2 = __funnelshift_l(__float_as_uint(c1[1]), pm2, 1);
+            pm3 = __funnelshift_l(__float_as_uint(c1[2]), pm3, 1); pm3 = __funnelshift_l(__float_as_uint(c1[3]), pm3, 1);
+        }
+        // byte q of P: this thread's 8 columns against particle q of the quad; transpose the 4 x 4 bytes of the quad
+        const uint32_t P = __byte_perm(__byte_perm(pm0, pm1, 0x0040), __byte_perm(pm2, pm3, 0x0040), 0x5410);
+        const uint32_t s1 = __shfl_xor_sync(SPH_FULL_MASK, P, 1), s2 = __shfl_xor_sync(SPH_FULL_MASK, P, 2),
+                       s3 = __shfl_xor_sync(SPH_FULL_MASK, P, 3);
+        uint32_t mask = __byte_perm(__byte_perm(P, s1, selA), __byte_perm(s2, s3, selB), selC);
+        if (!ing) mask = 0u;
+        ws.mask[st.M][lane] = mask;
+        if (mask) st.nz |= 1u << st.M;
+        if (lane == 0) { ws.base[st.M] = cb0; ws.bcode[st.M] = ccode; }
+        if (ing) st.tests += (unsigned)min(32u, ce - cb0);
+        ++st.M;
+    };
+
+    // streams batches until the mask store is full (true) or every group is done (false)
+    auto fill = [&]() -> bool {
+        for (;;) {
+            if (st.M >= TILE_MMAX) return true;
+            if (!have) {
+                if (pop_run()) { pjn = load_batch(nb0, ne); have = true; continue; }
+                if (grp) {
+                    if (++pass < npass) { setup_pass(); continue; }
+                    if (++b < nlev) { setup_level(); pass = -1; continue; }
+                    grp = false;
                 }
-                if (segs == 0u) { seg = NSEG; b0 = e = 0u; continue; }   // group done
-                seg = __ffs(segs) - 1; segs &= segs - 1u;
-                b0 = ws.seg_s[seg]; e = ws.seg_e[seg];
-                const uint32_t code = ws.seg_c[seg];      // image shifts: 1 -> -L (wrapped below), 2 -> +L (wrapped above)
-                seg_shift = code != 0u;
-                const float fx = (code & 3u) == 1u ? -g.L[0] : ((code & 3u) == 2u ? g.L[0] : 0.0f);
-                const float fy = ((code >> 2) & 3u) == 1u ? -g.L[1] : (((code >> 2) & 3u) == 2u ? g.L[1] : 0.0f);
-                const float fz = ((code >> 4) & 3u) == 1u ? -g.L[2] : (((code >> 4) & 3u) == 2u ? g.L[2] : 0.0f);
-                sx = f2(fx, fx); sy = f2(fy, fy); sz = f2(fz, fz);
+                if (!remaining) return false;
+                setup_group(); grp = true; b = -1; npass = 0; pass = 0;
                 continue;
             }
-            // one batch of <= 32 candidates [b0, min(b0 + 32, e))
-            const uint32_t j = b0 + (uint32_t)lane;
-            float4 pj = make_float4(3.0e38f, 0.0f, 0.0f, 0.0f);           // padding: r2 = inf, never a hit
-            if (j < e) pj = __ldg(posh + j);
-            __syncwarp();                                                  // readers of the previous batch are done
-            ws.x[lane] = pj.x; ws.y[lane] = pj.y;
-            if (DIM == 3) ws.z[lane] = pj.z;
-            if (VARH) ws.h[lane] = pj.w;
-            __syncwarp();
-            const int len = (int)min(32u, e - b0);
-            const int n8 = (len + 7) >> 3;                                // 8 candidates per branch-free step
-            uint32_t mask = 0;
-            if (seg_shift) {
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (u < n8) {
-                        const uint32_t m0 = tile_test4<DIM, VARH, true>(ws, 8 * u, xi, yi, zi, sx, sy, sz, cut2c, kh2, hi2);
-                        const uint32_t m1 = tile_test4<DIM, VARH, true>(ws, 8 * u + 4, xi, yi, zi, sx, sy, sz, cut2c, kh2, hi2);
-                        mask |= (m0 << (8 * u)) | (m1 << (8 * u + 4));
-                    }
-                st.shifted = true;
-            } else {
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (u < n8) {
-                        const uint32_t m0 = tile_test4<DIM, VARH, false>(ws, 8 * u, xi, yi, zi, sx, sy, sz, cut2c, kh2, hi2);
-                        const uint32_t m1 = tile_test4<DIM, VARH, false>(ws, 8 * u + 4, xi, yi, zi, sx, sy, sz, cut2c, kh2, hi2);
-                        mask |= (m0 << (8 * u)) | (m1 << (8 * u + 4));
-                    }
-            }
-            if (!ing) mask = 0u;
-            ws.mask[st.M][lane] = mask;
-            if (mask) st.nz |= 1u << st.M;
-            if (lane == 0) ws.base[st.M] = b0;
-            if (ing) st.tests += (unsigned)len;
-            st.hits += (unsigned)__popc(mask);
-            ++st.M;
-            b0 += 32u;
+            const uint32_t cb0 = nb0, ce = ne, ccode = ncode;
+            const float4 pj = pjn;
+            if (nb0 + 32u < ne) { nb0 += 32u; pjn = load_batch(nb0, ne); }     // prefetch the next batch
+            else if (pop_run()) pjn = load_batch(nb0, ne);
+            else have = false;
+            process(cb0, ce, ccode, pj);
         }
-        drain();                                                           // consumes the masks, resets st
+    };
+
+    for (;;) {
+        const bool more = fill();
+        drain();                                                // consumes the masks, resets st
+        if (!more) break;
     }
 }
 
-// Every lane pops its own hits of the stored batches in order (nz: the lane's non-empty masks) and evaluates
-// them.  Branch-free and software-pipelined: DEPTH hits are in flight, the source data of a later hit is
-// gathered (Src = load(sorted index)) before the current one is computed, so the gather latency (L2: the sorted
-// state does not fit L1) overlaps the arithmetic.  A lane that has run out keeps executing with has = false and
-// the harmless index `idle` (its own particle) until the slowest lane of the warp is done; compute(src, has)
-// must contribute nothing when has is false.
-template <class Src, int DEPTH = 2, class Load, class Compute>
+// Every lane pops its own candidates of the stored batches in order (nz: the lane's non-empty masks) and evaluates
+// them.  Branch-free and software-pipelined: DEPTH candidates are in flight, the source data of a later one is
+// gathered (Src = load(sorted index)) before the current one is computed, so the gather latency overlaps the
+// arithmetic.  A lane that has run out keeps executing with has = false and the harmless index `idle` (its own
+// particle) until the slowest lane of the warp is done; compute(src, has, code, per) must apply the exact
+// predicate and contribute nothing when it fails or has is false.  PER: some batch is a periodic image (code != 0).
+template <class Src, int DEPTH, bool PER, class Load, class Compute>
 __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
     const int lane = threadIdx.x & 31;
     __syncwarp();
-    uint32_t cur = 0u, b = 0u;
-    auto pop = [&](bool& has) -> uint32_t {
+    uint32_t cur = 0u, b = 0u, code = 0u;
+    auto pop = [&](bool& has, uint32_t& cd) -> uint32_t {
         const bool refill = cur == 0u && nz != 0u;
         const int m = max(__ffs(nz) - 1, 0);
         const uint32_t nm = ws.mask[m][lane], nb = ws.base[m];
         cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? (nz & (nz - 1u)) : nz;
+        if (PER) { const uint32_t nc = ws.bcode[m]; code = refill ? nc : code; }
         has = cur != 0u;
         const uint32_t j = has ? b + (uint32_t)(__ffs(cur) - 1) : idle;
         cur &= cur - 1u;                        // stays 0 when it is 0
+        cd = code;
         return j;
     };
-    Src R[DEPTH]; bool H[DEPTH];                    // DEPTH hits in flight; fully unrolled, so R and H live in registers
+    Src R[DEPTH]; bool H[DEPTH]; uint32_t C[DEPTH];   // fully unrolled, so these live in registers
 #pragma unroll
-    for (int d = 0; d + 1 < DEPTH; ++d) R[d] = load(pop(H[d]));
+    for (int d = 0; d + 1 < DEPTH; ++d) R[d] = load(pop(H[d], C[d]));
     for (;;) {
 #pragma unroll
         for (int d = 0; d < DEPTH; ++d) {
             const int nx = (d + DEPTH - 1) % DEPTH;
-            R[nx] = load(pop(H[nx]));               // gather for a later hit ...
-            compute(R[d], H[d]);                    // ... while this one is evaluated
+            R[nx] = load(pop(H[nx], C[nx]));        // gather for a later candidate ...
+            compute(R[d], H[d], C[d], std::integral_constant<bool, PER>{});   // ... while this one is evaluated
         }
-        if (!__any_sync(SPH_FULL_MASK, H[0])) break;   // pops are in order: no pending hit 0 means no pending hit at all
+        if (!__any_sync(SPH_FULL_MASK, H[0])) break;   // pops are in order: no pending candidate 0 means none at all
     }
     __syncwarp();
 }
 
 // ---- mask records (recorded by the density pass, replayed by the acceleration pass) -----------------------
 // The pool is an array of ROWS of 32 words.  A warp appends BLOCKS: a header row {next block (row index, 0 =
-// end), number of batches M <= TILE_MMAX | 0x100 if a batch came from a periodic image, base[0..M-1]} followed
-// by M rows of masks (word = lane).  head[warp] = SPH_NL_NONE marks a warp whose masks did not fit the pool.
+// end), number of batches M <= TILE_MMAX | 0x100 if a batch came from a periodic image, base[0..M-1]}, then -- only
+// when that flag is set -- one row of shift codes (word = batch), then M rows of masks (word = lane).
+// head[warp] = SPH_NL_NONE marks a warp whose masks did not fit the pool.
 struct TileRecorder {
     NList nl; uint32_t prev_hdr; bool ok;
     __device__ __forceinline__ void init(const NList& n) { nl = n; prev_hdr = 0u; ok = n.pool != nullptr; }
     __device__ __forceinline__ void append(const TileWarpSmem& ws, int M, bool shifted, int warp_id, unsigned long long* counters) {
         if (!ok || M <= 0) return;
         const int lane = threadIdx.x & 31;
+        const uint32_t rows = (uint32_t)M + 1u + (shifted ? 1u : 0u);
         uint32_t blk = 0;
-        if (lane == 0) blk = atomicAdd(nl.used, (uint32_t)M + 1u) + 1u;
+        if (lane == 0) blk = atomicAdd(nl.used, rows) + 1u;
         blk = __shfl_sync(SPH_FULL_MASK, blk, 0);
-        if ((unsigned long long)blk + (unsigned)M + 1ull > (unsigned long long)nl.pool_rows) {
+        if ((unsigned long long)blk + rows > (unsigned long long)nl.pool_rows) {
             ok = false;                         // the warp's record is incomplete: the replaying pass searches again
             if (lane == 0) { nl.head[warp_id] = SPH_NL_NONE; atomicAdd(&counters[CNT_OVERFLOW], 1ull); }
             return;
@@ -290,15 +380,17 @@ struct TileRecorder {
         __syncwarp();
         uint32_t* hdr = nl.pool + (size_t)blk * 32;
         hdr[lane] = lane == 0 ? 0u : (lane == 1 ? ((uint32_t)M | (shifted ? 0x100u : 0u)) : ws.base[lane - 2]);
-        for (int m = 0; m < M; ++m) __stcs(hdr + (size_t)(m + 1) * 32 + lane, ws.mask[m][lane]);   // streaming: keep the state in L2
+        uint32_t* rows0 = hdr + 32;
+        if (shifted) { rows0[lane] = ws.bcode[lane]; rows0 += 32; }
+        for (int m = 0; m < M; ++m) __stcs(rows0 + (size_t)m * 32 + lane, ws.mask[m][lane]);   // streaming: keep the state in L2
         if (lane == 0) { if (prev_hdr) nl.pool[(size_t)prev_hdr * 32] = blk; else nl.head[warp_id] = blk; }
         prev_hdr = blk;
     }
 };
 
-// drain(nz, shifted) is called once per recorded block with the masks and bases in ws
+// drain(nz, shifted) is called once per recorded block with the masks, bases and shift codes in ws
 template <class Drain>
-__device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileWarpSmem& ws, bool active, unsigned long long& hits, Drain&& drain) {
+__device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileWarpSmem& ws, bool active, Drain&& drain) {
     const int lane = threadIdx.x & 31;
     while (blk) {
         const uint32_t* hdr = nl.pool + (size_t)blk * 32;
@@ -306,17 +398,20 @@ __device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileW
         const uint32_t next = __shfl_sync(SPH_FULL_MASK, hw, 0);
         const uint32_t w1 = __shfl_sync(SPH_FULL_MASK, hw, 1);
         const int M = (int)(w1 & 0xffu);
+        const bool shifted = (w1 & 0x100u) != 0u;
+        const uint32_t* rows0 = hdr + 32;
         __syncwarp();
         if (lane >= 2) ws.base[lane - 2] = hw;
+        if (shifted) { ws.bcode[lane] = __ldcs(rows0 + lane); rows0 += 32; }
         uint32_t nz = 0u;
         for (int m0 = 0; m0 < M; m0 += 8) {                              // 8 independent loads in flight
             uint32_t w[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) w[k] = (m0 + k < M && active) ? __ldcs(hdr + (size_t)(m0 + k + 1) * 32 + lane) : 0u;   // a lane that is no destination of this pass drops its masks
+            for (int k = 0; k < 8; ++k) w[k] = (m0 + k < M && active) ? __ldcs(rows0 + (size_t)(m0 + k) * 32 + lane) : 0u;   // a lane that is no destination of this pass drops its masks
 #pragma unroll
-            for (int k = 0; k < 8; ++k) if (m0 + k < M) { ws.mask[m0 + k][lane] = w[k]; if (w[k]) nz |= 1u << (m0 + k); hits += (unsigned)__popc(w[k]); }
+            for (int k = 0; k < 8; ++k) if (m0 + k < M) { ws.mask[m0 + k][lane] = w[k]; if (w[k]) nz |= 1u << (m0 + k); }
         }
-        drain(nz, (w1 & 0x100u) != 0u);
+        drain(nz, shifted);
         blk = next;
     }
 }
@@ -325,7 +420,3 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(SPH_FULL_MASK, v, o);
     return v;
 }
-
-// Minimum image for the FIELD arithmetic of phase 2 (any accurate image will do there; the set membership was
-// decided bit-exactly in phase 1).  For a true neighbour |d_min| < L/3, so rint picks the same image as R7.
-__device__ __forceinline__ float min_image(float d, float L, float invL) { return fmaf(-rintf(d * invL), L, d); }

@@ -33,7 +33,7 @@ def test_header_symbols_are_exported(lib):
     for n in names:
         assert hasattr(lib, n), f"{n} declared in sph.h but not exported"
     assert sorted(binding.EXPORTS) == names
-    assert lib.sph_abi_version() == 4
+    assert lib.sph_abi_version() == 5
 
 
 def test_struct_layouts_match_the_c_compiler(tmp_path):
