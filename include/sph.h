@@ -127,17 +127,18 @@ typedef struct sph_stats {
     int64_t pairs_density;      /* (i,j) pairs passing the exact predicate in the last density pass(es), self pairs included */
     int64_t pairs_accel;        /* same for the last acceleration pass(es) */
     int64_t candidates;         /* candidates streamed through the filter in the last density + acceleration passes */
-    int64_t candidates_density, candidates_accel;
+    int64_t candidates_density, candidates_accel;   /* ... by pair passes that searched themselves (no record pool) */
     int64_t kernel_launches;    /* CUDA kernels launched by this context since sph_create */
     int64_t steps_done;         /* predictor-corrector steps since the last sph_nnps_build */
     int32_t variable_h;         /* 1 if h_min != h_max at the last build */
     float h_max;
     int32_t xsub;               /* x sub-cells per support radius of the current grid (n_cells[0] counts sub-cells) */
-    int32_t used_rows;          /* 1 if the last acceleration pass replayed the hit masks recorded by the density pass */
+    int32_t used_rows;          /* 1 if the last acceleration pass replayed the candidate masks recorded by the search */
     int64_t nlist_rows_used, nlist_rows_capacity;   /* record pool occupancy after the last recording pass */
     int64_t nlist_fallback_warps;                   /* warps whose masks did not fit the pool in that pass (they search again) */
     int32_t n_levels;           /* h classes / level grids of the current build (1 when h is constant) */
     int64_t n_keys;             /* entries of the shared cell table (all levels x arrays) */
+    int64_t candidates_search;  /* candidates streamed through the filter by the last search (one per sorted order) */
 } sph_stats;
 
 /* Per-kernel device timing (CUDA events on the context stream around every launch), for the roofline report. */
@@ -151,7 +152,9 @@ enum sph_kernel_id {
     SPH_K_ACCEL = 6,            /* a6 + a7: momentum (+ continuity) pair loop                     */
     SPH_K_OUTPUT = 7,           /* caller-order output gather                                     */
     SPH_K_NEIGHBORS = 8,        /* verification export                                            */
-    SPH_K_ACCEL_LIST = 9,       /* a6 + a7 replayed over the hit masks recorded by a4              */
+    SPH_K_ACCEL_LIST = 9,       /* a6 + a7 replayed over the candidate masks recorded by the search */
+    SPH_K_SEARCH = 10,          /* neighbour search of one sorted order: tensor-core filter -> mask records */
+    SPH_K_DENSITY_LIST = 11,    /* a4 + a5 replayed over the candidate masks recorded by the search */
     SPH_K_COUNT = 16
 };
 typedef struct sph_profile {

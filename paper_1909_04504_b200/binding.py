@@ -56,7 +56,8 @@ class sph_stats(C.Structure):
                 ("kernel_launches", C.c_int64), ("steps_done", C.c_int64), ("variable_h", C.c_int32),
                 ("h_max", C.c_float), ("xsub", C.c_int32), ("used_rows", C.c_int32),
                 ("nlist_rows_used", C.c_int64), ("nlist_rows_capacity", C.c_int64),
-                ("nlist_fallback_warps", C.c_int64), ("n_levels", C.c_int32), ("n_keys", C.c_int64)]
+                ("nlist_fallback_warps", C.c_int64), ("n_levels", C.c_int32), ("n_keys", C.c_int64),
+                ("candidates_search", C.c_int64)]
 
 
 class sph_profile(C.Structure):

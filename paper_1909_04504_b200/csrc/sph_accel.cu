@@ -7,9 +7,9 @@
 // viscosity of eq.10 (L134-136) is added in the same loop (LAMINAR instantiations).
 #include "sph_tile.cuh"
 
-// One kernel, two modes (sph_tile.cuh).  REPLAY = false: the warp tests its own candidates (continuity mode,
-// custom tables).  REPLAY = true: it replays the hit masks recorded by the density pass of the same evaluation
-// and tests nothing (a warp whose record did not fit the pool searches).  Destination arrays named in
+// One kernel, two modes (sph_tile.cuh).  REPLAY = false: the warp searches its own candidates (no record pool).
+// REPLAY = true: it replays the candidate masks recorded by launch_search for this sorted order and walks
+// nothing (a warp whose record did not fit the pool searches).  Destination arrays named in
 // arho_only_arrays serve ContinuityEquation(dest=solid, sources=[fluid]) (Listing 3): the same loop,
 // only arho is stored; they share the launch with the momentum destinations.
 // This file is compiled four times (build.py): once per smoothing kernel with -DSPH_ACCEL_KERNEL=<id> (the kernel
@@ -135,7 +135,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         S.acc[i] = a;
         if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
-    const unsigned long long h = warp_sum_u64(nhits), t = warp_sum_u64(st.tests);
+    const unsigned long long h = warp_sum_u64(nhits), t = warp_sum_u64((unsigned long long)st.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_ACCEL], h); if (t) atomicAdd(&counters[CNT_CAND_ACCEL], t); }
 }
 
@@ -176,11 +176,11 @@ int SPH_CAT(launch_accel_k, SPH_ACCEL_KERNEL)(sph_ctx* c, int dim, bool filter, 
 // One launch serves every destination array whose mask is non-zero.  roles.arho_only: bit a = array a stores only
 // its continuity sum (ContinuityEquation(dest=solid, sources=[fluid]), Listing 3).
 int launch_accel(sph_ctx* c, const uint32_t* src_mask_per_dest, bool want_arho, const AccelRoles& roles) {
-    bool filter = false, use_list = c->nl_valid && !roles.arho_only;
+    bool filter = false;
+    const bool use_list = c->nl_valid && c->nl.pool != nullptr;     // records of launch_search for this sorted order
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
         if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) filter = true;
-        if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->nl_mask[a]) use_list = false;   // rows recorded with another mask
     }
     c->last_used_rows = use_list;
     const int k = c->prm.kernel, d = c->grid.dim;

@@ -314,14 +314,21 @@ static int zero_counters(sph_ctx* c, int first, int last) {       // one memset 
     return SPH_OK;
 }
 
+// one search per sorted order, shared by every pair pass that follows (no-op without a record pool)
+static int ensure_search(sph_ctx* c) {
+    if (c->nl_valid || c->nl.pool == nullptr) return SPH_OK;
+    return launch_search(c);
+}
+
 extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask, float* rho_out, float* p_out, int mem) {
     if (!c) return SPH_ERR_NULL;
     if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
     if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
     uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
     masks[dest] = source_mask;
-    int rc = zero_counters(c, CNT_PAIRS_DENSITY, CNT_NL_USED); if (rc) return rc;
-    rc = launch_density(c, masks, true); if (rc) return rc;
+    int rc = ensure_search(c); if (rc) return rc;
+    rc = zero_counters(c, CNT_PAIRS_DENSITY, CNT_CAND_DENSITY); if (rc) return rc;
+    rc = launch_density(c, masks); if (rc) return rc;
     if (rho_out || p_out) { OutPtrs O; memset(&O, 0, sizeof(O)); O.rho = rho_out; O.p = p_out; return emit(c, dest, O, mem); }
     return SPH_OK;
 }
@@ -332,7 +339,8 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
     if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
     uint32_t masks[SPH_MAX_ARRAYS] = { 0, 0, 0, 0 };
     masks[dest] = source_mask;
-    int rc = zero_counters(c, CNT_PAIRS_ACCEL, CNT_CAND_ACCEL); if (rc) return rc;
+    int rc = ensure_search(c); if (rc) return rc;
+    rc = zero_counters(c, CNT_PAIRS_ACCEL, CNT_CAND_ACCEL); if (rc) return rc;
     const AccelRoles roles = { 0u, 0u, 0u, 0u };
     rc = launch_accel(c, masks, arho != nullptr, roles); if (rc) return rc;
     if (ax || ay || az || arho) { OutPtrs O; memset(&O, 0, sizeof(O)); O.ax = ax; O.ay = ay; O.az = az; O.arho = arho; return emit(c, dest, O, mem); }
@@ -343,6 +351,7 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
 // continuity + momentum.  Destinations that share a source mask share a launch.
 static int evaluate(sph_ctx* c, bool continuity) {
     int rc;
+    rc = ensure_search(c); if (rc) return rc;
     rc = zero_counters(c, CNT_PAIRS_DENSITY, CNT_CAND_ACCEL); if (rc) return rc;
     auto grouped = [&](const uint32_t* tbl, const bool* take, auto&& fn) -> int {
         bool done[SPH_MAX_ARRAYS] = { false, false, false, false };
@@ -356,17 +365,7 @@ static int evaluate(sph_ctx* c, bool continuity) {
     };
     bool all[SPH_MAX_ARRAYS] = { true, true, true, true };
     if (!continuity) {
-        // a density launch records its neighbour rows when it serves every destination of the momentum pass
-        // with the same source masks (the default tables do): the momentum pass then replays the rows.
-        rc = grouped(c->tbl_density, all, [&](const uint32_t* m) {
-            bool rec = false;
-            for (int a = 0; a < c->na; ++a) if (c->tbl_accel[a]) rec = true;
-            for (int a = 0; a < c->na; ++a) if (c->tbl_accel[a] && m[a] != c->tbl_accel[a]) rec = false;
-            const bool keep = c->nl_valid;                     // rows of an earlier launch of this evaluation
-            uint32_t keep_mask[SPH_MAX_ARRAYS]; memcpy(keep_mask, c->nl_mask, sizeof(keep_mask));
-            int r = launch_density(c, m, rec);
-            if (!rec && keep) { c->nl_valid = true; memcpy(c->nl_mask, keep_mask, sizeof(keep_mask)); }
-            return r; });
+        rc = grouped(c->tbl_density, all, [&](const uint32_t* m) { return launch_density(c, m); });
         if (rc) return rc;
     }
     bool fused[SPH_MAX_ARRAYS], plain[SPH_MAX_ARRAYS], only[SPH_MAX_ARRAYS];
@@ -495,7 +494,8 @@ extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->pairs_accel = (int64_t)h[CNT_PAIRS_ACCEL];
     out->candidates_density = (int64_t)h[CNT_CAND_DENSITY];
     out->candidates_accel = (int64_t)h[CNT_CAND_ACCEL];
-    out->candidates = out->candidates_density + out->candidates_accel;
+    out->candidates_search = (int64_t)h[CNT_CAND_SEARCH];
+    out->candidates = out->candidates_density + out->candidates_accel + out->candidates_search;
     out->kernel_launches = c->launches;
     out->steps_done = c->steps_done;
     out->variable_h = c->variable_h ? 1 : 0;
@@ -568,6 +568,8 @@ extern "C" const char* sph_kernel_name(int id) {
         case SPH_K_OUTPUT: return "k_gather_out";
         case SPH_K_NEIGHBORS: return "k_neighbors";
         case SPH_K_ACCEL_LIST: return "k_accel_list";
+        case SPH_K_SEARCH: return "k_search";
+        case SPH_K_DENSITY_LIST: return "k_density_list";
     }
     return "";
 }

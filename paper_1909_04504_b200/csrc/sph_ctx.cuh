@@ -3,11 +3,10 @@
 #include "sph_internal.cuh"
 #include <stdio.h>
 
-// device counters: [2..5] belong to a density (recording) pass, [6..7] to an acceleration pass, so that one
-// memset clears what a pass (or a whole evaluation: [2..7]) is about to count
-enum { CNT_OUT_OF_DOMAIN = 0, CNT_NONFINITE = 1, CNT_PAIRS_DENSITY = 2, CNT_CAND_DENSITY = 3, CNT_OVERFLOW = 4,
-       CNT_NL_USED = 5 /* low 32 bits: record rows handed out (NList::used) */, CNT_PAIRS_ACCEL = 6, CNT_CAND_ACCEL = 7,
-       CNT_COUNT = 8 };
+// device counters: [2..5] are cleared by every evaluation / pair call, [6..8] by every search
+enum { CNT_OUT_OF_DOMAIN = 0, CNT_NONFINITE = 1, CNT_PAIRS_DENSITY = 2, CNT_CAND_DENSITY = 3, CNT_PAIRS_ACCEL = 4,
+       CNT_CAND_ACCEL = 5, CNT_OVERFLOW = 6, CNT_NL_USED = 7 /* low 32 bits: record rows handed out (NList::used) */,
+       CNT_CAND_SEARCH = 8, CNT_COUNT = 9 };
 
 struct sph_ctx {
     cudaStream_t stream;
@@ -40,8 +39,7 @@ struct sph_ctx {
 
     // neighbour rows recorded by a density launch for the acceleration launch that follows it
     NList nl;                  // nl.pool == nullptr: recording disabled
-    bool nl_valid;             // rows match the current sort and the masks below
-    uint32_t nl_mask[SPH_MAX_ARRAYS];   // per dest array: the source mask the rows were recorded with (0 = none)
+    bool nl_valid;             // the records match the current sorted order (launch_search ran since the last sort)
     bool last_used_rows;       // the last acceleration launch replayed recorded rows
     bool xsub_auto;            // xsub was not given: 6, or 16 when h varies
     int xsub;                  // x sub-cells per support radius requested (GridDesc::xsub is what the grid got)
@@ -88,7 +86,8 @@ int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O);
 int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32_t* indices, int64_t cap,
                           int64_t* total, int mem);
 // sph_density.cu / sph_accel.cu: one launch serves every dest array whose mask is non-zero
-int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record);
+int launch_search(sph_ctx* c);                       // sph_search.cu: records the candidate masks of the current sorted order
+int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest);
 // what a momentum launch stores for which array (bitmasks over arrays)
 struct AccelRoles {
     uint32_t arho_only;        // destination arrays that store only their continuity sum (acc.w)

@@ -1,12 +1,12 @@
 // Summation density, eq.3 (L112): rho_i = sum_j m_j W(x_i - x_j, h_ij), with the Tait EOS
 // (eq.6, Listing 4) fused as the epilogue (the group barrier of L337/L382 is the kernel
-// boundary: every p is stored before the acceleration kernel starts).  A RECORD launch also writes the
-// hit masks of its candidate tests (sph_tile.cuh), for the acceleration pass of the same evaluation to replay.
+// boundary: every p is stored before the acceleration kernel starts).  A REPLAY launch takes its candidates from
+// the records of launch_search (sph_search.cu) and walks nothing; otherwise the warp searches itself.
 #include "sph_tile.cuh"
 
 struct DensitySrc { float4 pj; float mj; uint32_t aid; };
 
-template <int KERNEL, int DIM, bool VARH, bool FILTER, bool RECORD, bool UM>
+template <int KERNEL, int DIM, bool VARH, bool FILTER, bool REPLAY, bool UM>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
 k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
                NList nl, unsigned long long* __restrict__ counters) {
@@ -62,14 +62,16 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
 
     TileState st; st.reset(); st.tests = 0;
     const uint32_t idle = in ? (uint32_t)i : 0u;
-    TileRecorder rec; rec.init(nl); if (!RECORD) rec.ok = false;
-    auto drain = [&]() {
-        if (RECORD) rec.append(ws, st.M, st.shifted, warp_id, counters);
-        if (st.shifted) tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, true>(ws, st.nz, idle, load, compute);
-        else            tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, false>(ws, st.nz, idle, load, compute);
-        st.reset();
+    auto drain = [&](uint32_t nz, bool shifted) {
+        if (shifted) tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, true>(ws, nz, idle, load, compute);
+        else         tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, false>(ws, nz, idle, load, compute);
     };
-    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, drain);
+    const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
+    if (head != SPH_NL_NONE) {
+        tile_replay(nl, head, ws, active, drain);
+    } else {                                    // no record (or one that did not fit the pool): search
+        tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
+    }
 
     if (active) {
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
@@ -78,19 +80,19 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         if (UM && !VARH) S.posh[i].w = p / (rho * rho);                 // UM layout: posh.w carries p/rho^2
         if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
-    const unsigned long long h = warp_sum_u64(nhits), t = warp_sum_u64(st.tests);
+    const unsigned long long h = warp_sum_u64(nhits), t = warp_sum_u64((unsigned long long)st.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CAND_DENSITY], t); }
 }
 
 template <int KERNEL, int DIM>
-static int launch_density_tile_kd(sph_ctx* c, bool filter, bool record) {
+static int launch_density_tile_kd(sph_ctx* c, bool filter, bool replay) {
     const int n = (int)c->n_total;
     if (n == 0) return SPH_OK;
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
     SortedState& S = c->S[c->cur];
-#define LD(VARH, FILTER, RECORD, UM) \
-        SPH_LAUNCH(c, SPH_K_DENSITY, (k_density_tile<KERNEL, DIM, VARH, FILTER, RECORD, UM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters)
-#define LD2(VARH, FILTER, UM) do { if (record) LD(VARH, FILTER, true, UM); else LD(VARH, FILTER, false, UM); } while (0)
+#define LD(VARH, FILTER, REPLAY, UM) \
+        SPH_LAUNCH(c, (REPLAY ? SPH_K_DENSITY_LIST : SPH_K_DENSITY), (k_density_tile<KERNEL, DIM, VARH, FILTER, REPLAY, UM>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters)
+#define LD2(VARH, FILTER, UM) do { if (replay) LD(VARH, FILTER, true, UM); else LD(VARH, FILTER, false, UM); } while (0)
 #define LD3(VARH, UM) do { if (filter) LD2(VARH, true, UM); else LD2(VARH, false, UM); } while (0)
     if (c->variable_h) { if (c->pc.varh_um) LD3(true, true); else LD3(true, false); } else if (c->pc.uniform_m) LD3(false, true); else LD3(false, false);
 #undef LD3
@@ -99,30 +101,21 @@ static int launch_density_tile_kd(sph_ctx* c, bool filter, bool record) {
     return SPH_OK;
 }
 
-// One launch computes rho,p for every array whose src_mask_per_dest entry is non-zero.
-int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest, bool record) {
+// One launch computes rho,p for every array whose src_mask_per_dest entry is non-zero; it replays the records of
+// launch_search when they match the current sorted order and searches itself otherwise.
+int launch_density(sph_ctx* c, const uint32_t* src_mask_per_dest) {
     bool filter = false;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) {
         c->pc.src_mask[a] = a < c->na ? src_mask_per_dest[a] : 0u;
         if (c->pc.src_mask[a] && c->pc.src_mask[a] != c->pc.all_mask) filter = true;
     }
-    record = record && c->nl.pool != nullptr && c->n_total > 0;
-    c->nl_valid = false;
-    if (record) {
-        SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.head, 0, (size_t)((c->n_total + 31) / 32 + 1) * sizeof(uint32_t), c->stream));
-        // nl.used and the overflow counter live in the counter block the caller has just cleared (CNT_NL_USED)
-    }
+    const bool replay = c->nl_valid && c->nl.pool != nullptr;
     const int k = c->prm.kernel, d = c->grid.dim;
     int rc = sph_fail(c, SPH_ERR_BAD_ARG, "unsupported kernel/dim");
-#define KD(K, D) if (k == K && d == D) rc = launch_density_tile_kd<K, D>(c, filter, record)
+#define KD(K, D) if (k == K && d == D) rc = launch_density_tile_kd<K, D>(c, filter, replay)
     KD(SPH_KERNEL_CUBIC, 2); KD(SPH_KERNEL_CUBIC, 3);
     KD(SPH_KERNEL_QUINTIC, 2); KD(SPH_KERNEL_QUINTIC, 3);
     KD(SPH_KERNEL_WENDLAND_C2, 2); KD(SPH_KERNEL_WENDLAND_C2, 3);
 #undef KD
-    if (rc == SPH_OK && record) {
-        c->nl_valid = true;
-        for (int a = 0; a < SPH_MAX_ARRAYS; ++a) c->nl_mask[a] = c->pc.src_mask[a];
-    }
     return rc;
 }
-

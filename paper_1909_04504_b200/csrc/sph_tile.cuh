@@ -58,13 +58,18 @@ struct __align__(16) TileWarpSmem {
     uint32_t base[32];                     // first sorted index of every batch
     uint32_t bcode[32];                    // image-shift code of every batch (2 bits per axis: 1 -> -L, 2 -> +L)
     uint32_t seg_s[32], seg_e[32], seg_c[32];   // candidate runs of the current pass: [s, e) and image-shift code
+    // warp-uniform walker state that only the (cold) group / level / pass set-up code touches: kept here, not in
+    // registers, so that the batch loop stays within the register budget
+    float bb[8];                           // group bounding box xmin, xmax, ymin, ymax, zmin, zmax, largest h, half extent
+    int lv[8];                             // level ranges x0, x1, y0, z0, ny, entries, nparts | low << 8 | high << 9
+    float inv_ny;
 };
 
 struct TileState {
     int M;                                 // masks stored since the last drain (warp-uniform)
     uint32_t nz;                           // bit m: this lane's mask m is not empty
     bool shifted;                          // some stored batch came from a periodic image (warp-uniform)
-    unsigned long long tests;              // candidates streamed for this lane's particle
+    unsigned tests;                        // candidates streamed for this lane's particle
     __device__ __forceinline__ void reset() { M = 0; nz = 0u; shifted = false; }
 };
 
@@ -133,14 +138,13 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
                           ((uint32_t)(4 + (tq ^ 2)) << (4 * (tq ^ 2))) | ((uint32_t)(4 + (tq ^ 3)) << (4 * (tq ^ 3)));
     const int cidx = 8 * (gq >> 1) + 7 - (gq & 1);           // column g of N-tile nt holds staged candidate cidx - 2 nt
 
-    // ---- group state (warp-uniform unless noted)
+    // ---- group state (warp-uniform unless noted); the cold part lives in ws.bb / ws.lv
     bool grp = false, ing = false /* per lane */;
-    float xmin = 0, xmax = 0, ymin = 0, ymax = 0, zmin = 0, zmax = 0, hg = pc.h_const, ox = 0, oy = 0, oz = 0, exm = 0;
+    float ox = 0, oy = 0, oz = 0;
     uint32_t A0[4] = {0, 0, 0, 0}, A1[4] = {0, 0, 0, 0};      // per lane: A operands (rows of the quad's four particles)
     // ---- level state
-    int b = 0, pass = 0, npass = 0, entries = 0, nparts = 1, ny = 1, x0 = 0, x1 = 0, y0 = 0, z0 = 0;
-    bool lowpart = false, highpart = false;
-    float margin = 0.0f, inv_ny = 1.0f;
+    int b = 0, pass = 0, npass = 0;
+    float nsub = 0.0f;                                         // subtracted on the candidate side: filter margin (+ cut^2 when h is constant)
     // ---- run / batch state
     unsigned segs = 0u;
     bool have = false;
@@ -168,12 +172,12 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         remaining &= ~gmask;
         ing = (gmask >> lane) & 1u;
         const float big = 3.0e38f;
-        xmin = warp_min_f(ing ? pi.x : big); xmax = warp_max_f(ing ? pi.x : -big);
-        ymin = warp_min_f(ing ? pi.y : big); ymax = warp_max_f(ing ? pi.y : -big);
+        const float xmin = warp_min_f(ing ? pi.x : big), xmax = warp_max_f(ing ? pi.x : -big);
+        const float ymin = warp_min_f(ing ? pi.y : big), ymax = warp_max_f(ing ? pi.y : -big);
+        float zmin = 0.0f, zmax = 0.0f, hg = pc.h_const;
         if (DIM == 3) { zmin = warp_min_f(ing ? pi.z : big); zmax = warp_max_f(ing ? pi.z : -big); }
         if (VARH) hg = __uint_as_float(__reduce_max_sync(SPH_FULL_MASK, ing ? __float_as_uint(pi.w) : 0u));
         ox = 0.5f * (xmin + xmax); oy = 0.5f * (ymin + ymax); oz = DIM == 3 ? 0.5f * (zmin + zmax) : 0.0f;
-        exm = 0.5f * fmaxf(fmaxf(xmax - xmin, ymax - ymin), DIM == 3 ? zmax - zmin : 0.0f);
         // A operands of this lane's particle: [-2x, -2y, -2z, -2 kh^2 h, n_hi, n_lo, 1, 1], n = |x|^2 - kh^2 h^2
         const float xt = tf32r(pi.x - ox), yt = tf32r(pi.y - oy), zt = DIM == 3 ? tf32r(pi.z - oz) : 0.0f;
         const float ht = VARH ? tf32r(pi.w) : 0.0f;
@@ -183,6 +187,10 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         float* af = ws.Af + lane * 9;
         af[0] = -2.0f * xt; af[1] = -2.0f * yt; af[2] = -2.0f * zt; af[3] = tf32r(-2.0f * khsq * ht);
         af[4] = nh; af[5] = nl; af[6] = 1.0f; af[7] = 1.0f;
+        if (lane == 0) {
+            ws.bb[0] = xmin; ws.bb[1] = xmax; ws.bb[2] = ymin; ws.bb[3] = ymax; ws.bb[4] = zmin; ws.bb[5] = zmax; ws.bb[6] = hg;
+            ws.bb[7] = 0.5f * fmaxf(fmaxf(xmax - xmin, ymax - ymin), DIM == 3 ? zmax - zmin : 0.0f);
+        }
         __syncwarp();
         const float* q = ws.Af + (4 * gq) * 9 + tq;             // rows of the quad's particles 0..3, features tq and tq + 4
         A0[0] = __float_as_uint(q[0]);      A0[1] = __float_as_uint(q[9]);       A0[2] = __float_as_uint(q[4]);      A0[3] = __float_as_uint(q[13]);
@@ -193,32 +201,40 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
     // candidate cells of level b: the level's cells that meet the group's bounding box grown by the reach R
     auto setup_level = [&]() {
         const LevelDesc& Lv = g.lev[b];
-        const float R = pc.kh * (hg + (VARH ? Lv.hmax : pc.h_const)) * 1.0001f + 16.0f * g.uabs;
-        const float X = exm + R;                               // bound of every tile-local coordinate that matters
-        margin = (R * X + R * R) * (1.0f / 128.0f) + X * X * (1.0f / 32768.0f) + 64.0f * g.uabs * (R + X);
+        const float xmin = ws.bb[0], xmax = ws.bb[1], ymin = ws.bb[2], ymax = ws.bb[3], zmin = ws.bb[4], zmax = ws.bb[5];
+        const float R = pc.kh * (ws.bb[6] + (VARH ? Lv.hmax : pc.h_const)) * 1.0001f + 16.0f * g.uabs;
+        const float X = ws.bb[7] + R;                          // bound of every tile-local coordinate that matters
+        // filter margin: bounds the tf32 rounding of operands and accumulation
+        nsub = (R * X + R * R) * (1.0f / 256.0f) + X * X * (1.0f / 32768.0f) + 64.0f * g.uabs * (R + X) + (VARH ? 0.0f : cut2c);
         const int n0 = Lv.nc[0], n1 = Lv.nc[1], n2 = Lv.nc[2];
         const float e0 = 1.0e-3f + 4.8e-7f * (float)n0, e1 = 1.0e-3f + 4.8e-7f * (float)n1, e2 = 1.0e-3f + 4.8e-7f * (float)n2;
-        x0 = __float2int_rd((xmin - R - g.lo[0]) * Lv.inv_cell[0] - e0); x1 = __float2int_rd((xmax + R - g.lo[0]) * Lv.inv_cell[0] + e0);
-        y0 = __float2int_rd((ymin - R - g.lo[1]) * Lv.inv_cell[1] - e1);
-        int y1 = __float2int_rd((ymax + R - g.lo[1]) * Lv.inv_cell[1] + e1);
-        int z1 = 0; z0 = 0;
+        int x0 = __float2int_rd((xmin - R - g.lo[0]) * Lv.inv_cell[0] - e0), x1 = __float2int_rd((xmax + R - g.lo[0]) * Lv.inv_cell[0] + e0);
+        int y0 = __float2int_rd((ymin - R - g.lo[1]) * Lv.inv_cell[1] - e1), y1 = __float2int_rd((ymax + R - g.lo[1]) * Lv.inv_cell[1] + e1);
+        int z0 = 0, z1 = 0;
         if (DIM == 3) { z0 = __float2int_rd((zmin - R - g.lo[2]) * Lv.inv_cell[2] - e2); z1 = __float2int_rd((zmax + R - g.lo[2]) * Lv.inv_cell[2] + e2); }
         if (!g.per[0]) { x0 = max(x0, 0); x1 = min(x1, n0 - 1); } else { x0 = max(x0, -n0); x1 = min(x1, 2 * n0 - 1); }
         if (!g.per[1]) { y0 = max(y0, 0); y1 = min(y1, n1 - 1); } else { y0 = max(y0, -n1); y1 = min(y1, 2 * n1 - 1); }
         if (DIM == 3) { if (!g.per[2]) { z0 = max(z0, 0); z1 = min(z1, n2 - 1); } else { z0 = max(z0, -n2); z1 = min(z1, 2 * n2 - 1); } }
-        lowpart = g.per[0] && x0 < 0; highpart = g.per[0] && x1 >= n0;
-        nparts = 1 + (lowpart ? 1 : 0) + (highpart ? 1 : 0);
-        ny = y1 - y0 + 1;
-        const int nzr = z1 - z0 + 1;
-        entries = (ny > 0 && nzr > 0 && x1 >= x0) ? ny * nzr * nparts : 0;
+        const bool lowpart = g.per[0] && x0 < 0, highpart = g.per[0] && x1 >= n0;
+        const int nparts = 1 + (lowpart ? 1 : 0) + (highpart ? 1 : 0);
+        const int ny = y1 - y0 + 1, nzr = z1 - z0 + 1;
+        const int entries = (ny > 0 && nzr > 0 && x1 >= x0) ? ny * nzr * nparts : 0;
         npass = (entries + 31) >> 5;
-        inv_ny = 1.0f / (float)max(ny, 1);
+        __syncwarp();
+        if (lane == 0) {
+            ws.lv[0] = x0; ws.lv[1] = x1; ws.lv[2] = y0; ws.lv[3] = z0; ws.lv[4] = ny; ws.lv[5] = entries;
+            ws.lv[6] = nparts | (lowpart ? 0x100 : 0) | (highpart ? 0x200 : 0);
+            ws.inv_ny = 1.0f / (float)max(ny, 1);
+        }
+        __syncwarp();
     };
 
     // 32 lanes look up 32 (row, x part) entries of the current level: [s, e) of the sorted order + shift code
     auto setup_pass = [&]() {
         const LevelDesc& Lv = g.lev[b];
         const int n0 = Lv.nc[0], n1 = Lv.nc[1], n2 = Lv.nc[2];
+        const int x0 = ws.lv[0], x1 = ws.lv[1], y0 = ws.lv[2], z0 = ws.lv[3], ny = ws.lv[4], entries = ws.lv[5];
+        const int nparts = ws.lv[6] & 0xff; const bool lowpart = (ws.lv[6] & 0x100) != 0;
         const int ent = pass * 32 + lane;
         bool nonempty = false;
         uint32_t s_ = 0u, e_ = 0u, code = 0u;
@@ -226,7 +242,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
             int r = ent, part = 0;
             if (nparts == 2) { r = ent >> 1; part = ent & 1; } else if (nparts == 3) { r = ent / 3; part = ent - 3 * r; }
             const int kind = part == 0 ? 0 : (part == 1 ? (lowpart ? 1 : 2) : 2);
-            const int rz = (int)(((float)r + 0.5f) * inv_ny);
+            const int rz = (int)(((float)r + 0.5f) * ws.inv_ny);
             int iy = y0 + (r - rz * ny), iz = z0 + rz;
             if (iy < 0) { iy += n1; code |= 1u << 2; } else if (iy >= n1) { iy -= n1; code |= 2u << 2; }
             if (iz < 0) { iz += n2; code |= 1u << 4; } else if (iz >= n2) { iz -= n2; code |= 2u << 4; }
@@ -256,7 +272,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         }
         const float xt = tf32r(xr - ox), yt = tf32r(yr - oy), zt = DIM == 3 ? tf32r(zr - oz) : 0.0f;
         const float ht = VARH ? tf32r(pj.w) : 0.0f;
-        float n = fmaf(zt, zt, fmaf(yt, yt, xt * xt)) - (VARH ? khsq * ht * ht : cut2c) - margin;
+        float n = fmaf(zt, zt, fmaf(yt, yt, xt * xt)) - (VARH ? khsq * ht * ht : 0.0f) - nsub;
         n = valid ? n : 1.0e30f;                                // padding never passes
         const float nh = tf32r(n), nl = tf32r(n - nh);
         __syncwarp();                                           // readers of the previous batch are done
@@ -265,15 +281,21 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         __syncwarp();
         uint32_t pm0 = 0u, pm1 = 0u, pm2 = 0u, pm3 = 0u;        // sign bits of the quad's particles 0..3 (this thread's columns)
 #pragma unroll
-        for (int nt = 0; nt < 4; ++nt) {
-            const float2 bf = ws.G[tq][cidx - 2 * nt];
-            float c0[4], c1[4];
-            mma_tf32_16x8x8(c0, A0, __float_as_uint(bf.x), __float_as_uint(bf.y));
-            mma_tf32_16x8x8(c1, A1, __float_as_uint(bf.x), __float_as_uint(bf.y));
-            pm0 = __funnelshift_l(__float_as_uint(c0[0]), pm0, 1); pm0 = __funnelshift_l(__float_as_uint(c0[1]), pm0, 1);
-            pm1 = __funnelshift_l(__float_as_uint(c0[2]), pm1, 1); pm1 = __funnelshift_l(__float_as_uint(c0[3]), pm1, 1);
-            pm2 = __funnelshift_l(__float_as_uint(c1[0]), pm2, 1); pm2 = __funnelshift_l(__float_as_uint(c1[1]), pm2, 1);
-            pm3 = __funnelshift_l(__float_as_uint(c1[2]), pm3, 1); pm3 = __funnelshift_l(__float_as_uint(c1[3]), pm3, 1);
+        for (int half = 0; half < 2; ++half) {                  // 4 independent MMAs in flight, then their 16 sign bits
+            float c[2][2][4];
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const float2 bf = ws.G[tq][cidx - 2 * (2 * half + k)];
+                mma_tf32_16x8x8(c[k][0], A0, __float_as_uint(bf.x), __float_as_uint(bf.y));
+                mma_tf32_16x8x8(c[k][1], A1, __float_as_uint(bf.x), __float_as_uint(bf.y));
+            }
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                pm0 = __funnelshift_l(__float_as_uint(c[k][0][0]), pm0, 1); pm0 = __funnelshift_l(__float_as_uint(c[k][0][1]), pm0, 1);
+                pm1 = __funnelshift_l(__float_as_uint(c[k][0][2]), pm1, 1); pm1 = __funnelshift_l(__float_as_uint(c[k][0][3]), pm1, 1);
+                pm2 = __funnelshift_l(__float_as_uint(c[k][1][0]), pm2, 1); pm2 = __funnelshift_l(__float_as_uint(c[k][1][1]), pm2, 1);
+                pm3 = __funnelshift_l(__float_as_uint(c[k][1][2]), pm3, 1); pm3 = __funnelshift_l(__float_as_uint(c[k][1][3]), pm3, 1);
+            }
         }
         // byte q of P: this thread's 8 columns against particle q of the quad; transpose the 4 x 4 bytes of the quad
         const uint32_t P = __byte_perm(__byte_perm(pm0, pm1, 0x0040), __byte_perm(pm2, pm3, 0x0040), 0x5410);
