@@ -7,7 +7,7 @@
 struct DensitySrc { float4 pj; float mj; uint32_t aid; };
 
 template <int KERNEL, int DIM, bool VARH, bool FILTER, bool REPLAY, bool UM>
-__global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
+__global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS_DENSITY)
 k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
                NList nl, unsigned long long* __restrict__ counters) {
     __shared__ TileWarpSmem smem[TILE_WARPS];
@@ -26,7 +26,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     const float hi = VARH ? pi.w : pc.h_const;
     const float cut2c = pair_cut2(kh, pc.h_const, pc.h_const);
     const float mfac_c = pc.m_const * pc.fac_const;                     // UM layout: posh.w is p/rho^2, the mass is m_const
-    float rho = 0.0f;
+    float2 rho2 = pk1(0.0f);                                            // two partial sums: even / odd candidates of the lane
     unsigned nhits = 0;                                                 // pairs that pass the exact predicate (and the source mask)
     // constant h: posh.w of the sorted state carries the MASS (SortedState), one 16-byte gather per pair.  Plain
     // loads: the epilogue of this launch rewrites .w words of posh / velm that other warps' gathers cover (x, y, z
@@ -37,34 +37,40 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
         return s;
     };
-    auto compute = [&](const DensitySrc& s, bool has, uint32_t code, auto per) {
-        // the exact predicate of DESIGN.md R7 on the candidate the tensor-core filter let through
-        float dx = __fsub_rn(pi.x, s.pj.x), dy = __fsub_rn(pi.y, s.pj.y), dz = DIM == 3 ? __fsub_rn(pi.z, s.pj.z) : 0.0f;
+    const float2 xi2 = pk1(pi.x), yi2 = pk1(pi.y), zi2 = pk1(pi.z);
+    // two candidates (a, b) of this lane at a time, packed f32x2
+    auto compute = [&](const DensitySrc& a, const DensitySrc& b, bool ha, bool hb, uint32_t ca, uint32_t cb, auto per) {
+        // the exact predicate of DESIGN.md R7 on the candidates the tensor-core filter let through
+        float2 dx = sub2(xi2, pk(a.pj.x, b.pj.x)), dy = sub2(yi2, pk(a.pj.y, b.pj.y));
+        float2 dz = DIM == 3 ? sub2(zi2, pk(a.pj.z, b.pj.z)) : pk1(0.0f);
         if (decltype(per)::value) {
-            dx = __fsub_rn(dx, img_shift(code, 0, Lx)); dy = __fsub_rn(dy, img_shift(code, 1, Ly));
-            if (DIM == 3) dz = __fsub_rn(dz, img_shift(code, 2, Lz));
+            dx = sub2(dx, pk(img_shift(ca, 0, Lx), img_shift(cb, 0, Lx))); dy = sub2(dy, pk(img_shift(ca, 1, Ly), img_shift(cb, 1, Ly)));
+            if (DIM == 3) dz = sub2(dz, pk(img_shift(ca, 2, Lz), img_shift(cb, 2, Lz)));
         }
-        const float r2 = pair_r2(dx, dy, dz);
-        has = has && r2 < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);
-        if (FILTER) has = has && ((my_mask >> s.aid) & 1u);
-        nhits += has ? 1u : 0u;
-        const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;
-        const float r = r2 * rinv;
-        float hinv, mfac;
+        const float2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        ha = ha && r2.x < (VARH ? pair_cut2(kh, hi, a.pj.w) : cut2c);
+        hb = hb && r2.y < (VARH ? pair_cut2(kh, hi, b.pj.w) : cut2c);
+        if (FILTER) { ha = ha && ((my_mask >> a.aid) & 1u); hb = hb && ((my_mask >> b.aid) & 1u); }
+        nhits += (ha ? 1u : 0u) + (hb ? 1u : 0u);
+        const float2 rinv = pk(r2.x > 0.0f ? rsqrt_approx(r2.x) : 0.0f, r2.y > 0.0f ? rsqrt_approx(r2.y) : 0.0f);
+        const float2 r = mul2(r2, rinv);
+        float2 hinv, mfac;
         if (VARH) {
-            hinv = rcp_approx(0.5f * (hi + s.pj.w));
-            mfac = (UM ? pc.m_const : s.mj) * sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
-        } else { hinv = hinv_c; mfac = UM ? mfac_c : s.pj.w * fac_c; }
-        float f, df;
-        kernel_profile<KERNEL, DIM>(r * hinv, f, df);
-        rho = has ? fmaf(mfac, f, rho) : rho;
+            hinv = rcp2(mul2(pk1(0.5f), add2(pk1(hi), pk(a.pj.w, b.pj.w))));
+            const float2 m2 = UM ? pk1(pc.m_const) : pk(a.mj, b.mj);
+            mfac = mul2(mul2(m2, pk1(sigma)), DIM == 3 ? mul2(mul2(hinv, hinv), hinv) : mul2(hinv, hinv));
+        } else { hinv = pk1(hinv_c); mfac = UM ? pk1(mfac_c) : mul2(pk(a.pj.w, b.pj.w), pk1(fac_c)); }
+        float2 f, df;
+        kernel_profile2<KERNEL, DIM>(mul2(r, hinv), f, df);
+        mfac = pk(ha ? mfac.x : 0.0f, hb ? mfac.y : 0.0f);              // a candidate that fails contributes nothing
+        rho2 = fma2(mfac, f, rho2);
     };
 
     TileState st; st.reset(); st.tests = 0;
     const uint32_t idle = in ? (uint32_t)i : 0u;
     auto drain = [&](uint32_t nz, bool shifted) {
-        if (shifted) tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, true>(ws, nz, idle, load, compute);
-        else         tile_drain<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, false>(ws, nz, idle, load, compute);
+        if (shifted) tile_drain2<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, true>(ws, nz, idle, load, compute);
+        else         tile_drain2<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, false>(ws, nz, idle, load, compute);
     };
     const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
     if (head != SPH_NL_NONE) {
@@ -74,6 +80,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     }
 
     if (active) {
+        const float rho = rho2.x + rho2.y;
         const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
         S.rp[i] = make_float2(rho, p / (rho * rho));
         if (!VARH || UM) S.velm[i].w = rho;                             // constant h, or VU layout: velm.w carries rho (SortedState)

@@ -131,6 +131,55 @@ __device__ __forceinline__ void kernel_profile(float q, float& f, float& df) {
     }
 }
 
+// ---- packed f32x2 forms (sm_100 FADD2 / FMUL2 / FFMA2: one issue slot for two lanes of work).  The drains evaluate
+// two neighbours of a particle at a time: .x and .y are the two neighbours.  Round-to-nearest, same results as the
+// scalar forms.
+__device__ __forceinline__ float2 pk(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 pk1(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 max2(float2 a, float b) { return make_float2(fmaxf(a.x, b), fmaxf(a.y, b)); }
+__device__ __forceinline__ float2 rcp2(float2 a) { return make_float2(rcp_approx(a.x), rcp_approx(a.y)); }
+
+template <int KERNEL, int DIM>
+__device__ __forceinline__ void kernel_profile2(float2 q, float2& f, float2& df) {
+    if (KERNEL == SPH_KERNEL_CUBIC) {
+        const float2 t = sub2(pk1(2.0f), q);
+        const float2 qq = mul2(q, q);
+        const float2 inner_f  = fma2(qq, fma2(pk1(0.75f), q, pk1(-1.5f)), pk1(1.0f));   // 1 - 1.5 q^2 + 0.75 q^3
+        const float2 inner_df = mul2(q, fma2(pk1(2.25f), q, pk1(-3.0f)));               // -3 q + 2.25 q^2
+        const float2 tt = mul2(t, t);
+        const float2 outer_f  = mul2(mul2(pk1(0.25f), t), tt);
+        const float2 outer_df = mul2(pk1(-0.75f), tt);
+        f.x  = q.x < 1.0f ? inner_f.x : (q.x < 2.0f ? outer_f.x : 0.0f);
+        f.y  = q.y < 1.0f ? inner_f.y : (q.y < 2.0f ? outer_f.y : 0.0f);
+        df.x = q.x < 1.0f ? inner_df.x : (q.x < 2.0f ? outer_df.x : 0.0f);
+        df.y = q.y < 1.0f ? inner_df.y : (q.y < 2.0f ? outer_df.y : 0.0f);
+    } else if (KERNEL == SPH_KERNEL_QUINTIC) {
+        const float2 a = max2(sub2(pk1(3.0f), q), 0.0f), b = max2(sub2(pk1(2.0f), q), 0.0f), c = max2(sub2(pk1(1.0f), q), 0.0f);
+        const float2 a2 = mul2(a, a), b2 = mul2(b, b), c2 = mul2(c, c);
+        const float2 a4 = mul2(a2, a2), b4 = mul2(b2, b2), c4 = mul2(c2, c2);
+        f  = fma2(pk1(15.0f), mul2(c4, c), fma2(pk1(-6.0f), mul2(b4, b), mul2(a4, a)));
+        df = fma2(pk1(-75.0f), c4, fma2(pk1(30.0f), b4, mul2(pk1(-5.0f), a4)));
+    } else {
+        const float2 t = max2(fma2(pk1(-0.5f), q, pk1(1.0f)), 0.0f);
+        const float2 t2 = mul2(t, t);
+        if (DIM == 1) { f = mul2(mul2(t2, t), fma2(pk1(1.5f), q, pk1(1.0f))); df = mul2(mul2(pk1(-3.0f), q), t2); }
+        else          { f = mul2(mul2(t2, t2), fma2(pk1(2.0f), q, pk1(1.0f))); df = mul2(mul2(pk1(-5.0f), q), mul2(t2, t)); }
+    }
+}
+
+// p/rho^2 of the gamma = 7 Tait EOS for two densities (same polynomial as eos7_p)
+__device__ __forceinline__ float2 eos7_p_over_rho2_2(float2 rho, float rho0, float inv_rho0, float B) {
+    const float2 t = mul2(sub2(rho, pk1(rho0)), pk1(inv_rho0));
+    float2 s = fma2(t, pk1(1.0f), pk1(7.0f));
+    s = fma2(t, s, pk1(21.0f)); s = fma2(t, s, pk1(35.0f)); s = fma2(t, s, pk1(35.0f)); s = fma2(t, s, pk1(21.0f)); s = fma2(t, s, pk1(7.0f));
+    s = mul2(t, s);
+    return mul2(mul2(pk1(B), s), rcp2(mul2(rho, rho)));
+}
+
 __host__ __device__ inline double kernel_sigma(int kernel, int dim) {
     const double pi = 3.141592653589793238462643383279502884;
     if (kernel == SPH_KERNEL_CUBIC)   return dim == 1 ? 2.0 / 3.0 : dim == 2 ? 10.0 / (7.0 * pi) : 1.0 / pi;

@@ -36,14 +36,17 @@
 #ifndef TILE_MIN_BLOCKS
 #define TILE_MIN_BLOCKS 8                 // resident blocks per SM the pair kernels are compiled for (64 registers)
 #endif
+#ifndef TILE_MIN_BLOCKS_DENSITY
+#define TILE_MIN_BLOCKS_DENSITY 8
+#endif
 #ifndef TILE_MIN_BLOCKS_ACCEL
 #define TILE_MIN_BLOCKS_ACCEL 6           // the momentum kernel is faster with 80 registers and 6 blocks (measured, C3, C4)
 #endif
 #ifndef TILE_DRAIN_DEPTH_REPLAY
-#define TILE_DRAIN_DEPTH_REPLAY 3         // hits in flight in the replaying momentum kernel
+#define TILE_DRAIN_DEPTH_REPLAY 3         // candidates in flight in the replaying momentum kernel
 #endif
 #ifndef TILE_DRAIN_DEPTH_DENSITY
-#define TILE_DRAIN_DEPTH_DENSITY 3        // hits in flight in the density drain
+#define TILE_DRAIN_DEPTH_DENSITY 2        // PAIRS of candidates in flight in the density drain
 #endif
 #ifndef TILE_MMAX
 #define TILE_MMAX 24                      // masks per warp before a forced drain (<= 30: 30 bases + 2 words = one header row)
@@ -375,6 +378,47 @@ __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32
             compute(R[d], H[d], C[d], std::integral_constant<bool, PER>{});   // ... while this one is evaluated
         }
         if (!__any_sync(SPH_FULL_MASK, H[0])) break;   // pops are in order: no pending candidate 0 means none at all
+    }
+    __syncwarp();
+}
+
+// tile_drain2: as tile_drain, but every lane pops TWO candidates at a time and evaluates the pair with packed f32x2
+// arithmetic (pays where the loop is bound by instruction issue: the density pass; the momentum pass is bound by
+// its L1 gathers and stays scalar).  Branch-free and software-pipelined: DEPTH pairs are in
+// flight, the source data of a later pair is gathered (Src = load(sorted index)) before the current one is
+// computed, so the gather latency overlaps the arithmetic.  A lane that has run out keeps executing with has =
+// false and the harmless index `idle` (its own particle) until the slowest lane of the warp is done;
+// compute(srcA, srcB, hasA, hasB, codeA, codeB, per) must apply the exact predicate and contribute nothing where
+// it fails or has is false.  PER: some batch is a periodic image (code != 0).
+template <class Src, int DEPTH, bool PER, class Load, class Compute>
+__device__ __forceinline__ void tile_drain2(TileWarpSmem& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
+    const int lane = threadIdx.x & 31;
+    __syncwarp();
+    uint32_t cur = 0u, b = 0u, code = 0u;
+    auto pop = [&](bool& has, uint32_t& cd) -> uint32_t {
+        const bool refill = cur == 0u && nz != 0u;
+        const int m = max(__ffs(nz) - 1, 0);
+        const uint32_t nm = ws.mask[m][lane], nb = ws.base[m];
+        cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? (nz & (nz - 1u)) : nz;
+        if (PER) { const uint32_t nc = ws.bcode[m]; code = refill ? nc : code; }
+        has = cur != 0u;
+        const uint32_t j = has ? b + (uint32_t)(__ffs(cur) - 1) : idle;
+        cur &= cur - 1u;                        // stays 0 when it is 0
+        cd = code;
+        return j;
+    };
+    Src R[DEPTH][2]; bool H[DEPTH][2]; uint32_t C[DEPTH][2];   // fully unrolled, so these live in registers
+#pragma unroll
+    for (int d = 0; d + 1 < DEPTH; ++d) { R[d][0] = load(pop(H[d][0], C[d][0])); R[d][1] = load(pop(H[d][1], C[d][1])); }
+    for (;;) {
+#pragma unroll
+        for (int d = 0; d < DEPTH; ++d) {
+            const int nx = (d + DEPTH - 1) % DEPTH;
+            R[nx][0] = load(pop(H[nx][0], C[nx][0]));       // gathers for a later pair ...
+            R[nx][1] = load(pop(H[nx][1], C[nx][1]));
+            compute(R[d][0], R[d][1], H[d][0], H[d][1], C[d][0], C[d][1], std::integral_constant<bool, PER>{});   // ... while this one is evaluated
+        }
+        if (!__any_sync(SPH_FULL_MASK, H[0][0])) break;   // pops are in order: no pending candidate here means none at all
     }
     __syncwarp();
 }
