@@ -155,6 +155,7 @@ enum sph_kernel_id {
     SPH_K_ACCEL_LIST = 9,       /* a6 + a7 replayed over the candidate masks recorded by the search */
     SPH_K_SEARCH = 10,          /* neighbour search of one sorted order: tensor-core filter -> mask records */
     SPH_K_DENSITY_LIST = 11,    /* a4 + a5 replayed over the candidate masks recorded by the search */
+    SPH_K_UPDATE_KICK = 12,     /* a8, eq.14 only (the launch that ends a sph_pc_step call): no drift, no key */
     SPH_K_COUNT = 16
 };
 typedef struct sph_profile {
@@ -240,6 +241,12 @@ int sph_synchronize(sph_ctx* ctx);   /* [sync] waits for the stream and reports 
  * 8 blocks of 256 threads per SM.  *tflops counts 2 flop per lane FMA; *ms (nullable) is the best of 3 timed
  * launches.  It is the measured denominator of the pair kernels' ALU roofline.  [sync] */
 int sph_fp32_probe(sph_ctx* ctx, int packed, int iters, double* tflops, double* ms);
+
+/* Diagnostic, not a step of the path: the size of the candidate set of the PAPER's cell-list search on the current
+ * state -- sum over all particles of the population of the 3^d cells of size >= k*h_max around them (L158, one
+ * uniform grid sized by h_max).  It is the work unit the roofline report charges a searching pass with, whatever
+ * this library really tests (sph_stats.candidates*).  Positions in the cell-sorted mirror are used.  [sync] */
+int sph_stencil_candidates(sph_ctx* ctx, int64_t* out);
 
 const char* sph_strerror(int code);
 const char* sph_last_error(const sph_ctx* ctx);

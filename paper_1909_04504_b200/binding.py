@@ -26,7 +26,7 @@ ARRAY_DYNAMIC, ARRAY_FIXED = 0, 1
 EXPORTS = ["sph_create", "sph_destroy", "sph_set_tables", "sph_nnps_build", "sph_summation_density",
            "sph_wcsph_accel", "sph_pc_step", "sph_sync_state", "sph_get_accel", "sph_nnps_get_neighbors",
            "sph_get_stats", "sph_synchronize", "sph_strerror", "sph_last_error", "sph_abi_version",
-           "sph_set_profiling", "sph_get_profile", "sph_kernel_name", "sph_fp32_probe"]
+           "sph_set_profiling", "sph_get_profile", "sph_kernel_name", "sph_fp32_probe", "sph_stencil_candidates"]
 
 _FP = C.POINTER(C.c_float)
 FIELD_NAMES = ("x", "y", "z", "u", "v", "w", "h", "m", "rho", "p", "ax", "ay", "az", "arho")
@@ -98,6 +98,7 @@ def load() -> C.CDLL:
         L.sph_get_profile.argtypes = [vp, C.POINTER(sph_profile)]
         L.sph_kernel_name.argtypes = [i32]; L.sph_kernel_name.restype = C.c_char_p
         L.sph_fp32_probe.argtypes = [vp, i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.sph_stencil_candidates.argtypes = [vp, C.POINTER(i64)]
         L.sph_strerror.argtypes = [i32]; L.sph_strerror.restype = C.c_char_p
         L.sph_last_error.argtypes = [vp]; L.sph_last_error.restype = C.c_char_p
         for name in EXPORTS:
@@ -277,6 +278,12 @@ class SphContext:
 
     def set_profiling(self, enable: bool):
         self._check(self.L.sph_set_profiling(self.ctx, int(bool(enable))))
+
+    def stencil_candidates(self) -> int:
+        """Candidate-set size of the paper's own cell-list search (3^d cells >= k h_max) on the current state."""
+        out = C.c_int64(0)
+        self._check(self.L.sph_stencil_candidates(self.ctx, C.byref(out)))
+        return int(out.value)
 
     def fp32_probe(self, packed: bool, iters: int = 4096):
         """(TFLOP/s, ms) of the FP32 FMA issue-rate probe (diagnostic; the ALU roofline denominator)."""

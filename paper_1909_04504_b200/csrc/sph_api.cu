@@ -26,6 +26,10 @@ extern "C" const char* sph_strerror(int code) {
 extern "C" const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context"; }
 extern "C" int sph_abi_version(void) { return SPH_ABI_VERSION; }
 
+static void drop_graph(sph_ctx* c) {
+    if (c->step_graph) { cudaGraphExecDestroy(c->step_graph); c->step_graph = nullptr; }
+}
+
 static void default_tables(sph_ctx* c) {
     uint32_t all = (1u << c->na) - 1u, dyn = 0;
     for (int a = 0; a < c->na; ++a) if (!c->fixed[a]) dyn |= 1u << a;
@@ -111,8 +115,8 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     const size_t scan_n = (size_t)(c->max_keys > tot ? c->max_keys : tot) + 2;
     SPH_CUDA_OK(c, cudaMalloc(&c->scan_state, (scan_n / 2048 + 4) * sizeof(unsigned long long)));
     SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_state, 0, (scan_n / 2048 + 4) * sizeof(unsigned long long), c->stream));
-    SPH_CUDA_OK(c, cudaMalloc(&c->scan_ticket, sizeof(uint32_t)));
-    SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_ticket, 0, sizeof(uint32_t), c->stream));
+    SPH_CUDA_OK(c, cudaMalloc(&c->scan_ticket, 2 * sizeof(uint32_t)));
+    SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_ticket, 0, 2 * sizeof(uint32_t), c->stream));
     SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(float)));
     SPH_CUDA_OK(c, cudaMalloc(&c->counters, CNT_COUNT * sizeof(unsigned long long)));
     SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 4 * sizeof(float)));
@@ -140,6 +144,7 @@ extern "C" int sph_destroy(sph_ctx* c) {
     cudaFree(c->S[0].acc); cudaFree(c->S[1].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
     cudaFree(c->nl.pool); cudaFree(c->nl.head);
     cudaFree(c->scan_state); cudaFree(c->scan_ticket); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
+    if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
     for (int k = 0; k < c->prof_cap; ++k) { cudaEventDestroy(c->prof[k].a); cudaEventDestroy(c->prof[k].b); }
     free(c->prof);
     delete c;
@@ -154,6 +159,7 @@ extern "C" int sph_set_tables(sph_ctx* c, const uint32_t* density_src, const uin
     for (int t = 0; t < 3; ++t) if (in[t]) for (int a = 0; a < c->na; ++a) if (in[t][a] & ~all) return sph_fail(c, SPH_ERR_BAD_ARG, "source mask names a non-existent array");
     for (int t = 0; t < 3; ++t) if (in[t]) for (int a = 0; a < c->na; ++a) dst[t][a] = in[t][a];
     c->tables_user = true;
+    drop_graph(c);
     return SPH_OK;
 }
 
@@ -230,6 +236,8 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     if (!c || !arrays) return SPH_ERR_NULL;
     if (n_arrays != c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "n_arrays differs from sph_create");
     c->built = false; c->have_accel = false; c->have_arho = false; c->nl_valid = false;
+    c->counters_fresh = false; c->heads_fresh = false;
+    drop_graph(c);
     int64_t tot = 0;
     bool all_acc = true, all_arho = true, any_p = false;
     for (int a = 0; a < c->na; ++a) {
@@ -352,7 +360,8 @@ extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float
 static int evaluate(sph_ctx* c, bool continuity) {
     int rc;
     rc = ensure_search(c); if (rc) return rc;
-    rc = zero_counters(c, CNT_PAIRS_DENSITY, CNT_CAND_ACCEL); if (rc) return rc;
+    if (!c->counters_fresh) { rc = zero_counters(c, CNT_PAIRS_DENSITY, CNT_CAND_ACCEL); if (rc) return rc; }   // (k_update clears them inside a step)
+    c->counters_fresh = false;
     auto grouped = [&](const uint32_t* tbl, const bool* take, auto&& fn) -> int {
         bool done[SPH_MAX_ARRAYS] = { false, false, false, false };
         for (int a = 0; a < c->na; ++a) {
@@ -412,6 +421,38 @@ static int evaluate(sph_ctx* c, bool continuity) {
     return SPH_OK;
 }
 
+// one step of the loop of sph_pc_step.   PC: (14 of the previous step) + 12 + 13 + key.   Euler: x += dt u ; u += dt a ;
+// rho += dt arho ; key.   Then the sort (NNPS rebuilt every step, L443) and the evaluation.
+static int step_body(sph_ctx* c, float dt, bool cont, bool kick2) {
+    int rc = nnps_update_key_hist(c, dt, kick2, true, cont, true); if (rc) return rc;
+    rc = nnps_sort_from_keys(c, false); if (rc) return rc;
+    rc = evaluate(c, cont); if (rc) return rc;
+    c->have_arho = cont;
+    return SPH_OK;
+}
+
+// Captures TWO consecutive middle steps (the state buffers flip every step, so two steps return to the same
+// buffers) into a CUDA graph: long runs of small problems are bound by launch latency, not by work.
+static bool ensure_step_graph(sph_ctx* c, float dt, bool cont, bool kick2) {
+    if (c->graph_off) return false;
+    if (c->step_graph && c->graph_dt == dt && c->graph_cont == (cont ? 1 : 0) && c->graph_cur == c->cur) return true;
+    drop_graph(c);
+    const int64_t l0 = c->launches;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); c->graph_off = true; return false; }
+    int rc = step_body(c, dt, cont, kick2);
+    if (!rc) rc = step_body(c, dt, cont, kick2);
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    c->graph_nodes = (int)(c->launches - l0);
+    c->launches = l0;                                   // nothing ran: the captured launches are counted per replay
+    if (rc || e != cudaSuccess || !graph) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); c->graph_off = true; return false; }
+    const cudaError_t e2 = cudaGraphInstantiate(&c->step_graph, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e2 != cudaSuccess) { c->step_graph = nullptr; cudaGetLastError(); c->graph_off = true; return false; }
+    c->graph_dt = dt; c->graph_cont = cont ? 1 : 0; c->graph_cur = c->cur;
+    return true;
+}
+
 extern "C" int sph_pc_step(sph_ctx* c, double dt, int n_steps, int density_mode) {
     if (!c) return SPH_ERR_NULL;
     if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
@@ -423,14 +464,16 @@ extern "C" int sph_pc_step(sph_ctx* c, double dt, int n_steps, int density_mode)
         rc = evaluate(c, cont); if (rc) return rc; c->have_accel = true; c->have_arho = cont;
     }
     const bool euler = c->prm.integrator == SPH_INTEGRATOR_EULER;
-    for (int s = 0; s < n_steps; ++s) {
-        // PC: (14 of step s-1) + 12 + 13 + key.   Euler: x += dt u ; u += dt a ; rho += dt arho ; key.
-        rc = nnps_update_key_hist(c, (float)dt, !euler && s > 0, true, cont, true); if (rc) return rc;
-        rc = nnps_sort_from_keys(c, false); if (rc) return rc;                                  // NNPS rebuilt every step (L443)
-        rc = evaluate(c, cont); if (rc) return rc;
-        c->have_arho = cont;
-        c->steps_done++;
+    int s = 0;
+    if (n_steps > 0) { rc = step_body(c, (float)dt, cont, false); if (rc) return rc; c->steps_done++; s = 1; }
+    // long runs: replay a captured pair of steps (same kernels, same arguments, one graph launch per two steps)
+    if (n_steps - s >= 8 && !c->prof_on && c->n_total > 0 && ensure_step_graph(c, (float)dt, cont, !euler)) {
+        while (n_steps - s >= 2) {
+            SPH_CUDA_OK(c, cudaGraphLaunch(c->step_graph, c->stream));
+            c->launches += c->graph_nodes; c->steps_done += 2; s += 2;
+        }
     }
+    for (; s < n_steps; ++s) { rc = step_body(c, (float)dt, cont, !euler); if (rc) return rc; c->steps_done++; }
     if (n_steps > 0 && !euler) { rc = nnps_update_key_hist(c, (float)dt, true, false, cont, false); if (rc) return rc; }   // eq.14
     return SPH_OK;
 }
@@ -460,6 +503,12 @@ extern "C" int sph_nnps_get_neighbors(sph_ctx* c, int dest, int src, int64_t* of
     if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
     if (dest < 0 || dest >= c->na || src < 0 || src >= c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / src");
     return nnps_export_neighbors(c, dest, src, offsets, indices, cap, total, mem);
+}
+
+extern "C" int sph_stencil_candidates(sph_ctx* c, int64_t* out) {
+    if (!c || !out) return SPH_ERR_NULL;
+    if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
+    return nnps_stencil_candidates(c, out);
 }
 
 static int read_counters(sph_ctx* c, unsigned long long* h) {
@@ -570,6 +619,7 @@ extern "C" const char* sph_kernel_name(int id) {
         case SPH_K_ACCEL_LIST: return "k_accel_list";
         case SPH_K_SEARCH: return "k_search";
         case SPH_K_DENSITY_LIST: return "k_density_list";
+        case SPH_K_UPDATE_KICK: return "k_update_kick";
     }
     return "";
 }

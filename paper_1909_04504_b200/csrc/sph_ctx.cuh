@@ -32,7 +32,7 @@ struct sph_ctx {
     int cur;
     uint32_t *key, *rank;      // per particle, pre-sort order
     uint32_t *cell_count, *cell_start;
-    unsigned long long* scan_state; uint32_t* scan_ticket; uint32_t scan_epoch;   // k_scan look-back table
+    unsigned long long* scan_state; uint32_t* scan_ticket;   // k_scan look-back table; scan_ticket[0] = ticket, [1] = epoch
     float* staging;            // host<->device staging for SPH_MEM_HOST (10 floats per particle of capacity)
     unsigned long long* counters;     // device, CNT_COUNT entries
     float* hminmax;            // device, 4 floats (as ordered ints): h min/max, |m| min/max
@@ -41,6 +41,10 @@ struct sph_ctx {
     NList nl;                  // nl.pool == nullptr: recording disabled
     bool nl_valid;             // the records match the current sorted order (launch_search ran since the last sort)
     bool last_used_rows;       // the last acceleration launch replayed recorded rows
+    bool counters_fresh;       // k_update has just cleared the counters of the search and the pair passes (consumed by evaluate)
+    bool heads_fresh;          // k_scatter has just cleared the record heads (consumed by launch_search)
+    // CUDA graph of two consecutive steps of sph_pc_step (the state buffers flip every step), replayed for long runs
+    cudaGraphExec_t step_graph; float graph_dt; int graph_cont, graph_cur, graph_nodes; bool graph_off;
     bool xsub_auto;            // xsub was not given: 6, or 16 when h varies
     int xsub;                  // x sub-cells per support radius requested (GridDesc::xsub is what the grid got)
 
@@ -83,6 +87,7 @@ int nnps_key_hist(sph_ctx* c);                       // key + rank + histogram f
 int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey);
 int nnps_sort_from_keys(sph_ctx* c, bool with_acc);  // scan + scatter (key/rank/cell_count filled); swaps buffers
 int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O);
+int nnps_stencil_candidates(sph_ctx* c, int64_t* out);
 int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32_t* indices, int64_t cap,
                           int64_t* total, int mem);
 // sph_density.cu / sph_accel.cu: one launch serves every dest array whose mask is non-zero

@@ -80,7 +80,7 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
 // way on EVERY array (the tank particles too, L142) and re-evaluates the EOS (group 1 of Listing 3).
 // ------------------------------------------------------------------------------------------------
 struct UpdateArgs {
-    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho, w_prr, euler;
+    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho, w_prr, euler, zero_cnt;
     int fixed[SPH_MAX_ARRAYS];
 };
 
@@ -89,6 +89,9 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
          uint32_t* __restrict__ key, uint32_t* __restrict__ rank, uint32_t* __restrict__ cell_count,
          unsigned long long* __restrict__ counters) {
     const int i = blockIdx.x * NB + threadIdx.x;
+    // inside sph_pc_step this launch precedes the search and the pair passes of the step: it clears their counters
+    // (no separate memset node per step)
+    if (U.zero_cnt && i < CNT_COUNT - CNT_PAIRS_DENSITY) counters[CNT_PAIRS_DENSITY + i] = 0ull;
     if (i >= n) return;
     float4 pos = S.posh[i];
     const uint32_t meta = S.meta[i];
@@ -168,14 +171,18 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
 // Single-pass scan with decoupled look-back: tile t publishes its aggregate, then warp 0 sums the aggregates of
 // its predecessors, 32 at a time, back to the nearest tile whose inclusive prefix is already known.  Tiles take
 // their number from a ticket, so every predecessor of a running tile is running or done (no deadlock).  A state
-// word is {epoch-tagged flag, value}; the epoch changes with every scan, so the table is never cleared.
+// word is {epoch-tagged flag, value}; the epoch (a device word) changes with every scan, so the table is never cleared.
 __global__ void __launch_bounds__(SCAN_T)
 k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int nb,
-       unsigned long long* __restrict__ state, uint32_t* __restrict__ ticket, uint32_t epoch, int zero_in) {
-    __shared__ uint32_t s_tile, s_total, s_prefix;
-    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+       unsigned long long* __restrict__ state, uint32_t* __restrict__ ticket, int zero_in) {
+    __shared__ uint32_t s_tile, s_total, s_prefix, s_epoch;
+    if (threadIdx.x == 0) {
+        s_epoch = *(volatile uint32_t*)(ticket + 1) + 1u;      // the epoch lives on the device (ticket[1]) so that a captured
+        __threadfence_block();                                 // launch can be replayed; read BEFORE the ticket is taken: the
+        s_tile = atomicAdd(ticket, 1u);                        // last tile bumps it only after every tile holds a ticket
+    }
     __syncthreads();
-    const uint32_t tile = s_tile;
+    const uint32_t tile = s_tile, epoch = s_epoch;
     const long long i0 = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
     uint32_t v[SCAN_ITEMS], s = 0;
 #pragma unroll
@@ -211,7 +218,9 @@ k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int n
         if (lane == 0) {
             vs[tile] = ((unsigned long long)F_INC << 32) | (prefix + total);
             s_prefix = prefix;
-            if ((int)tile == nb - 1) { out[n] = prefix + total; *ticket = 0u; }   // last tile: grand total, ticket reset
+            if ((int)tile == nb - 1) {                                  // last tile: grand total, ticket reset, next epoch
+                out[n] = prefix + total; ticket[1] = epoch >= 0x3ffffff0u ? 0u : epoch; ticket[0] = 0u;
+            }
         }
     }
     __syncthreads();
@@ -223,15 +232,14 @@ k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int n
 static int scan_exclusive(sph_ctx* c, uint32_t* in, uint32_t* out, long long n, bool zero_in) {
     const int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
     if (nb == 0) { SPH_CUDA_OK(c, cudaMemsetAsync(out, 0, sizeof(uint32_t), c->stream)); return SPH_OK; }
-    c->scan_epoch = c->scan_epoch >= 0x3fffffffu ? 1u : c->scan_epoch + 1u;
-    SPH_LAUNCH(c, SPH_K_SCAN, k_scan, nb, SCAN_T, 0, in, n, out, nb, c->scan_state, c->scan_ticket, c->scan_epoch, zero_in ? 1 : 0);
+    SPH_LAUNCH(c, SPH_K_SCAN, k_scan, nb, SCAN_T, 0, in, n, out, nb, c->scan_state, c->scan_ticket, zero_in ? 1 : 0);
     return SPH_OK;
 }
 
 // a3: gather every persistent property into cell order (double buffer A -> B).
 __global__ void __launch_bounds__(NB)
 k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass, const uint32_t* __restrict__ key,
-          const uint32_t* __restrict__ rank, const uint32_t* __restrict__ cell_start) {
+          const uint32_t* __restrict__ rank, const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nl_head) {
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
     const uint32_t k = key[i];
@@ -247,6 +255,7 @@ k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass,
     B.rp[d] = r;
     B.meta[d] = A.meta[i];
     B.cell[d] = k / (uint32_t)na;
+    if (nl_head && (d & 31u) == 0u) nl_head[d >> 5] = 0u;          // the records of the old order are void: clear the heads for the next search
     if (with_acc) B.acc[d] = A.acc[i];
 }
 
@@ -259,15 +268,17 @@ int nnps_key_hist(sph_ctx* c) {
 }
 
 int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey) {
+    const bool kick_only = kick2 && !kick1_drift;
     const int n = (int)c->n_total;
     UpdateArgs U;
     U.euler = c->prm.integrator == SPH_INTEGRATOR_EULER ? 1 : 0;
     U.dt_half = U.euler ? dt : 0.5f * dt;              // Euler: the one kick per step is a full dt
     U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
-    U.continuity = continuity; U.rekey = rekey; U.w_rho = (!c->variable_h || c->pc.varh_um) ? 1 : 0; U.w_prr = (!c->variable_h && c->pc.uniform_m) ? 1 : 0;
+    U.continuity = continuity; U.rekey = rekey; U.zero_cnt = rekey ? 1 : 0; U.w_rho = (!c->variable_h || c->pc.varh_um) ? 1 : 0; U.w_prr = (!c->variable_h && c->pc.uniform_m) ? 1 : 0;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
-    if (n) SPH_LAUNCH(c, SPH_K_UPDATE, k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
+    if (n) SPH_LAUNCH(c, (kick_only ? SPH_K_UPDATE_KICK : SPH_K_UPDATE), k_update, (n + NB - 1) / NB, NB, 0, c->grid, c->pc, c->S[c->cur], n, U, c->key, c->rank,
                       c->cell_count, c->counters);
+    if (n && rekey) c->counters_fresh = true;
     return SPH_OK;
 }
 
@@ -276,7 +287,8 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys, true);   // leaves cell_count cleared
     if (rc) return rc;
     if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
-                      with_acc ? 1 : 0, !with_acc ? 0 : (c->variable_h ? (c->pc.varh_um ? 3 : 0) : (c->pc.uniform_m ? 2 : 1)), c->key, c->rank, c->cell_start);
+                      with_acc ? 1 : 0, !with_acc ? 0 : (c->variable_h ? (c->pc.varh_um ? 3 : 0) : (c->pc.uniform_m ? 2 : 1)), c->key, c->rank, c->cell_start, c->nl.head);
+    c->heads_fresh = n > 0 && c->nl.head != nullptr;
     c->cur ^= 1;
     c->nl_valid = false;                 // recorded neighbour rows index the previous sorted order
     return SPH_OK;
@@ -408,5 +420,66 @@ int nnps_pack(sph_ctx* c, const PackArgs& A) {
     const int init[4] = { 0x7f7fffff, 0, 0x7f7fffff, 0 };
     SPH_CUDA_OK(c, cudaMemcpyAsync(c->hminmax, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
     if (n) SPH_LAUNCH(c, SPH_K_PACK, k_pack, (n + NB - 1) / NB, NB, 0, A, c->S[c->cur], n, c->pc, (int*)c->hminmax);
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Diagnostic: size of the candidate set of the PAPER's cell-list search (L158: "3^d neighbouring boxes" of a
+// uniform grid with cells >= k h_max): sum over particles of the population of the 3^d coarse cells around them.
+// It is the algorithmic work unit of the searching passes in the roofline report.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void coarse_coords(const GridDesc& g, float4 p, int (&c)[3], int (&nc)[3]) {
+    const LevelDesc& Lv = g.lev[g.nlev - 1];
+    nc[0] = Lv.nc[0] / Lv.xsub; nc[1] = Lv.nc[1]; nc[2] = Lv.nc[2];
+    c[0] = cell_coord(p.x, g.lo[0], Lv.inv_cell[0], Lv.nc[0]) / Lv.xsub;
+    c[1] = cell_coord(p.y, g.lo[1], Lv.inv_cell[1], Lv.nc[1]);
+    c[2] = g.dim == 3 ? cell_coord(p.z, g.lo[2], Lv.inv_cell[2], Lv.nc[2]) : 0;
+}
+__global__ void __launch_bounds__(NB)
+k_coarse_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ cnt) {
+    const int i = blockIdx.x * NB + threadIdx.x;
+    if (i >= n) return;
+    int c[3], nc[3];
+    coarse_coords(g, S.posh[i], c, nc);
+    atomicAdd(&cnt[(c[2] * nc[1] + c[1]) * nc[0] + c[0]], 1u);
+}
+__global__ void __launch_bounds__(NB)
+k_coarse_sum(GridDesc g, SortedState S, int n, const uint32_t* __restrict__ cnt, unsigned long long* __restrict__ out) {
+    const int i = blockIdx.x * NB + threadIdx.x;
+    unsigned long long sum = 0ull;
+    if (i < n) {
+        int c[3], nc[3];
+        coarse_coords(g, S.posh[i], c, nc);
+        for (int dz = (g.dim == 3 ? -1 : 0); dz <= (g.dim == 3 ? 1 : 0); ++dz)
+            for (int dy = -1; dy <= 1; ++dy)
+                for (int dx = -1; dx <= 1; ++dx) {
+                    int q[3] = { c[0] + dx, c[1] + dy, c[2] + dz }; bool ok = true;
+                    for (int a = 0; a < 3; ++a) {
+                        if (q[a] < 0) { if (g.per[a]) q[a] += nc[a]; else ok = false; }
+                        else if (q[a] >= nc[a]) { if (g.per[a]) q[a] -= nc[a]; else ok = false; }
+                    }
+                    if (ok) sum += cnt[(q[2] * nc[1] + q[1]) * nc[0] + q[0]];
+                }
+    }
+    sum = warp_sum_u64(sum);
+    if ((threadIdx.x & 31) == 0 && sum) atomicAdd(out, sum);
+}
+
+int nnps_stencil_candidates(sph_ctx* c, int64_t* out) {
+    const int n = (int)c->n_total;
+    *out = 0;
+    if (n == 0) return SPH_OK;
+    const LevelDesc& Lv = c->grid.lev[c->grid.nlev - 1];
+    const size_t cells = (size_t)(Lv.nc[0] / Lv.xsub) * Lv.nc[1] * Lv.nc[2];
+    unsigned long long* acc = (unsigned long long*)c->hminmax;                     // 16 bytes of scratch, idle between builds
+    uint32_t* cnt = c->cell_count;                                                 // all zero between sorts; cleared again below
+    SPH_CUDA_OK(c, cudaMemsetAsync(acc, 0, sizeof(unsigned long long), c->stream));
+    SPH_LAUNCH(c, SPH_K_NEIGHBORS, k_coarse_hist, (n + NB - 1) / NB, NB, 0, c->grid, c->S[c->cur], n, cnt);
+    SPH_LAUNCH(c, SPH_K_NEIGHBORS, k_coarse_sum, (n + NB - 1) / NB, NB, 0, c->grid, c->S[c->cur], n, cnt, acc);
+    SPH_CUDA_OK(c, cudaMemsetAsync(cnt, 0, cells * sizeof(uint32_t), c->stream));
+    unsigned long long h = 0;
+    SPH_CUDA_OK(c, cudaMemcpyAsync(&h, acc, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    *out = (int64_t)h;
     return SPH_OK;
 }

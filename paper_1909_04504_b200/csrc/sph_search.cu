@@ -31,8 +31,11 @@ int launch_search(sph_ctx* c) {
     c->nl_valid = false;
     const int n = (int)c->n_total;
     if (c->nl.pool == nullptr || n == 0) return SPH_OK;
-    SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.head, 0, (size_t)((c->n_total + 31) / 32 + 1) * sizeof(uint32_t), c->stream));
-    SPH_CUDA_OK(c, cudaMemsetAsync(c->counters + CNT_OVERFLOW, 0, (size_t)(CNT_CAND_SEARCH - CNT_OVERFLOW + 1) * sizeof(unsigned long long), c->stream));
+    if (!c->heads_fresh)           // (inside sph_pc_step k_scatter and k_update have already cleared both)
+        SPH_CUDA_OK(c, cudaMemsetAsync(c->nl.head, 0, (size_t)((c->n_total + 31) / 32 + 1) * sizeof(uint32_t), c->stream));
+    if (!c->counters_fresh)
+        SPH_CUDA_OK(c, cudaMemsetAsync(c->counters + CNT_OVERFLOW, 0, (size_t)(CNT_CAND_SEARCH - CNT_OVERFLOW + 1) * sizeof(unsigned long long), c->stream));
+    c->heads_fresh = false;
     const int grid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
     SortedState& S = c->S[c->cur];
 #define LS(DIM, VARH) SPH_LAUNCH(c, SPH_K_SEARCH, (k_search_tile<DIM, VARH>), grid, TILE_BLOCK, 0, c->grid, c->pc, S, c->cell_start, n, c->nl, c->counters)

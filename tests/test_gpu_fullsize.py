@@ -1,5 +1,5 @@
 """-m gpu parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one context, device
-arrays, default tuning), on SAMPLED destination particles the oracle computes one by one (full
+arrays, default tuning: default record pool, default levels; C5 additionally with no pool), on SAMPLED destination particles the oracle computes one by one (full
 runs of the fp64 oracle take minutes to hours at these sizes), plus properties that hold at any size.
 
 For every config the oracle evaluates eq.3 / eq.8-9 (+ eq.7) for a seeded sample of destination particles
@@ -17,6 +17,10 @@ from gpu_helpers import TOL, make_ctx, mask_of
 pytestmark = pytest.mark.gpu
 
 N_SAMPLE = 4096
+
+
+def min_image(d, L=1.0):
+    return d - L * np.rint(d / L)
 
 
 def _sample(n, k, seed):
@@ -110,7 +114,7 @@ def test_c3_full_density_accel_and_counts(O, WL):
     st2 = _gpu_state_into(O, wl, ctx)
     _check_accel(O, wl, ctx, st2, 0, [0], seed=101, want_arho=False)
     s = ctx.get_stats()
-    assert s.used_rows == 1                       # the momentum pass replayed the density pass's hit masks
+    assert s.used_rows == 1                       # the momentum pass replayed the records of the one search
     assert s.pairs_accel == pairs_gpu             # ... and saw exactly the same pairs
     # every sampled particle has exactly the oracle's neighbour count (exact sets are gated on the small cases)
     sub = _sample(wl.arrays[0].n, N_SAMPLE, 102)
@@ -195,20 +199,58 @@ def test_c4_full_two_arrays(O, WL):
     ctx.close(); ctx2.close()
 
 
-def test_c5_full_variable_h(O, WL):
+@pytest.mark.parametrize("pool", ["default_pool", "no_pool"])
+def test_c5_full_variable_h(O, WL, pool):
+    """C5 in the configuration bench.py times (default record pool: one search, both pair passes replay; level
+    grids) and with no pool (every pair pass searches itself)."""
     wl = WL.gaussian_mixture_3d()
     assert wl.arrays[0].n == 1 << 24
-    ctx, _ = make_ctx(wl, nlist_slots=-1)         # every pair pass searches (hit masks of 5e3 tests per particle
-                                                  # would need > 25 KB per warp)
+    ctx, _ = make_ctx(wl, nlist_slots=(0 if pool == "default_pool" else -1))
     st = O.State(wl)
     _check_density(O, wl, ctx, st, seed=130, abs_gate=True)
     st2 = _gpu_state_into(O, wl, ctx)
     _check_accel(O, wl, ctx, st2, 0, [0], seed=131, want_arho=False, abs_gate=True)
     s = ctx.get_stats()
-    assert s.variable_h == 1 and s.used_rows == 0
+    assert s.variable_h == 1 and s.n_levels >= 2
+    if pool == "default_pool":
+        assert s.used_rows == 1 and s.nlist_fallback_warps == 0 and s.candidates_accel == 0
+        assert s.candidates_search / wl.arrays[0].n <= 1000.0          # f3: not the ~2,650 (r1) / ~4,800 (one grid) per particle
+        print(f"C5 default pool: {s.candidates_search / wl.arrays[0].n:.0f} candidates per particle, "
+              f"{s.nlist_rows_used} of {s.nlist_rows_capacity} record rows, fallback warps {s.nlist_fallback_warps}, levels {s.n_levels}")
+    else:
+        assert s.used_rows == 0 and s.candidates_accel > 0
     assert s.pairs_accel == s.pairs_density
     sub = _sample(wl.arrays[0].n, N_SAMPLE, 132)
     assert np.array_equal(ctx.neighbor_counts(0, 0)[sub], _rows_count(O, wl, st, 0, [0], sub))
+    ctx.synchronize()
+    ctx.close()
+
+
+def test_c3_full_state_after_100_steps(O, WL):
+    """A15 at full size: the C3 state after its 100 steps (ragged cells, the state bench.py times) goes back through
+    the C ABI as a new build; density, momentum and neighbour counts of sampled particles against the oracle."""
+    import copy
+    wl = WL.periodic_box_3d((128, 128, 128), seed=1, dx=1.0 / 128)
+    ctx, _ = make_ctx(wl)
+    ctx.pc_step(wl.dt, 100, "summation")
+    ctx.synchronize()
+    out = {k: v.cpu().numpy() for k, v in ctx.sync_state(0).items()}
+    ctx.close()
+    wl2 = copy.deepcopy(wl)
+    for k in ("x", "y", "z", "u", "v", "w", "rho"):
+        setattr(wl2.arrays[0], k, np.ascontiguousarray(out[k], dtype=np.float32))
+    moved = np.abs(min_image(out["x"] - wl.arrays[0].x)).max() * 128
+    assert moved > 0.3, moved                                     # in units of dx
+    ctx, _ = make_ctx(wl2)
+    st = O.State(wl2)
+    _check_density(O, wl2, ctx, st, seed=140)
+    pairs = ctx.get_stats().pairs_density
+    st2 = _gpu_state_into(O, wl2, ctx)
+    _check_accel(O, wl2, ctx, st2, 0, [0], seed=141, want_arho=False)
+    s = ctx.get_stats()
+    assert s.used_rows == 1 and s.pairs_accel == pairs
+    sub = _sample(wl2.arrays[0].n, N_SAMPLE, 142)
+    assert np.array_equal(ctx.neighbor_counts(0, 0)[sub], _rows_count(O, wl2, st, 0, [0], sub))
     ctx.synchronize()
     ctx.close()
 

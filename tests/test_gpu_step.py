@@ -108,7 +108,8 @@ def test_record_pool_overflow_falls_back_to_searching(WL):
 @pytest.mark.parametrize("name", ["dam2d_euler_laminar", "3d_per_euler_laminar", "3d_varh_pc_laminar"])
 def test_laminar_viscosity_and_euler_steps(O, WL, name):
     """eq.10 in the pair loop (nu > 0) and the forward-Euler integrator of the paper's worked example (L335,
-    Fig.2): a^0 + two steps on the GPU == the oracle's, from the same state (second step from the GPU's state)."""
+    Fig.2): a^0 + ONE step on the GPU == the oracle's, from the same state (steps from an evolved state:
+    test_gpu_evolved.py)."""
     if name == "dam2d_euler_laminar":
         wl, mode = WL.dam_break_2d(dx=0.04), "continuity"
         wl.integrator, wl.nu = "euler", 1.0e-3
