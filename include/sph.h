@@ -12,7 +12,11 @@
  *   - groups are barriers: the EOS of ALL arrays completes before the momentum equation (L337).
  *
  * Conventions
- *   real type      float (the paper's GPU runs are single precision, L733).
+ *   real type      sph_real = float (the paper's GPU runs are single precision, L733): libsph_b200.so.  The same sources
+ *                  built with -DSPH_REAL_DOUBLE give libsph_b200_f64.so with sph_real = double (north_star: "1e-12
+ *                  for an fp64 build flag"): the same calls, every particle buffer in double; sph_real_size() tells
+ *                  which one was loaded.  There the neighbour search still runs in float on float-rounded positions
+ *                  (it is conservative), the exact predicate and all field arithmetic in double.
  *   pointers       every particle buffer is CALLER-OWNED.  `mem` says where it lives: SPH_MEM_DEVICE
  *                  (device pointers on the context's device) or SPH_MEM_HOST (host pointers; the library
  *                  copies through its own staging buffers with cudaMemcpyAsync on the context stream --
@@ -36,6 +40,12 @@
 
 #ifdef __cplusplus
 extern "C" {
+#endif
+
+#ifdef SPH_REAL_DOUBLE
+typedef double sph_real;
+#else
+typedef float sph_real;
 #endif
 
 #define SPH_MAX_ARRAYS 4
@@ -107,13 +117,13 @@ typedef struct sph_array {      /* one named particle array (L316) */
     int64_t n;
     int flags;                  /* enum sph_array_flags */
     int mem;                    /* enum sph_mem: where the pointers below live */
-    float *x, *y, *z;           /* positions      (z NULL allowed when dim == 2) */
-    float *u, *v, *w;           /* velocities     (w NULL allowed when dim == 2; all NULL -> 0) */
-    float *h;                   /* smoothing length; sets the search radius (L316) */
-    float *m;                   /* mass           (NULL -> 0: array only queries, never a source of mass) */
-    float *rho;                 /* density        (NULL -> rho0) */
-    float *p;                   /* pressure       (NULL -> EOS(rho)) */
-    float *ax, *ay, *az, *arho; /* accelerations of the last evaluation: the paper's au, av, aw, arho properties
+    sph_real *x, *y, *z;        /* positions      (z NULL allowed when dim == 2) */
+    sph_real *u, *v, *w;        /* velocities     (w NULL allowed when dim == 2; all NULL -> 0) */
+    sph_real *h;                /* smoothing length; sets the search radius (L316) */
+    sph_real *m;                /* mass           (NULL -> 0: array only queries, never a source of mass) */
+    sph_real *rho;              /* density        (NULL -> rho0) */
+    sph_real *p;                /* pressure       (NULL -> EOS(rho)) */
+    sph_real *ax, *ay, *az, *arho; /* accelerations of the last evaluation: the paper's au, av, aw, arho properties
                                  * (L402-418).  Input to sph_nnps_build (restart: if every dynamic array gives
                                  * ax,ay,(az) -- and, for continuity mode, every array gives arho -- the first
                                  * sph_pc_step reuses them as a^n instead of re-evaluating); output of sph_sync_state.
@@ -192,15 +202,15 @@ int sph_nnps_build(sph_ctx* ctx, int n_arrays, const sph_array* arrays);
 
 /* Summation density, eq.3 (L112): rho_i = sum_{b in source_mask} sum_{j in N_b(i)} m_j W(r_ij, h_ij) for
  * every particle i of array `dest`, self pair included; then the EOS (eq.6) on that array.  Updates the
- * context's rho/p of `dest` and, if non-NULL, writes rho_out / p_out (n_dest floats, caller order, `mem`). */
-int sph_summation_density(sph_ctx* ctx, int dest, uint32_t source_mask, float* rho_out, float* p_out, int mem);
+ * context's rho/p of `dest` and, if non-NULL, writes rho_out / p_out (n_dest reals, caller order, `mem`). */
+int sph_summation_density(sph_ctx* ctx, int dest, uint32_t source_mask, sph_real* rho_out, sph_real* p_out, int mem);
 
 /* WCSPH acceleration, eq.8-9 (L128-132) + artificial viscosity + optional continuity RHS eq.7 (L126):
  *   a_i = g - sum_b sum_j m_j (p_i/rho_i^2 + p_j/rho_j^2 + Pi_ij) grad_i W_ij,   arho_i = sum m_j v_ij . grad_i W_ij
  * from the context's current rho,p (as loaded by sph_nnps_build or computed by sph_summation_density).
  * ax,ay,az (az may be NULL when dim == 2) and arho (NULL: not computed) receive n_dest floats, caller order. */
 int sph_wcsph_accel(sph_ctx* ctx, int dest, uint32_t source_mask,
-                    float* ax, float* ay, float* az, float* arho, int mem);
+                    sph_real* ax, sph_real* ay, sph_real* az, sph_real* arho, int mem);
 
 /* n_steps time steps on the context's state.  sph_params.integrator == SPH_INTEGRATOR_EULER: forward Euler
  * (see enum sph_integrator), one evaluation per step.  Default: predictor-corrector, eqs. 12-14 (L148-152),
@@ -219,7 +229,7 @@ int sph_pc_step(sph_ctx* ctx, double dt, int n_steps, int density_mode);
 int sph_sync_state(sph_ctx* ctx, int array, const sph_array* out);
 
 /* Last accelerations of array `array` (ax,ay,az,arho; any may be NULL), caller order. */
-int sph_get_accel(sph_ctx* ctx, int array, float* ax, float* ay, float* az, float* arho, int mem);
+int sph_get_accel(sph_ctx* ctx, int array, sph_real* ax, sph_real* ay, sph_real* az, sph_real* arho, int mem);
 
 /* Neighbour lists N_src(i) of every particle i of array `dest` as CSR in ORIGINAL indices of array `src`,
  * each row sorted ascending: offsets[n_dest+1], indices[total].  Pass indices == NULL (or too small a cap)
@@ -251,6 +261,7 @@ int sph_stencil_candidates(sph_ctx* ctx, int64_t* out);
 const char* sph_strerror(int code);
 const char* sph_last_error(const sph_ctx* ctx);
 int sph_abi_version(void);
+int sph_real_size(void);              /* sizeof(sph_real) of the loaded library: 4 or 8 */
 
 #ifdef __cplusplus
 }

@@ -14,6 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("SPH_B200_LIB") or os.path.join(_HERE, "libsph_b200.so")
+LIB_PATHS = {"f32": LIB_PATH, "f64": os.path.join(_HERE, "libsph_b200_f64.so")}     # sph_real = float / double
 
 SPH_MAX_ARRAYS = 4
 KERNEL_ID = {"cubic": 0, "quintic": 1, "wendland_c2": 2}
@@ -26,7 +27,8 @@ ARRAY_DYNAMIC, ARRAY_FIXED = 0, 1
 EXPORTS = ["sph_create", "sph_destroy", "sph_set_tables", "sph_nnps_build", "sph_summation_density",
            "sph_wcsph_accel", "sph_pc_step", "sph_sync_state", "sph_get_accel", "sph_nnps_get_neighbors",
            "sph_get_stats", "sph_synchronize", "sph_strerror", "sph_last_error", "sph_abi_version",
-           "sph_set_profiling", "sph_get_profile", "sph_kernel_name", "sph_fp32_probe", "sph_stencil_candidates"]
+           "sph_set_profiling", "sph_get_profile", "sph_kernel_name", "sph_fp32_probe", "sph_stencil_candidates",
+           "sph_real_size"]
 
 _FP = C.POINTER(C.c_float)
 FIELD_NAMES = ("x", "y", "z", "u", "v", "w", "h", "m", "rho", "p", "ax", "ay", "az", "arho")
@@ -70,17 +72,18 @@ class SphError(RuntimeError):
         self.code = code
 
 
-_lib = None
+_libs = {}
 
 
-def load() -> C.CDLL:
-    """Loads libsph_b200.so (build it first with `python -m paper_1909_04504_b200.build`)."""
-    global _lib
-    if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise ImportError(f"{LIB_PATH} is missing: build the CUDA library "
+def load(precision: str = "f32") -> C.CDLL:
+    """Loads libsph_b200.so ("f32") or libsph_b200_f64.so ("f64") (build them first with
+    `python -m paper_1909_04504_b200.build`)."""
+    if precision not in _libs:
+        path = LIB_PATHS[precision]
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: build the CUDA library "
                               "(python -m paper_1909_04504_b200.build); there is no CPU fallback")
-        L = C.CDLL(LIB_PATH)
+        L = C.CDLL(path)
         vp, i32, i64, u32p = C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_uint32)
         L.sph_create.argtypes = [C.POINTER(vp), C.POINTER(sph_params), C.POINTER(sph_domain), i32, C.POINTER(i64), vp]
         L.sph_destroy.argtypes = [vp]
@@ -104,29 +107,31 @@ def load() -> C.CDLL:
         for name in EXPORTS:
             if name not in ("sph_strerror", "sph_last_error", "sph_kernel_name"):
                 getattr(L, name).restype = i32
-        _lib = L
-    return _lib
+        if L.sph_real_size() != (4 if precision == "f32" else 8):
+            raise ImportError(f"{path}: sph_real_size() does not match precision {precision}")
+        _libs[precision] = L
+    return _libs[precision]
 
 
-def _ptr_and_mem(t):
+def _ptr_and_mem(t, real_size=4):
     """(address, mem) of a torch tensor (cuda -> DEVICE, cpu -> HOST) or a numpy array (HOST)."""
     if t is None:
         return None, None
     if isinstance(t, np.ndarray):
-        assert t.dtype == np.float32 and t.flags["C_CONTIGUOUS"]
+        assert t.dtype == (np.float32 if real_size == 4 else np.float64) and t.flags["C_CONTIGUOUS"]
         return t.ctypes.data, MEM_HOST
-    assert t.dtype.is_floating_point and t.element_size() == 4 and t.is_contiguous()
+    assert t.dtype.is_floating_point and t.element_size() == real_size and t.is_contiguous()
     return t.data_ptr(), (MEM_DEVICE if t.is_cuda else MEM_HOST)
 
 
-def make_array(fields: Dict[str, object], fixed: bool) -> sph_array:
+def make_array(fields: Dict[str, object], fixed: bool, real_size: int = 4) -> sph_array:
     """fields: name -> torch tensor / numpy float32 array (all on the same side) for x,y,z,u,v,w,h,m,rho,p."""
     a = sph_array()
     a.flags = ARRAY_FIXED if fixed else ARRAY_DYNAMIC
     mem = None
     n = None
     for k in FIELD_NAMES:
-        ptr, m = _ptr_and_mem(fields.get(k))
+        ptr, m = _ptr_and_mem(fields.get(k), real_size)
         setattr(a, k, ptr)
         if ptr is not None or (fields.get(k) is not None):
             t = fields[k]
@@ -145,12 +150,15 @@ class SphContext:
     def __init__(self, *, dim: int, lo, hi, periodic, kernel: str, rho0: float, c0: float, gamma: float = 7.0,
                  alpha: float = 0.1, eps: float = 0.01, g=(0.0, 0.0, 0.0), move: bool = True,
                  capacity: Sequence[int], stream=None, xsub: int = 0, nlist_slots: int = 0, levels: int = 0,
-                 nu: float = 0.0, eta: float = 0.01, integrator: str = "pc"):
+                 nu: float = 0.0, eta: float = 0.01, integrator: str = "pc", precision: str = "f32"):
         import torch
         if not torch.cuda.is_available():
             raise SphError(-7, "no CUDA device: the SPH path has no CPU fallback")
-        self.L = load()
+        self.L = load(precision)
         self.torch = torch
+        self.precision = precision
+        self.real_size = 4 if precision == "f32" else 8
+        self.dtype = torch.float32 if precision == "f32" else torch.float64
         self.stream = stream
         dom = sph_domain(); dom.dim = int(dim)
         prm = sph_params(); prm.kernel = KERNEL_ID[kernel]
@@ -204,14 +212,14 @@ class SphContext:
 
     def nnps_build(self, arrays: List[Dict[str, object]], fixed: Sequence[bool]):
         """arrays[a]: dict of float32 tensors (cuda or cpu) / numpy arrays keyed x,y,z,u,v,w,h,m,rho,p."""
-        A = (sph_array * self.na)(*[make_array(f, fx) for f, fx in zip(arrays, fixed)])
+        A = (sph_array * self.na)(*[make_array(f, fx, self.real_size) for f, fx in zip(arrays, fixed)])
         self._keep = arrays                      # keep caller buffers alive while copies are in flight
         self.n = [int(A[a].n) for a in range(self.na)]
         self._check(self.L.sph_nnps_build(self.ctx, self.na, A))
 
     def _out(self, n, host):
         t = self.torch
-        return t.empty(n, dtype=t.float32, pin_memory=True) if host else t.empty(n, dtype=t.float32, device=self.device)
+        return t.empty(n, dtype=self.dtype, pin_memory=True) if host else t.empty(n, dtype=self.dtype, device=self.device)
 
     def summation_density(self, dest: int, source_mask: int, want_p: bool = True, host: bool = False):
         rho = self._out(self.n[dest], host)
@@ -238,7 +246,7 @@ class SphContext:
         n = self.n[array]
         if out is None:
             out = {k: self._out(n, host) for k in fields if not (self.dim == 2 and k in ("z", "w", "az"))}
-        a = make_array(out, False)
+        a = make_array(out, False, self.real_size)
         a.n = n; a.mem = MEM_HOST if host else MEM_DEVICE
         self._check(self.L.sph_sync_state(self.ctx, array, C.byref(a)))
         return out
@@ -303,12 +311,14 @@ class SphContext:
         return out
 
 
-def device_arrays(wl, device=None):
-    """Uploads a workload's float32 numpy arrays as torch CUDA tensors (one dict per particle array)."""
+def device_arrays(wl, device=None, precision: str = "f32"):
+    """Uploads a workload's float32 numpy arrays as torch CUDA tensors (one dict per particle array); precision
+    "f64" widens them to double (the values stay the float32-representable ones the workload holds)."""
     import torch
     dev = device or torch.device("cuda", torch.cuda.current_device())
+    dt = torch.float32 if precision == "f32" else torch.float64
     keys = ("x", "y", "z", "u", "v", "w", "h", "m", "rho")
-    return [{k: torch.from_numpy(getattr(a, k)).to(dev) for k in keys} for a in wl.arrays]
+    return [{k: torch.from_numpy(getattr(a, k)).to(dev).to(dt).contiguous() for k in keys} for a in wl.arrays]
 
 
 def pinned_arrays(wl):

@@ -1,7 +1,7 @@
 """In-tree build of the CUDA library: csrc/*.cu -> paper_1909_04504_b200/libsph_b200.so for sm_100a.
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box with the snapshot.
-Usage: python -m paper_1909_04504_b200.build [--force] [--verbose]
+Usage: python -m paper_1909_04504_b200.build [--force] [--verbose] [--f32 | --f64]   (default: both libraries)
 """
 from __future__ import annotations
 
@@ -17,6 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 # SPH_B200_LIB / SPH_B200_NVCC_FLAGS: build (and load, see binding.py) a tuning variant beside the default library
 LIB = os.environ.get("SPH_B200_LIB") or os.path.join(HERE, "libsph_b200.so")
+LIB_F64 = os.path.join(HERE, "libsph_b200_f64.so")      # the same sources with -DSPH_REAL_DOUBLE (sph_real = double)
 EXTRA = os.environ.get("SPH_B200_NVCC_FLAGS", "").split()
 OBJ = os.path.join(HERE, "build" if not os.environ.get("SPH_B200_LIB") else
                    "build_" + hashlib.sha256(LIB.encode()).hexdigest()[:8])
@@ -38,21 +39,27 @@ def _nvcc() -> str:
     return cand
 
 
-def _digest() -> str:
+def _digest(extra=()) -> str:
     h = hashlib.sha256()
     names = sorted(os.listdir(CSRC)) + ["../../include/sph.h"]
     for n in names:
         p = os.path.normpath(os.path.join(CSRC, n))
         if os.path.isfile(p):
             h.update(n.encode()); h.update(open(p, "rb").read())
-    h.update(" ".join(ARCH + FLAGS + EXTRA + [repr(SOURCES)]).encode())
+    h.update(" ".join(ARCH + FLAGS + EXTRA + list(extra) + [repr(SOURCES)]).encode())
     return h.hexdigest()
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, precision: str = "f32") -> str:
+    """precision "f32": libsph_b200.so (sph_real = float); "f64": libsph_b200_f64.so (-DSPH_REAL_DOUBLE)."""
+    lib, objdir, extra = (LIB, OBJ, []) if precision == "f32" else (LIB_F64, OBJ + "_f64", ["-DSPH_REAL_DOUBLE"])
+    return _build(lib, objdir, extra, force, verbose)
+
+
+def _build(LIB: str, OBJ: str, extra, force: bool, verbose: bool) -> str:
     os.makedirs(OBJ, exist_ok=True)
     stamp = os.path.join(OBJ, "digest.txt")
-    dig = _digest()
+    dig = _digest(extra)
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == dig:
         return LIB
     nvcc = _nvcc()
@@ -60,7 +67,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     def compile_one(item) -> str:
         src, defs, oname = item
         obj = os.path.join(OBJ, oname)
-        cmd = [nvcc, *ARCH, *FLAGS, *EXTRA, *defs, "-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc, *ARCH, *FLAGS, *EXTRA, *extra, *defs, "-I", INCLUDE, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -81,4 +88,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    for prec in (("f64",) if "--f64" in sys.argv else ("f32",) if "--f32" in sys.argv else ("f32", "f64")):
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, precision=prec))

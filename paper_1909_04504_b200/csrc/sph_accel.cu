@@ -19,7 +19,7 @@ int launch_accel_k1(sph_ctx* c, int dim, bool filter, bool want_arho, const Acce
 int launch_accel_k2(sph_ctx* c, int dim, bool filter, bool want_arho, const AccelRoles& roles, bool replay);
 
 #ifdef SPH_ACCEL_KERNEL
-struct AccelSrc { float4 pj, vj; float2 rj; uint32_t aid; };
+struct AccelSrc { real4 pj, vj; real2 rj; uint32_t aid; };
 
 template <int KERNEL, int DIM, bool VARH, bool ARHO, bool FILTER, bool REPLAY, int PM, bool LAMINAR>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS_ACCEL)
@@ -30,86 +30,87 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
     const int warp_id = i >> 5;
     const bool in = i < n;
-    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1), vi = make_float4(0, 0, 0, 0);
-    float2 ri = make_float2(1, 0);
-    if (in) { meta = S.meta[i]; pi = __ldg(S.posh + i); vi = __ldg(S.velm + i); ri = __ldg(S.rp + i); ci = S.cell[i]; }
+    uint32_t meta = 0, ci = 0; real4 pi = make_real4(0, 0, 0, 1), vi = make_real4(0, 0, 0, 0);
+    real2 ri = make_real2(1, 0);
+    if (in) { meta = S.meta[i]; pi = ldg_r(S.posh + i); vi = ldg_r(S.velm + i); ri = ldg_r(S.rp + i); ci = S.cell[i]; }
     const uint32_t aid_i = meta >> SPH_META_IDX_BITS;
     const uint32_t my_mask = in ? pc.src_mask[aid_i] : 0u;
     const bool active = my_mask != 0u;
     // arrays that are no destination of any launch of this evaluation: their accelerations are zero (the sort does
     // not carry acc along, so what lies in their rows belongs to other particles)
     if (in && !active && (((roles.zero_xyz | roles.zero_w) >> aid_i) & 1u)) {
-        float4 a = S.acc[i];
+        real4 a = S.acc[i];
         if ((roles.zero_xyz >> aid_i) & 1u) { a.x = 0.0f; a.y = 0.0f; a.z = 0.0f; }
         if ((roles.zero_w >> aid_i) & 1u) a.w = 0.0f;
         S.acc[i] = a;
     }
     if (!__any_sync(SPH_FULL_MASK, active)) return;
 
-    const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
-    const float sigma = pc.sigma, h_c = pc.h_const, hinv_c = pc.hinv_const, fac_c = pc.fac_const, kh = pc.kh;
-    const float visc = pc.visc, eps = pc.eps, nu4 = pc.nu4, eta = pc.eta;
-    const float hi = VARH ? pi.w : h_c;
-    const float cut2c = pair_cut2(kh, h_c, h_c);
+    const real Lx = g.Lr[0], Ly = g.Lr[1], Lz = g.Lr[2];
+    const real sigma = pc.sigma, h_c = pc.h_const, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
+    const real kh = sizeof(real) == 8 ? pc.ksup : pc.kh;               // what pair_cut2 of the build's real type takes
+    const real visc = pc.visc, eps = pc.eps, nu4 = pc.nu4, eta = pc.eta;
+    const real hi = VARH ? pi.w : h_c;
+    const real cut2c = pair_cut2(kh, h_c, h_c);
     // PM: where the neighbour's rho and p/rho^2 come from (the loop is L1-gather bound: fewer gathers pay).
     //   0  gathered from rp (caller-supplied p, gamma != 7 ...): three gathers
     //   1  gamma = 7, every p is the EOS of its rho, and velm.w carries rho (constant h, or variable h with uniform
     //      mass): p/rho^2 is recomputed (the destination's own term too, so that the pair terms stay antisymmetric):
     //      two gathers
     //   2  UM layout (constant h, uniform mass): rho in velm.w, p/rho^2 in posh.w, m = m_const: two gathers
-    const float inv_rho0 = 1.0f / pc.rho0, rho0 = pc.rho0, Beos = pc.B;
-    const float rho_i = ri.x, pr_i = PM == 1 ? eos7_p_over_rho2(ri.x, rho0, inv_rho0, Beos) : ri.y;
-    const float m_const = pc.m_const;
-    float ax = pc.g[0], ay = pc.g[1], az = pc.g[2], ar = 0.0f;      // gravity = accumulator init (Listing 4)
+    const real inv_rho0 = 1.0f / pc.rho0, rho0 = pc.rho0, Beos = pc.B;
+    const real rho_i = ri.x, pr_i = PM == 1 ? eos7_p_over_rho2(ri.x, rho0, inv_rho0, Beos) : ri.y;
+    const real m_const = pc.m_const;
+    real ax = pc.g[0], ay = pc.g[1], az = pc.g[2], ar = 0.0f;      // gravity = accumulator init (Listing 4)
     unsigned nhits = 0;                                                 // pairs that pass the exact predicate (and the source mask)
     auto load = [&](uint32_t j) {
-        AccelSrc s; s.pj = __ldg(S.posh + j); s.vj = __ldg(S.velm + j); s.aid = 0u;
-        s.rj = PM ? make_float2(0.0f, 0.0f) : __ldg(S.rp + j);
+        AccelSrc s; s.pj = ldg_r(S.posh + j); s.vj = ldg_r(S.velm + j); s.aid = 0u;
+        s.rj = PM ? make_real2(0.0f, 0.0f) : ldg_r(S.rp + j);
         if (FILTER) { if (my_mask != pc.all_mask) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS; }   // lanes fed by all arrays skip the gather
         return s;
     };
     auto compute = [&](const AccelSrc& s, bool has, uint32_t code, auto per) {
         // the exact predicate of DESIGN.md R7 on the candidate the tensor-core filter let through
-        float dx = __fsub_rn(pi.x, s.pj.x), dy = __fsub_rn(pi.y, s.pj.y), dz = DIM == 3 ? __fsub_rn(pi.z, s.pj.z) : 0.0f;
+        real dx = rsub(pi.x, s.pj.x), dy = rsub(pi.y, s.pj.y), dz = DIM == 3 ? rsub(pi.z, s.pj.z) : real(0);
         if (decltype(per)::value) {
-            dx = __fsub_rn(dx, img_shift(code, 0, Lx)); dy = __fsub_rn(dy, img_shift(code, 1, Ly));
-            if (DIM == 3) dz = __fsub_rn(dz, img_shift(code, 2, Lz));
+            dx = rsub(dx, img_shift(code, 0, Lx)); dy = rsub(dy, img_shift(code, 1, Ly));
+            if (DIM == 3) dz = rsub(dz, img_shift(code, 2, Lz));
         }
-        const float r2 = pair_r2(dx, dy, dz);
+        const real r2 = pair_r2(dx, dy, dz);
         has = has && r2 < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);
         if (FILTER) has = has && (my_mask == pc.all_mask || ((my_mask >> s.aid) & 1u));
         nhits += has ? 1u : 0u;
-        const float rinv = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;       // grad W := 0 at r = 0 (R18): rinv = 0
-        const float r = r2 * rinv;
-        float hij, hinv, fac;
+        const real rinv = r2 > 0.0f ? rsqrt_approx(r2) : real(0);       // grad W := 0 at r = 0 (R18): rinv = 0
+        const real r = r2 * rinv;
+        real hij, hinv, fac;
         if (VARH) {
             hij = 0.5f * (hi + s.pj.w);
             hinv = rcp_approx(hij);
-            fac = sigma * hinv * hinv * (DIM == 3 ? hinv : 1.0f);
+            fac = sigma * hinv * hinv * (DIM == 3 ? hinv : real(1));
         } else { hij = h_c; hinv = hinv_c; fac = fac_c; }
-        float f, df;
+        real f, df;
         kernel_profile<KERNEL, DIM>(r * hinv, f, df);
-        const float gc = fac * hinv * df * rinv;                        // grad_i W_ij = gc * (dx,dy,dz)
-        const float vx = vi.x - s.vj.x, vy = vi.y - s.vj.y;
-        float vr = fmaf(vy, dy, vx * dx);
-        if (DIM == 3) vr = fmaf(vi.z - s.vj.z, dz, vr);
+        const real gc = fac * hinv * df * rinv;                        // grad_i W_ij = gc * (dx,dy,dz)
+        const real vx = vi.x - s.vj.x, vy = vi.y - s.vj.y;
+        real vr = rfma(vy, dy, vx * dx);
+        if (DIM == 3) vr = rfma(vi.z - s.vj.z, dz, vr);
         // SortedState layouts: where m, rho and p/rho^2 of the neighbour ride
-        const float mj = PM == 2 ? m_const : (VARH ? (PM == 1 ? m_const : s.vj.w) : s.pj.w);
-        const float rho_j = PM ? s.vj.w : s.rj.x;
-        const float pr_j = PM == 2 ? s.pj.w : (PM == 1 ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y);
+        const real mj = PM == 2 ? m_const : (VARH ? (PM == 1 ? m_const : s.vj.w) : s.pj.w);
+        const real rho_j = PM ? s.vj.w : s.rj.x;
+        const real pr_j = PM == 2 ? s.pj.w : (PM == 1 ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y);
         // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
-        const float den = fmaf(eps * hij, hij, r2) * (rho_i + rho_j);
-        const float Pi = vr < 0.0f ? visc * hij * vr * rcp_approx(den) : 0.0f;
-        const float mg = has ? mj * gc : 0.0f;                          // a lane that has run out contributes nothing
-        const float sc = -mg * (pr_i + pr_j + Pi);
-        ax = fmaf(sc, dx, ax); ay = fmaf(sc, dy, ay);
-        if (DIM == 3) az = fmaf(sc, dz, az);
-        if (ARHO) ar = fmaf(mg, vr, ar);
+        const real den = rfma(eps * hij, hij, r2) * (rho_i + rho_j);
+        const real Pi = vr < real(0) ? visc * hij * vr * rcp_approx(den) : real(0);
+        const real mg = has ? mj * gc : real(0);                          // a lane that has run out contributes nothing
+        const real sc = -mg * (pr_i + pr_j + Pi);
+        ax = rfma(sc, dx, ax); ay = rfma(sc, dy, ay);
+        if (DIM == 3) az = rfma(sc, dz, az);
+        if (ARHO) ar = rfma(mg, vr, ar);
         if (LAMINAR) {                                                  // laminar viscosity, eq.10 (launches with nu != 0)
             // m_j 4nu/(rho_i+rho_j) (r.gradW)/(r^2 + eta h^2) u_ij,  r.gradW = gc r^2
-            const float lam = mg * nu4 * r2 * rcp_approx(fmaxf(fmaf(eta * hij, hij, r2) * (rho_i + rho_j), 1.0e-30f));
-            ax = fmaf(lam, vx, ax); ay = fmaf(lam, vy, ay);
-            if (DIM == 3) az = fmaf(lam, vi.z - s.vj.z, az);
+            const real lam = mg * nu4 * r2 * rcp_approx(rmax(rfma(eta * hij, hij, r2) * (rho_i + rho_j), real(1.0e-30)));
+            ax = rfma(lam, vx, ax); ay = rfma(lam, vy, ay);
+            if (DIM == 3) az = rfma(lam, vi.z - s.vj.z, az);
         }
     };
     const uint32_t idle = in ? (uint32_t)i : 0u;
@@ -124,14 +125,14 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     if (head != SPH_NL_NONE) {
         tile_replay(nl, head, ws, active, drain);
     } else {                                    // no record (or one that did not fit the pool): search
-        tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
+        tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, to_float4(pi), ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
     }
     if (active) {
-        float4 a;
+        real4 a;
         if ((roles.arho_only >> aid_i) & 1u) {                          // ContinuityEquation-only destination array
-            a = ((roles.keep_xyz >> aid_i) & 1u) ? S.acc[i] : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            a = ((roles.keep_xyz >> aid_i) & 1u) ? S.acc[i] : make_real4(0.0f, 0.0f, 0.0f, 0.0f);
             a.w = ar;
-        } else a = make_float4(ax, ay, DIM == 3 ? az : 0.0f, ARHO ? ar : 0.0f);
+        } else a = make_real4(ax, ay, DIM == 3 ? az : real(0), ARHO ? ar : real(0));
         S.acc[i] = a;
         if (!isfinite(a.x) || !isfinite(a.y) || !isfinite(a.z) || !isfinite(a.w)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }

@@ -25,6 +25,7 @@ extern "C" const char* sph_strerror(int code) {
 }
 extern "C" const char* sph_last_error(const sph_ctx* c) { return c ? c->err : "null context"; }
 extern "C" int sph_abi_version(void) { return SPH_ABI_VERSION; }
+extern "C" int sph_real_size(void) { return (int)sizeof(sph_real); }
 
 static void drop_graph(sph_ctx* c) {
     if (c->step_graph) { cudaGraphExecDestroy(c->step_graph); c->step_graph = nullptr; }
@@ -45,18 +46,19 @@ static void set_consts(sph_ctx* c) {
     const sph_params& P = c->prm;
     PairConsts& pc = c->pc;
     memset(&pc, 0, sizeof(pc));
-    pc.kh = (float)(0.5 * kernel_support(P.kernel));
-    pc.sigma = (float)kernel_sigma(P.kernel, c->dom.dim);
-    pc.rho0 = (float)P.rho0;
-    pc.B = (float)(P.rho0 * P.c0 * P.c0 / P.gamma);
-    pc.gamma = (float)P.gamma;
+    pc.kh = (real)(0.5 * kernel_support(P.kernel));
+    pc.ksup = (real)kernel_support(P.kernel);
+    pc.sigma = (real)kernel_sigma(P.kernel, c->dom.dim);
+    pc.rho0 = (real)P.rho0;
+    pc.B = (real)(P.rho0 * P.c0 * P.c0 / P.gamma);
+    pc.gamma = (real)P.gamma;
     pc.gamma_is_7 = (P.gamma == 7.0);
-    pc.visc = (float)(-2.0 * P.alpha * P.c0);
-    pc.eps = (float)P.eps;
-    pc.nu4 = (float)(4.0 * P.nu); pc.eta = (float)P.eta;
-    for (int k = 0; k < 3; ++k) pc.g[k] = (float)P.g[k];
+    pc.visc = (real)(-2.0 * P.alpha * P.c0);
+    pc.eps = (real)P.eps;
+    pc.nu4 = (real)(4.0 * P.nu); pc.eta = (real)P.eta;
+    for (int k = 0; k < 3; ++k) pc.g[k] = (real)P.g[k];
     pc.all_mask = (1u << c->na) - 1u;
-    pc.h_const = 1.0f; pc.hinv_const = 1.0f; pc.fac_const = 1.0f;
+    pc.h_const = 1; pc.hinv_const = 1; pc.fac_const = 1;
 }
 
 extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_domain* domain,
@@ -101,13 +103,13 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     const size_t N = (size_t)tot + 1;
     c->max_keys = 8 * tot + 65536; if (c->max_keys > ((int64_t)1 << 27)) c->max_keys = (int64_t)1 << 27;
     for (int b = 0; b < 2; ++b) {
-        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].posh, N * sizeof(float4)));
-        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].velm, N * sizeof(float4)));
-        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].rp, N * sizeof(float2)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].posh, N * sizeof(real4)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].velm, N * sizeof(real4)));
+        SPH_CUDA_OK(c, cudaMalloc(&c->S[b].rp, N * sizeof(real2)));
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].meta, N * sizeof(uint32_t)));
         SPH_CUDA_OK(c, cudaMalloc(&c->S[b].cell, N * sizeof(uint32_t)));
     }
-    for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMalloc(&c->S[b].acc, N * sizeof(float4)));
+    for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMalloc(&c->S[b].acc, N * sizeof(real4)));
     SPH_CUDA_OK(c, cudaMalloc(&c->key, (N + 1) * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMalloc(&c->rank, (N + 1) * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMalloc(&c->cell_count, (size_t)(c->max_keys + 2) * sizeof(uint32_t)));
@@ -117,9 +119,9 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_state, 0, (scan_n / 2048 + 4) * sizeof(unsigned long long), c->stream));
     SPH_CUDA_OK(c, cudaMalloc(&c->scan_ticket, 2 * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_ticket, 0, 2 * sizeof(uint32_t), c->stream));
-    SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(float)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(real)));
     SPH_CUDA_OK(c, cudaMalloc(&c->counters, CNT_COUNT * sizeof(unsigned long long)));
-    SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 4 * sizeof(float)));
+    SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 4 * sizeof(long long)));
     if (nl_slots > 0 && tot > 0) {
         const size_t warps = (size_t)(tot + 31) / 32;
         size_t rows = warps * (size_t)nl_slots + 32;
@@ -130,7 +132,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
         c->nl.used = (uint32_t*)(c->counters + CNT_NL_USED);
     }
     SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
-    for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMemsetAsync(c->S[b].acc, 0, N * sizeof(float4), c->stream));
+    for (int b = 0; b < 2; ++b) SPH_CUDA_OK(c, cudaMemsetAsync(c->S[b].acc, 0, N * sizeof(real4), c->stream));
     SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
     return SPH_OK;
 }
@@ -178,6 +180,8 @@ static int size_grid(sph_ctx* c) {
         g.per[k] = (k < g.dim) ? (c->dom.periodic[k] != 0) : 0;
         g.lo[k] = (float)c->dom.lo[k]; g.hi[k] = (float)c->dom.hi[k];
         g.L[k] = (float)(c->dom.hi[k] - c->dom.lo[k]);
+        g.Lr[k] = sizeof(real) == 8 ? (real)(c->dom.hi[k] - c->dom.lo[k]) : (real)g.L[k];
+        g.lor[k] = (real)c->dom.lo[k]; g.hir[k] = (real)c->dom.hi[k];
         if (k < g.dim) big = fmax(big, fmax(fmax(fabs(c->dom.lo[k]), fabs(c->dom.hi[k])), c->dom.hi[k] - c->dom.lo[k]));
     }
     g.uabs = (float)(1.1920929e-7 * big);
@@ -195,8 +199,9 @@ static int size_grid(sph_ctx* c) {
         for (int l = 0; l < nlev && ok; ++l) {
             LevelDesc& Lv = g.lev[l];
             // every h of level l is <= hmax_l (float thresholds; level_of_h uses the same comparisons on both sides)
-            Lv.hmax = (l == nlev - 1) ? c->h_max : (float)((double)c->h_min * pow(ratio, (l + 1.0) / nlev));
-            if (l == nlev - 1 || Lv.hmax > c->h_max) Lv.hmax = c->h_max;
+            const float hmax_f = (float)c->h_max;           // float(h) <= float(h_max) for every h (monotone rounding): the search runs in float
+            Lv.hmax = (l == nlev - 1) ? hmax_f : (float)((double)c->h_min * pow(ratio, (l + 1.0) / nlev));
+            if (l == nlev - 1 || Lv.hmax > hmax_f) Lv.hmax = hmax_f;
             const double cutoff = ksup * (double)Lv.hmax;
             int64_t cells = 1;
             for (int k = 0; k < 3; ++k) {
@@ -230,7 +235,7 @@ static int size_grid(sph_ctx* c) {
     return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
 }
 
-static float* stage_field(sph_ctx* c, int field, int array) { return c->staging + ((size_t)field * (c->cap_total + 1) + c->base[array]); }
+static real* stage_field(sph_ctx* c, int field, int array) { return c->staging + ((size_t)field * (c->cap_total + 1) + c->base[array]); }
 
 extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays) {
     if (!c || !arrays) return SPH_ERR_NULL;
@@ -260,13 +265,13 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     for (int a = 0; a <= c->na; ++a) P.base[a] = c->base[a];
     for (int a = 0; a < c->na; ++a) {
         const sph_array& A = arrays[a];
-        const float* src[N_STAGE_FIELDS] = { A.x, A.y, A.z, A.u, A.v, A.w, A.h, A.m, A.rho, A.p, A.ax, A.ay, A.az, A.arho };
-        const float* use[N_STAGE_FIELDS];
+        const real* src[N_STAGE_FIELDS] = { A.x, A.y, A.z, A.u, A.v, A.w, A.h, A.m, A.rho, A.p, A.ax, A.ay, A.az, A.arho };
+        const real* use[N_STAGE_FIELDS];
         for (int f = 0; f < N_STAGE_FIELDS; ++f) {
             use[f] = src[f];
             if (A.mem == SPH_MEM_HOST && src[f] && A.n > 0) {
-                float* d = stage_field(c, f, a);
-                SPH_CUDA_OK(c, cudaMemcpyAsync(d, src[f], (size_t)A.n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+                real* d = stage_field(c, f, a);
+                SPH_CUDA_OK(c, cudaMemcpyAsync(d, src[f], (size_t)A.n * sizeof(real), cudaMemcpyHostToDevice, c->stream));
                 use[f] = d;
             }
         }
@@ -276,24 +281,26 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
     SPH_CUDA_OK(c, cudaMemsetAsync(c->counters, 0, CNT_COUNT * sizeof(unsigned long long), c->stream));
     c->cur = 0;
     int rc = nnps_pack(c, P); if (rc) return rc;
-    int hmm[4] = { 0, 0, 0, 0 };
-    SPH_CUDA_OK(c, cudaMemcpyAsync(hmm, c->hminmax, sizeof(hmm), cudaMemcpyDeviceToHost, c->stream));
+    long long hmm[4] = { 0, 0, 0, 0 };                  // ordered-integer images of h min/max, |m| min/max (int or long long words)
+    SPH_CUDA_OK(c, cudaMemcpyAsync(hmm, c->hminmax, 4 * (sizeof(real) == 8 ? sizeof(long long) : sizeof(int)), cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    real hm[4];
+    for (int k = 0; k < 4; ++k) memcpy(&hm[k], (const char*)hmm + k * sizeof(real), sizeof(real));
     if (tot == 0) {                            // no particles at all: any grid will do; size it so that a periodic box gets its >= 3 cells
         double minL = 1.0e300;
         for (int k = 0; k < c->dom.dim; ++k) minL = fmin(minL, c->dom.hi[k] - c->dom.lo[k]);
-        c->h_min = c->h_max = (float)(minL / (4.0 * kernel_support(c->prm.kernel)));
+        c->h_min = c->h_max = (real)(minL / (4.0 * kernel_support(c->prm.kernel)));
     }
-    else { memcpy(&c->h_min, &hmm[0], 4); memcpy(&c->h_max, &hmm[1], 4); }
-    if (!(c->h_max > 0.0f) || !isfinite(c->h_max)) return sph_fail(c, SPH_ERR_BAD_ARG, "smoothing lengths must be positive and finite");
+    else { c->h_min = hm[0]; c->h_max = hm[1]; }
+    if (!(c->h_max > 0) || !isfinite((double)c->h_max)) return sph_fail(c, SPH_ERR_BAD_ARG, "smoothing lengths must be positive and finite");
     c->variable_h = (c->h_min != c->h_max);
     c->p_is_eos = !any_p;
-    c->pc.uniform_m = (tot > 0 && !c->variable_h && hmm[2] == hmm[3]) ? 1 : 0;
-    c->pc.varh_um = (tot > 0 && c->variable_h && hmm[2] == hmm[3] && c->p_is_eos && c->pc.gamma_is_7) ? 1 : 0;
-    memcpy(&c->pc.m_const, &hmm[3], 4);
+    c->pc.uniform_m = (tot > 0 && !c->variable_h && hm[2] == hm[3]) ? 1 : 0;
+    c->pc.varh_um = (tot > 0 && c->variable_h && hm[2] == hm[3] && c->p_is_eos && c->pc.gamma_is_7) ? 1 : 0;
+    c->pc.m_const = hm[3];
     c->pc.h_const = c->h_max;
-    c->pc.hinv_const = (float)(1.0 / (double)c->h_max);
-    c->pc.fac_const = (float)(kernel_sigma(c->prm.kernel, c->dom.dim) / pow((double)c->h_max, c->dom.dim));
+    c->pc.hinv_const = (real)(1.0 / (double)c->h_max);
+    c->pc.fac_const = (real)(kernel_sigma(c->prm.kernel, c->dom.dim) / pow((double)c->h_max, c->dom.dim));
     rc = size_grid(c); if (rc) return rc;
     SPH_CUDA_OK(c, cudaMemsetAsync(c->cell_count, 0, (size_t)(c->n_keys + 1) * sizeof(uint32_t), c->stream));   // once per build; k_scan re-clears it
     rc = nnps_key_hist(c); if (rc) return rc;
@@ -305,14 +312,14 @@ extern "C" int sph_nnps_build(sph_ctx* c, int n_arrays, const sph_array* arrays)
 
 // caller-order output of up to 12 fields of one array, to device pointers or through the staging buffer to host
 static int emit(sph_ctx* c, int array, OutPtrs O, int mem) {
-    float** f = (float**)&O;
-    const int NF = sizeof(OutPtrs) / sizeof(float*);
+    real** f = (real**)&O;
+    const int NF = sizeof(OutPtrs) / sizeof(real*);
     const size_t n = (size_t)c->n[array];
     if (mem == SPH_MEM_DEVICE) return nnps_gather_out(c, array, O);
-    float* host[NF]; int used = 0;
+    real* host[NF]; int used = 0;
     for (int k = 0; k < NF; ++k) { host[k] = f[k]; if (f[k]) { if (used >= N_STAGE_FIELDS) return sph_fail(c, SPH_ERR_BAD_ARG, "too many host outputs in one call"); f[k] = c->staging + (size_t)used * (c->cap_total + 1); ++used; } }
     int rc = nnps_gather_out(c, array, O); if (rc) return rc;
-    for (int k = 0; k < NF; ++k) if (host[k] && n) SPH_CUDA_OK(c, cudaMemcpyAsync(host[k], f[k], n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    for (int k = 0; k < NF; ++k) if (host[k] && n) SPH_CUDA_OK(c, cudaMemcpyAsync(host[k], f[k], n * sizeof(real), cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA_OK(c, cudaStreamSynchronize(c->stream));
     return SPH_OK;
 }
@@ -328,7 +335,7 @@ static int ensure_search(sph_ctx* c) {
     return launch_search(c);
 }
 
-extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask, float* rho_out, float* p_out, int mem) {
+extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask, sph_real* rho_out, sph_real* p_out, int mem) {
     if (!c) return SPH_ERR_NULL;
     if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
     if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
@@ -341,7 +348,7 @@ extern "C" int sph_summation_density(sph_ctx* c, int dest, uint32_t source_mask,
     return SPH_OK;
 }
 
-extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, float* ax, float* ay, float* az, float* arho, int mem) {
+extern "C" int sph_wcsph_accel(sph_ctx* c, int dest, uint32_t source_mask, sph_real* ax, sph_real* ay, sph_real* az, sph_real* arho, int mem) {
     if (!c) return SPH_ERR_NULL;
     if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
     if (dest < 0 || dest >= c->na || source_mask == 0 || (source_mask & ~c->pc.all_mask)) return sph_fail(c, SPH_ERR_BAD_ARG, "bad dest / source_mask");
@@ -417,13 +424,13 @@ static int evaluate(sph_ctx* c, bool continuity) {
             return accel(m, true, ao, true); }); if (rc) return rc;
     }
     if (!launched && c->n_total > 0)      // no momentum / continuity destination at all: every acceleration is zero
-        SPH_CUDA_OK(c, cudaMemsetAsync(c->S[c->cur].acc, 0, (size_t)c->n_total * sizeof(float4), c->stream));
+        SPH_CUDA_OK(c, cudaMemsetAsync(c->S[c->cur].acc, 0, (size_t)c->n_total * sizeof(real4), c->stream));
     return SPH_OK;
 }
 
 // one step of the loop of sph_pc_step.   PC: (14 of the previous step) + 12 + 13 + key.   Euler: x += dt u ; u += dt a ;
 // rho += dt arho ; key.   Then the sort (NNPS rebuilt every step, L443) and the evaluation.
-static int step_body(sph_ctx* c, float dt, bool cont, bool kick2) {
+static int step_body(sph_ctx* c, real dt, bool cont, bool kick2) {
     int rc = nnps_update_key_hist(c, dt, kick2, true, cont, true); if (rc) return rc;
     rc = nnps_sort_from_keys(c, false); if (rc) return rc;
     rc = evaluate(c, cont); if (rc) return rc;
@@ -433,7 +440,7 @@ static int step_body(sph_ctx* c, float dt, bool cont, bool kick2) {
 
 // Captures TWO consecutive middle steps (the state buffers flip every step, so two steps return to the same
 // buffers) into a CUDA graph: long runs of small problems are bound by launch latency, not by work.
-static bool ensure_step_graph(sph_ctx* c, float dt, bool cont, bool kick2) {
+static bool ensure_step_graph(sph_ctx* c, real dt, bool cont, bool kick2) {
     if (c->graph_off) return false;
     if (c->step_graph && c->graph_dt == dt && c->graph_cont == (cont ? 1 : 0) && c->graph_cur == c->cur) return true;
     drop_graph(c);
@@ -465,16 +472,16 @@ extern "C" int sph_pc_step(sph_ctx* c, double dt, int n_steps, int density_mode)
     }
     const bool euler = c->prm.integrator == SPH_INTEGRATOR_EULER;
     int s = 0;
-    if (n_steps > 0) { rc = step_body(c, (float)dt, cont, false); if (rc) return rc; c->steps_done++; s = 1; }
+    if (n_steps > 0) { rc = step_body(c, (real)dt, cont, false); if (rc) return rc; c->steps_done++; s = 1; }
     // long runs: replay a captured pair of steps (same kernels, same arguments, one graph launch per two steps)
-    if (n_steps - s >= 8 && !c->prof_on && c->n_total > 0 && ensure_step_graph(c, (float)dt, cont, !euler)) {
+    if (n_steps - s >= 8 && !c->prof_on && c->n_total > 0 && ensure_step_graph(c, (real)dt, cont, !euler)) {
         while (n_steps - s >= 2) {
             SPH_CUDA_OK(c, cudaGraphLaunch(c->step_graph, c->stream));
             c->launches += c->graph_nodes; c->steps_done += 2; s += 2;
         }
     }
-    for (; s < n_steps; ++s) { rc = step_body(c, (float)dt, cont, !euler); if (rc) return rc; c->steps_done++; }
-    if (n_steps > 0 && !euler) { rc = nnps_update_key_hist(c, (float)dt, true, false, cont, false); if (rc) return rc; }   // eq.14
+    for (; s < n_steps; ++s) { rc = step_body(c, (real)dt, cont, !euler); if (rc) return rc; c->steps_done++; }
+    if (n_steps > 0 && !euler) { rc = nnps_update_key_hist(c, (real)dt, true, false, cont, false); if (rc) return rc; }   // eq.14
     return SPH_OK;
 }
 
@@ -489,7 +496,7 @@ extern "C" int sph_sync_state(sph_ctx* c, int array, const sph_array* out) {
     return emit(c, array, O, out->mem);
 }
 
-extern "C" int sph_get_accel(sph_ctx* c, int array, float* ax, float* ay, float* az, float* arho, int mem) {
+extern "C" int sph_get_accel(sph_ctx* c, int array, sph_real* ax, sph_real* ay, sph_real* az, sph_real* arho, int mem) {
     if (!c) return SPH_ERR_NULL;
     if (!c->built) return sph_fail(c, SPH_ERR_STALE_NNPS, sph_strerror(SPH_ERR_STALE_NNPS));
     if (array < 0 || array >= c->na) return sph_fail(c, SPH_ERR_BAD_ARG, "bad array");
@@ -548,7 +555,7 @@ extern "C" int sph_get_stats(sph_ctx* c, sph_stats* out) {
     out->kernel_launches = c->launches;
     out->steps_done = c->steps_done;
     out->variable_h = c->variable_h ? 1 : 0;
-    out->h_max = c->h_max;
+    out->h_max = (float)c->h_max;
     out->xsub = top.xsub;
     out->used_rows = c->last_used_rows ? 1 : 0;
     out->nlist_rows_capacity = c->nl.pool_rows;

@@ -24,7 +24,7 @@ struct sph_ctx {
     PairConsts pc;
     bool built, have_accel, have_arho, variable_h;
     bool p_is_eos;             // every p of the state is the EOS of its rho (no array supplied p at the last build)
-    float h_min, h_max;
+    real h_min, h_max;
     int64_t n_keys, max_keys;
 
     SortedState S[2];          // double-buffered (permute A -> B); acc is permuted only by sph_nnps_build (inside
@@ -33,9 +33,9 @@ struct sph_ctx {
     uint32_t *key, *rank;      // per particle, pre-sort order
     uint32_t *cell_count, *cell_start;
     unsigned long long* scan_state; uint32_t* scan_ticket;   // k_scan look-back table; scan_ticket[0] = ticket, [1] = epoch
-    float* staging;            // host<->device staging for SPH_MEM_HOST (10 floats per particle of capacity)
+    real* staging;             // host<->device staging for SPH_MEM_HOST (14 reals per particle of capacity)
     unsigned long long* counters;     // device, CNT_COUNT entries
-    float* hminmax;            // device, 4 floats (as ordered ints): h min/max, |m| min/max
+    void* hminmax;             // device, 4 x 8 bytes: h min/max, |m| min/max as ordered integers of the real type
 
     // neighbour rows recorded by a density launch for the acceleration launch that follows it
     NList nl;                  // nl.pool == nullptr: recording disabled
@@ -44,7 +44,7 @@ struct sph_ctx {
     bool counters_fresh;       // k_update has just cleared the counters of the search and the pair passes (consumed by evaluate)
     bool heads_fresh;          // k_scatter has just cleared the record heads (consumed by launch_search)
     // CUDA graph of two consecutive steps of sph_pc_step (the state buffers flip every step), replayed for long runs
-    cudaGraphExec_t step_graph; float graph_dt; int graph_cont, graph_cur, graph_nodes; bool graph_off;
+    cudaGraphExec_t step_graph; real graph_dt; int graph_cont, graph_cur, graph_nodes; bool graph_off;
     bool xsub_auto;            // xsub was not given: 6, or 16 when h varies
     int xsub;                  // x sub-cells per support radius requested (GridDesc::xsub is what the grid got)
 
@@ -77,14 +77,14 @@ void sph_prof_end(sph_ctx* c, int rec);
         snprintf((ctx)->err, sizeof((ctx)->err), "launch %s: %s", #kernel, cudaGetErrorString(e__)); \
         return SPH_ERR_CUDA; } } while (0)
 
-struct PackSrc { const float *x, *y, *z, *u, *v, *w, *h, *m, *rho, *p, *ax, *ay, *az, *arho; };
+struct PackSrc { const real *x, *y, *z, *u, *v, *w, *h, *m, *rho, *p, *ax, *ay, *az, *arho; };
 struct PackArgs { PackSrc a[SPH_MAX_ARRAYS]; long long base[SPH_MAX_ARRAYS + 1]; int na; };
-struct OutPtrs { float *x, *y, *z, *u, *v, *w, *rho, *p, *ax, *ay, *az, *arho; };
+struct OutPtrs { real *x, *y, *z, *u, *v, *w, *rho, *p, *ax, *ay, *az, *arho; };
 
 // sph_nnps.cu
 int nnps_pack(sph_ctx* c, const PackArgs& A);        // caller SoA -> float4 groups (unsorted) + h_min/h_max
 int nnps_key_hist(sph_ctx* c);                       // key + rank + histogram from S[cur]
-int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey);
+int nnps_update_key_hist(sph_ctx* c, real dt, bool kick2, bool kick1_drift, bool continuity, bool rekey);
 int nnps_sort_from_keys(sph_ctx* c, bool with_acc);  // scan + scatter (key/rank/cell_count filled); swaps buffers
 int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O);
 int nnps_stencil_candidates(sph_ctx* c, int64_t* out);

@@ -4,7 +4,7 @@
 // the records of launch_search (sph_search.cu) and walks nothing; otherwise the warp searches itself.
 #include "sph_tile.cuh"
 
-struct DensitySrc { float4 pj; float mj; uint32_t aid; };
+struct DensitySrc { real4 pj; real mj; uint32_t aid; };
 
 template <int KERNEL, int DIM, bool VARH, bool FILTER, bool REPLAY, bool UM>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS_DENSITY)
@@ -15,28 +15,53 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
     const int warp_id = i >> 5;
     const bool in = i < n;
-    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
+    uint32_t meta = 0, ci = 0; real4 pi = make_real4(0, 0, 0, 1);
     if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = ld_state(S.posh + i); }
     const uint32_t my_mask = in ? pc.src_mask[meta >> SPH_META_IDX_BITS] : 0u;
     const bool active = my_mask != 0u;
     if (!__any_sync(SPH_FULL_MASK, active)) return;
 
-    const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
-    const float sigma = pc.sigma, hinv_c = pc.hinv_const, fac_c = pc.fac_const, kh = pc.kh;
-    const float hi = VARH ? pi.w : pc.h_const;
-    const float cut2c = pair_cut2(kh, pc.h_const, pc.h_const);
-    const float mfac_c = pc.m_const * pc.fac_const;                     // UM layout: posh.w is p/rho^2, the mass is m_const
-    float2 rho2 = pk1(0.0f);                                            // two partial sums: even / odd candidates of the lane
+    const real Lx = g.Lr[0], Ly = g.Lr[1], Lz = g.Lr[2];
+    const real sigma = pc.sigma, hinv_c = pc.hinv_const, fac_c = pc.fac_const;
+    const real kh = sizeof(real) == 8 ? pc.ksup : pc.kh;               // what pair_cut2 of the build's real type takes
+    const real hi = VARH ? pi.w : pc.h_const;
+    const real cut2c = pair_cut2(kh, pc.h_const, pc.h_const);
+    const real mfac_c = pc.m_const * pc.fac_const;                      // UM layout: posh.w is p/rho^2, the mass is m_const
     unsigned nhits = 0;                                                 // pairs that pass the exact predicate (and the source mask)
     // constant h: posh.w of the sorted state carries the MASS (SortedState), one 16-byte gather per pair.  Plain
     // loads: the epilogue of this launch rewrites .w words of posh / velm that other warps' gathers cover (x, y, z
     // never change and the .w they return is not used then).
     auto load = [&](uint32_t j) {
-        DensitySrc s; s.pj = ld_state(S.posh + j); s.mj = 0.0f; s.aid = 0u;
+        DensitySrc s; s.pj = ld_state(S.posh + j); s.mj = 0; s.aid = 0u;
         if (VARH && !UM) s.mj = ld_state(&S.velm[j].w);            // VU layout (variable h, uniform mass): m = m_const
         if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
         return s;
     };
+#ifdef SPH_REAL_DOUBLE
+    real rho = 0.0;
+    // the double build: one candidate at a time, plain double arithmetic
+    auto compute = [&](const DensitySrc& s, bool has, uint32_t code, auto per) {
+        real dx = rsub(pi.x, s.pj.x), dy = rsub(pi.y, s.pj.y), dz = DIM == 3 ? rsub(pi.z, s.pj.z) : real(0);
+        if (decltype(per)::value) {
+            dx = rsub(dx, img_shift(code, 0, Lx)); dy = rsub(dy, img_shift(code, 1, Ly));
+            if (DIM == 3) dz = rsub(dz, img_shift(code, 2, Lz));
+        }
+        const real r2 = pair_r2(dx, dy, dz);
+        has = has && r2 < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);
+        if (FILTER) has = has && ((my_mask >> s.aid) & 1u);
+        nhits += has ? 1u : 0u;
+        const real r = sqrt(r2);
+        real hinv, mfac;
+        if (VARH) {
+            hinv = real(1) / (real(0.5) * (hi + s.pj.w));
+            mfac = (UM ? pc.m_const : s.mj) * sigma * hinv * hinv * (DIM == 3 ? hinv : real(1));
+        } else { hinv = hinv_c; mfac = UM ? mfac_c : s.pj.w * fac_c; }
+        real f, df;
+        kernel_profile<KERNEL, DIM>(r * hinv, f, df);
+        rho = has ? rfma(mfac, f, rho) : rho;
+    };
+#else
+    float2 rho2 = pk1(0.0f);                                            // two partial sums: even / odd candidates of the lane
     const float2 xi2 = pk1(pi.x), yi2 = pk1(pi.y), zi2 = pk1(pi.z);
     // two candidates (a, b) of this lane at a time, packed f32x2
     auto compute = [&](const DensitySrc& a, const DensitySrc& b, bool ha, bool hb, uint32_t ca, uint32_t cb, auto per) {
@@ -65,27 +90,35 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         mfac = pk(ha ? mfac.x : 0.0f, hb ? mfac.y : 0.0f);              // a candidate that fails contributes nothing
         rho2 = fma2(mfac, f, rho2);
     };
+#endif
 
     TileState st; st.reset(); st.tests = 0;
     const uint32_t idle = in ? (uint32_t)i : 0u;
     auto drain = [&](uint32_t nz, bool shifted) {
+#ifdef SPH_REAL_DOUBLE
+        if (shifted) tile_drain<DensitySrc, 2, true>(ws, nz, idle, load, compute);
+        else         tile_drain<DensitySrc, 2, false>(ws, nz, idle, load, compute);
+#else
         if (shifted) tile_drain2<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, true>(ws, nz, idle, load, compute);
         else         tile_drain2<DensitySrc, TILE_DRAIN_DEPTH_DENSITY, false>(ws, nz, idle, load, compute);
+#endif
     };
     const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
     if (head != SPH_NL_NONE) {
         tile_replay(nl, head, ws, active, drain);
     } else {                                    // no record (or one that did not fit the pool): search
-        tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
+        tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, to_float4(pi), ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
     }
 
     if (active) {
-        const float rho = rho2.x + rho2.y;
-        const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
-        S.rp[i] = make_float2(rho, p / (rho * rho));
+#ifndef SPH_REAL_DOUBLE
+        const real rho = rho2.x + rho2.y;
+#endif
+        const real p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
+        S.rp[i] = make_real2(rho, p / (rho * rho));
         if (!VARH || UM) S.velm[i].w = rho;                             // constant h, or VU layout: velm.w carries rho (SortedState)
         if (UM && !VARH) S.posh[i].w = p / (rho * rho);                 // UM layout: posh.w carries p/rho^2
-        if (!isfinite(rho) || !(rho > 0.0f)) atomicAdd(&counters[CNT_NONFINITE], 1ull);
+        if (!isfinite(rho) || !(rho > real(0))) atomicAdd(&counters[CNT_NONFINITE], 1ull);
     }
     const unsigned long long h = warp_sum_u64(nhits), t = warp_sum_u64((unsigned long long)st.tests);
     if ((threadIdx.x & 31) == 0) { atomicAdd(&counters[CNT_PAIRS_DENSITY], h); atomicAdd(&counters[CNT_CAND_DENSITY], t); }

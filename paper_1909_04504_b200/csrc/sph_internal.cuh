@@ -4,6 +4,20 @@
 #include <stdint.h>
 #include "../../include/sph.h"
 
+// The real type of the particle state and of the field arithmetic: float (libsph_b200.so), or double when built with
+// -DSPH_REAL_DOUBLE (libsph_b200_f64.so; north_star: "1e-12 for an fp64 build flag").  The neighbour SEARCH (cell
+// coordinates, walker, tensor-core filter) always runs in float on float-rounded positions -- it is conservative by
+// construction -- and the exact predicate and every field are evaluated in `real`.
+#ifdef SPH_REAL_DOUBLE
+typedef double real; typedef double2 real2; typedef double4 real4;
+#define make_real2 make_double2
+#define make_real4 make_double4
+#else
+typedef float real; typedef float2 real2; typedef float4 real4;
+#define make_real2 make_float2
+#define make_real4 make_float4
+#endif
+
 #define SPH_FULL_MASK 0xffffffffu
 #define SPH_META_IDX_BITS 28u                    // meta = (array id << 28) | original index
 #define SPH_META_IDX_MASK ((1u << SPH_META_IDX_BITS) - 1u)
@@ -29,6 +43,8 @@ struct GridDesc {
     int per[3];                // periodic per axis
     float lo[3];               // domain origin
     float L[3];                // (float)(hi - lo): the period used by the neighbour predicate (R7)
+    real Lr[3];                // the same in the real type of the build (double build: hi - lo in double)
+    real lor[3], hir[3];       // domain bounds in the real type (periodic wrap of eq.13)
     float hi[3];
     float uabs;                // 2^-23 * largest coordinate magnitude: absolute rounding unit of positions
     LevelDesc lev[SPH_MAX_LEVELS];
@@ -53,27 +69,28 @@ struct NList {
 
 // Per-launch constants of the pair loops.
 struct PairConsts {
-    float kh;                  // k/2: cut = kh * (h_i + h_j)
-    float sigma;               // kernel normalisation sigma_d
-    float h_const;             // constant-h fast path: h, 1/h, sigma/h^d
-    float hinv_const;
-    float fac_const;
-    float rho0, B, gamma;      // Tait EOS
+    real kh;                   // k/2: cut = kh * (h_i + h_j)
+    real ksup;                 // k (the double build forms cut = k * (0.5 * (h_i + h_j)) like the oracle's double predicate)
+    real sigma;                // kernel normalisation sigma_d
+    real h_const;              // constant-h fast path: h, 1/h, sigma/h^d
+    real hinv_const;
+    real fac_const;
+    real rho0, B, gamma;       // Tait EOS
     int   gamma_is_7;
-    float visc;                // -2 alpha c0   (Pi = visc * h vr / ((r2 + eps h^2)(rho_i + rho_j)))
-    float eps;
-    float m_const; int uniform_m;   // constant h and every particle of every array has the same mass: the UM layout
+    real visc;                 // -2 alpha c0   (Pi = visc * h vr / ((r2 + eps h^2)(rho_i + rho_j)))
+    real eps;
+    real m_const; int uniform_m;   // constant h and every particle of every array has the same mass: the UM layout
     int varh_um;               // variable h, uniform mass, gamma = 7 and p = EOS(rho): the VU layout (velm.w = rho, m = m_const)
-    float nu4, eta;            // laminar viscosity eq.10: 4 nu (0 = term off) and its regulariser
-    float g[3];
+    real nu4, eta;             // laminar viscosity eq.10: 4 nu (0 = term off) and its regulariser
+    real g[3];
     uint32_t src_mask[SPH_MAX_ARRAYS];   // per DEST array: source-array bitmask; 0 = not a destination of this launch
     uint32_t all_mask;         // (1 << na) - 1
 };
 
 // Cell-sorted particle state (struct of float4 groups: one 16-B vector load per candidate test).
 struct SortedState {
-    float4* posh;              // x, y, z, h          | constant h (h_min == h_max; the kernels then take h from
-    float4* velm;              // u, v, w, m          | PairConsts): after the sort velm = (u, v, w, RHO) and posh =
+    real4* posh;               // x, y, z, h          | constant h (h_min == h_max; the kernels then take h from
+    real4* velm;               // u, v, w, m          | PairConsts): after the sort velm = (u, v, w, RHO) and posh =
                                //                     | (x, y, z, M), so that the density pair loop gathers ONE 16-byte
                                //                     | word per neighbour and the momentum pair loop TWO (p/rho^2 is
                                //                     | recomputed from rho when p is the EOS of rho).  UM layout (all
@@ -83,8 +100,8 @@ struct SortedState {
                                //                     | the gamma = 7 EOS of rho; PairConsts::varh_um): posh = (x, y, z,
                                //                     | h), velm = (u, v, w, RHO), mass = m_const: the density loop gathers
                                //                     | one word per neighbour, the momentum loop two.
-    float2* rp;                // rho, p / rho^2   (p itself is returned as (p/rho^2) * rho^2)
-    float4* acc;               // ax, ay, az, arho
+    real2* rp;                 // rho, p / rho^2   (p itself is returned as (p/rho^2) * rho^2)
+    real4* acc;                // ax, ay, az, arho
     uint32_t* meta;            // (array << 28) | original index
     uint32_t* cell;            // linear cell id of the particle (x fastest)
 };
@@ -92,6 +109,22 @@ struct SortedState {
 // ---- device math ------------------------------------------------------------------------------
 __device__ __forceinline__ float rcp_approx(float x)  { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_approx(float x){ float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+__device__ __forceinline__ double rcp_approx(double x)  { return 1.0 / x; }
+__device__ __forceinline__ double rsqrt_approx(double x){ return 1.0 / sqrt(x); }
+__device__ __forceinline__ float  rfma(float a, float b, float c)    { return fmaf(a, b, c); }
+__device__ __forceinline__ double rfma(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float  rmax(float a, float b)   { return fmaxf(a, b); }
+__device__ __forceinline__ double rmax(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ float4 ldg_r(const float4* p) { return __ldg(p); }
+__device__ __forceinline__ float2 ldg_r(const float2* p) { return __ldg(p); }
+__device__ __forceinline__ double2 ldg_r(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ double4 ldg_r(const double4* p) {
+    const double2 a = __ldg(reinterpret_cast<const double2*>(p)), b = __ldg(reinterpret_cast<const double2*>(p) + 1);
+    return make_double4(a.x, a.y, b.x, b.y);
+}
+__device__ __forceinline__ float4 to_float4(float4 v)  { return v; }
+__device__ __forceinline__ float4 to_float4(double4 v) { return make_float4((float)v.x, (float)v.y, (float)v.z, (float)v.w); }
 
 // Neighbour predicate, R7 (bit-specified):
 //   d_a = fl(x_i - x_j) - shift_a   (shift_a in {-L_a, 0, +L_a}: the minimum image; exact when 0)
@@ -104,30 +137,42 @@ __device__ __forceinline__ float pair_cut2(float kh, float hi, float hj) {
     return __fmul_rn(cut, cut);
 }
 
+// The double build evaluates DESIGN.md R7 in double as the reference side states it (products and sums rounded one by
+// one, cut = k * (0.5 * (h_i + h_j))), so that the sets stay bit-exact there too.
+__device__ __forceinline__ double pair_r2(double dx, double dy, double dz) {
+    return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
+__device__ __forceinline__ double pair_cut2(double ksup, double hi, double hj) {
+    const double cut = __dmul_rn(ksup, __dmul_rn(0.5, __dadd_rn(hi, hj)));
+    return __dmul_rn(cut, cut);
+}
+__device__ __forceinline__ float  rsub(float a, float b)   { return __fsub_rn(a, b); }
+__device__ __forceinline__ double rsub(double a, double b) { return __dsub_rn(a, b); }
+
 // Dimensionless kernel profile f(q) and f'(q); W = sigma h^-d f, dW/dr = sigma h^-(d+1) f'.
-template <int KERNEL, int DIM>
-__device__ __forceinline__ void kernel_profile(float q, float& f, float& df) {
+template <int KERNEL, int DIM, class T>
+__device__ __forceinline__ void kernel_profile(T q, T& f, T& df) {
     if (KERNEL == SPH_KERNEL_CUBIC) {
-        float t = 2.0f - q;
-        float inner_f  = fmaf(q * q, fmaf(0.75f, q, -1.5f), 1.0f);    // 1 - 1.5 q^2 + 0.75 q^3
-        float inner_df = q * fmaf(2.25f, q, -3.0f);                     // -3 q + 2.25 q^2
-        float outer_f  = 0.25f * t * t * t;
-        float outer_df = -0.75f * t * t;
-        bool in = q < 1.0f;
+        T t = T(2.0) - q;
+        T inner_f  = rfma(q * q, rfma(T(0.75), q, T(-1.5)), T(1.0));    // 1 - 1.5 q^2 + 0.75 q^3
+        T inner_df = q * rfma(T(2.25), q, T(-3.0));                     // -3 q + 2.25 q^2
+        T outer_f  = T(0.25) * t * t * t;
+        T outer_df = T(-0.75) * t * t;
+        bool in = q < T(1.0);
         f  = in ? inner_f : outer_f;
         df = in ? inner_df : outer_df;
-        if (q >= 2.0f) { f = 0.0f; df = 0.0f; }
+        if (q >= T(2.0)) { f = T(0.0); df = T(0.0); }
     } else if (KERNEL == SPH_KERNEL_QUINTIC) {
-        float a = fmaxf(3.0f - q, 0.0f), b = fmaxf(2.0f - q, 0.0f), c = fmaxf(1.0f - q, 0.0f);
-        float a2 = a * a, b2 = b * b, c2 = c * c;
-        float a4 = a2 * a2, b4 = b2 * b2, c4 = c2 * c2;
-        f  = fmaf(15.0f, c4 * c, fmaf(-6.0f, b4 * b, a4 * a));
-        df = fmaf(-75.0f, c4, fmaf(30.0f, b4, -5.0f * a4));
+        T a = rmax(T(3.0) - q, T(0.0)), b = rmax(T(2.0) - q, T(0.0)), c = rmax(T(1.0) - q, T(0.0));
+        T a2 = a * a, b2 = b * b, c2 = c * c;
+        T a4 = a2 * a2, b4 = b2 * b2, c4 = c2 * c2;
+        f  = rfma(T(15.0), c4 * c, rfma(T(-6.0), b4 * b, a4 * a));
+        df = rfma(T(-75.0), c4, rfma(T(30.0), b4, T(-5.0) * a4));
     } else {
-        float t = fmaxf(fmaf(-0.5f, q, 1.0f), 0.0f);
-        float t2 = t * t;
-        if (DIM == 1) { f = t2 * t * fmaf(1.5f, q, 1.0f); df = -3.0f * q * t2; }
-        else          { f = t2 * t2 * fmaf(2.0f, q, 1.0f); df = -5.0f * q * t2 * t; }
+        T t = rmax(rfma(T(-0.5), q, T(1.0)), T(0.0));
+        T t2 = t * t;
+        if (DIM == 1) { f = t2 * t * rfma(T(1.5), q, T(1.0)); df = T(-3.0) * q * t2; }
+        else          { f = t2 * t2 * rfma(T(2.0), q, T(1.0)); df = T(-5.0) * q * t2 * t; }
     }
 }
 
@@ -193,22 +238,27 @@ __host__ __device__ inline double kernel_support(int kernel) { return kernel == 
 // is evaluated from t = (rho - rho0)/rho0 (the subtraction is exact for rho within a factor 2 of rho0):
 //   gamma = 7:  (1+t)^7 - 1 = t (7 + 21 t + 35 t^2 + 35 t^3 + 21 t^4 + 7 t^5 + t^6)   (exact identity)
 //   otherwise:  expm1(gamma * log1p(t))
-__device__ __forceinline__ float eos_pressure(float rho, float rho0, float B, float gamma, int gamma_is_7) {
-    const float t = (rho - rho0) / rho0;
-    float s;
-    if (gamma_is_7) s = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.0f, 7.0f), 21.0f), 35.0f), 35.0f), 21.0f), 7.0f);
-    else s = expm1f(gamma * log1pf(t));
+__device__ __forceinline__ float  eos_general(float gamma, float t)   { return expm1f(gamma * log1pf(t)); }
+__device__ __forceinline__ double eos_general(double gamma, double t) { return expm1(gamma * log1p(t)); }
+template <class T>
+__device__ __forceinline__ T eos_pressure(T rho, T rho0, T B, T gamma, int gamma_is_7) {
+    const T t = (rho - rho0) / rho0;
+    T s;
+    if (gamma_is_7) s = t * rfma(t, rfma(t, rfma(t, rfma(t, rfma(t, rfma(t, T(1.0), T(7.0)), T(21.0)), T(35.0)), T(35.0)), T(21.0)), T(7.0));
+    else s = eos_general(gamma, t);
     return B * s;
 }
 
 // p/rho^2 of the Tait EOS with gamma = 7 from rho alone (the momentum pair loop recomputes it per neighbour
 // instead of gathering it): same polynomial as eos_pressure, t formed with a multiplication by 1/rho0.
-__device__ __forceinline__ float eos7_p(float rho, float rho0, float inv_rho0, float B) {
-    const float t = (rho - rho0) * inv_rho0;
-    const float s = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.0f, 7.0f), 21.0f), 35.0f), 35.0f), 21.0f), 7.0f);
+template <class T>
+__device__ __forceinline__ T eos7_p(T rho, T rho0, T inv_rho0, T B) {
+    const T t = (rho - rho0) * inv_rho0;
+    const T s = t * rfma(t, rfma(t, rfma(t, rfma(t, rfma(t, rfma(t, T(1.0), T(7.0)), T(21.0)), T(35.0)), T(35.0)), T(21.0)), T(7.0));
     return B * s;
 }
-__device__ __forceinline__ float eos7_p_over_rho2(float rho, float rho0, float inv_rho0, float B) {
+template <class T>
+__device__ __forceinline__ T eos7_p_over_rho2(T rho, T rho0, T inv_rho0, T B) {
     return eos7_p(rho, rho0, inv_rho0, B) * rcp_approx(rho * rho);
 }
 

@@ -9,7 +9,7 @@
 // ------------------------------------------------------------------------------------------------
 // cell of a position (a1).  Linear key, x fastest, so the 3 x-adjacent cells of a stencil row are one run.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, int level, bool& oob) {
+__device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, int level, bool& oob) {   // float-rounded position: the search runs in float
     const LevelDesc& Lv = g.lev[level];
     int c[3]; const float x[3] = { p.x, p.y, p.z };
     oob = false;
@@ -24,39 +24,48 @@ __device__ __forceinline__ uint32_t cell_of(const GridDesc& g, float4 p, int lev
     return Lv.base + (uint32_t)((c[2] * Lv.nc[1] + c[1]) * Lv.nc[0] + c[0]);
 }
 
-// Loads the caller's SoA arrays into the (not yet sorted) float4 groups and reduces h_min / h_max.
+// positive reals order like their bit patterns: min/max through integer atomics
+#ifdef SPH_REAL_DOUBLE
+typedef long long real_bits;
+__device__ __forceinline__ real_bits real_as_bits(double x) { return __double_as_longlong(x); }
+#else
+typedef int real_bits;
+__device__ __forceinline__ real_bits real_as_bits(float x) { return __float_as_int(x); }
+#endif
+__device__ __forceinline__ real_bits shfl_xor_bits(real_bits v, int o) { return __shfl_xor_sync(SPH_FULL_MASK, v, o); }
+
+// Loads the caller's SoA arrays into the (not yet sorted) real4 groups and reduces h_min / h_max, |m|_min / |m|_max.
 __global__ void __launch_bounds__(NB)
-k_pack(PackArgs A, SortedState S, int n, PairConsts pc, int* __restrict__ hminmax) {
+k_pack(PackArgs A, SortedState S, int n, PairConsts pc, real_bits* __restrict__ hminmax) {
     const int gidx = blockIdx.x * NB + threadIdx.x;
-    float hmin = 3.0e38f, hmax = 0.0f, mmin = 3.0e38f, mmax = 0.0f;
+    real hmin = real(3.0e38), hmax = 0, mmin = real(3.0e38), mmax = 0;
     if (gidx < n) {
         int a = 0;
         while (a + 1 < A.na && gidx >= A.base[a + 1]) ++a;
         const long long i = gidx - A.base[a];
         const PackSrc s = A.a[a];
-        const float h = s.h[i];
-        const float rho = s.rho ? s.rho[i] : pc.rho0;
-        const float p = s.p ? s.p[i] : eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
-        S.posh[gidx] = make_float4(s.x[i], s.y[i], s.z ? s.z[i] : 0.0f, h);
-        S.velm[gidx] = make_float4(s.u ? s.u[i] : 0.0f, s.v ? s.v[i] : 0.0f, s.w ? s.w[i] : 0.0f, s.m ? s.m[i] : 0.0f);
-        S.rp[gidx] = make_float2(rho, p / (rho * rho));
+        const real h = s.h[i];
+        const real rho = s.rho ? s.rho[i] : pc.rho0;
+        const real p = s.p ? s.p[i] : eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
+        S.posh[gidx] = make_real4(s.x[i], s.y[i], s.z ? s.z[i] : real(0), h);
+        S.velm[gidx] = make_real4(s.u ? s.u[i] : real(0), s.v ? s.v[i] : real(0), s.w ? s.w[i] : real(0), s.m ? s.m[i] : real(0));
+        S.rp[gidx] = make_real2(rho, p / (rho * rho));
         S.meta[gidx] = ((uint32_t)a << SPH_META_IDX_BITS) | (uint32_t)i;
-        S.acc[gidx] = make_float4(s.ax ? s.ax[i] : 0.0f, s.ay ? s.ay[i] : 0.0f, s.az ? s.az[i] : 0.0f,
-                                  s.arho ? s.arho[i] : 0.0f);
+        S.acc[gidx] = make_real4(s.ax ? s.ax[i] : real(0), s.ay ? s.ay[i] : real(0), s.az ? s.az[i] : real(0),
+                                 s.arho ? s.arho[i] : real(0));
         hmin = hmax = h;
-        mmin = mmax = fabsf(s.m ? s.m[i] : 0.0f);
+        mmin = mmax = fabs(s.m ? s.m[i] : real(0));
     }
+    real_bits bhmin = real_as_bits(hmin), bhmax = real_as_bits(hmax), bmmin = real_as_bits(mmin), bmmax = real_as_bits(mmax);
     for (int o = 16; o > 0; o >>= 1) {
-        hmin = fminf(hmin, __shfl_xor_sync(SPH_FULL_MASK, hmin, o));
-        hmax = fmaxf(hmax, __shfl_xor_sync(SPH_FULL_MASK, hmax, o));
-        mmin = fminf(mmin, __shfl_xor_sync(SPH_FULL_MASK, mmin, o));
-        mmax = fmaxf(mmax, __shfl_xor_sync(SPH_FULL_MASK, mmax, o));
+        bhmin = min(bhmin, shfl_xor_bits(bhmin, o)); bhmax = max(bhmax, shfl_xor_bits(bhmax, o));
+        bmmin = min(bmmin, shfl_xor_bits(bmmin, o)); bmmax = max(bmmax, shfl_xor_bits(bmmax, o));
     }
-    if ((threadIdx.x & 31) == 0 && hmax > 0.0f) {      // positive floats order like their bit patterns
-        atomicMin(&hminmax[0], __float_as_int(hmin));
-        atomicMax(&hminmax[1], __float_as_int(hmax));
-        atomicMin(&hminmax[2], __float_as_int(mmin));          // |m|: uniform mass is detected for the UM state layout
-        atomicMax(&hminmax[3], __float_as_int(mmax));
+    if ((threadIdx.x & 31) == 0 && bhmax > 0) {        // positive reals order like their bit patterns
+        atomicMin(&hminmax[0], bhmin);
+        atomicMax(&hminmax[1], bhmax);
+        atomicMin(&hminmax[2], bmmin);                 // |m|: uniform mass is detected for the UM / VU state layouts
+        atomicMax(&hminmax[3], bmmax);
     }
 }
 
@@ -66,7 +75,7 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
     bool oob;
-    const float4 p = S.posh[i];                                       // posh.w is still h here (k_pack; the layouts change at the sort)
+    const float4 p = to_float4(S.posh[i]);                            // posh.w is still h here (k_pack; the layouts change at the sort)
     const uint32_t cell = cell_of(g, p, level_of_h(g, p.w), oob);
     const uint32_t k = cell * (uint32_t)g.na + (S.meta[i] >> SPH_META_IDX_BITS);
     key[i] = k;
@@ -80,7 +89,7 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
 // way on EVERY array (the tank particles too, L142) and re-evaluates the EOS (group 1 of Listing 3).
 // ------------------------------------------------------------------------------------------------
 struct UpdateArgs {
-    float dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho, w_prr, euler, zero_cnt;
+    real dt_half, dt; int kick2, kick1, move, continuity, rekey, w_rho, w_prr, euler, zero_cnt;
     int fixed[SPH_MAX_ARRAYS];
 };
 
@@ -93,48 +102,49 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
     // (no separate memset node per step)
     if (U.zero_cnt && i < CNT_COUNT - CNT_PAIRS_DENSITY) counters[CNT_PAIRS_DENSITY + i] = 0ull;
     if (i >= n) return;
-    float4 pos = S.posh[i];
+    real4 pos = S.posh[i];
     const uint32_t meta = S.meta[i];
     const uint32_t aid = meta >> SPH_META_IDX_BITS;
-    const float4 a = S.acc[i];
+    const real4 a = S.acc[i];
     if (!U.fixed[aid]) {
-        float4 vel = S.velm[i];
+        real4 vel = S.velm[i];
         if (U.kick2) {                                                  // eq.14
-            vel.x = fmaf(U.dt_half, a.x, vel.x); vel.y = fmaf(U.dt_half, a.y, vel.y);
-            if (g.dim == 3) vel.z = fmaf(U.dt_half, a.z, vel.z);
+            vel.x = rfma(U.dt_half, a.x, vel.x); vel.y = rfma(U.dt_half, a.y, vel.y);
+            if (g.dim == 3) vel.z = rfma(U.dt_half, a.z, vel.z);
         }
         if (U.euler && U.move) {                                        // forward Euler: x^{n+1} = x^n + dt u^n (old u)
-            pos.x = fmaf(U.dt, vel.x, pos.x); pos.y = fmaf(U.dt, vel.y, pos.y);
-            if (g.dim == 3) pos.z = fmaf(U.dt, vel.z, pos.z);
+            pos.x = rfma(U.dt, vel.x, pos.x); pos.y = rfma(U.dt, vel.y, pos.y);
+            if (g.dim == 3) pos.z = rfma(U.dt, vel.z, pos.z);
         }
         if (U.kick1) {
-            vel.x = fmaf(U.dt_half, a.x, vel.x); vel.y = fmaf(U.dt_half, a.y, vel.y);   // eq.12
-            if (g.dim == 3) vel.z = fmaf(U.dt_half, a.z, vel.z);
+            vel.x = rfma(U.dt_half, a.x, vel.x); vel.y = rfma(U.dt_half, a.y, vel.y);   // eq.12
+            if (g.dim == 3) vel.z = rfma(U.dt_half, a.z, vel.z);
             if (U.move) {                                                // eq.13 + periodic wrap
                 if (!U.euler) {
-                    pos.x = fmaf(U.dt, vel.x, pos.x); pos.y = fmaf(U.dt, vel.y, pos.y);
-                    if (g.dim == 3) pos.z = fmaf(U.dt, vel.z, pos.z);
+                    pos.x = rfma(U.dt, vel.x, pos.x); pos.y = rfma(U.dt, vel.y, pos.y);
+                    if (g.dim == 3) pos.z = rfma(U.dt, vel.z, pos.z);
                 }
-                if (g.per[0]) { if (pos.x >= g.hi[0]) pos.x -= g.L[0]; else if (pos.x < g.lo[0]) pos.x += g.L[0]; }
-                if (g.per[1]) { if (pos.y >= g.hi[1]) pos.y -= g.L[1]; else if (pos.y < g.lo[1]) pos.y += g.L[1]; }
-                if (g.dim == 3 && g.per[2]) { if (pos.z >= g.hi[2]) pos.z -= g.L[2]; else if (pos.z < g.lo[2]) pos.z += g.L[2]; }
+                if (g.per[0]) { if (pos.x >= g.hir[0]) pos.x -= g.Lr[0]; else if (pos.x < g.lor[0]) pos.x += g.Lr[0]; }
+                if (g.per[1]) { if (pos.y >= g.hir[1]) pos.y -= g.Lr[1]; else if (pos.y < g.lor[1]) pos.y += g.Lr[1]; }
+                if (g.dim == 3 && g.per[2]) { if (pos.z >= g.hir[2]) pos.z -= g.Lr[2]; else if (pos.z < g.lor[2]) pos.z += g.Lr[2]; }
                 S.posh[i] = pos;
             }
         }
         S.velm[i] = vel;
     }
     if (U.continuity) {
-        float rho = S.rp[i].x;
-        if (U.kick2) rho = fmaf(U.dt_half, a.w, rho);
-        if (U.kick1) rho = fmaf(U.dt_half, a.w, rho);
-        const float p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
-        S.rp[i] = make_float2(rho, p / (rho * rho));
+        real rho = S.rp[i].x;
+        if (U.kick2) rho = rfma(U.dt_half, a.w, rho);
+        if (U.kick1) rho = rfma(U.dt_half, a.w, rho);
+        const real p = eos_pressure(rho, pc.rho0, pc.B, pc.gamma, pc.gamma_is_7);
+        S.rp[i] = make_real2(rho, p / (rho * rho));
         if (U.w_rho) S.velm[i].w = rho;         // constant h: velm.w of the sorted state carries rho (SortedState)
         if (U.w_prr) S.posh[i].w = p / (rho * rho);   // ... and, with uniform mass, posh.w carries p/rho^2
     }
     if (U.rekey) {
         bool oob;
-        const uint32_t cell = cell_of(g, pos, g.nlev > 1 ? level_of_h(g, pos.w) : 0, oob);   // several levels only when h varies: posh.w = h
+        const float4 posf = to_float4(pos);
+        const uint32_t cell = cell_of(g, posf, g.nlev > 1 ? level_of_h(g, posf.w) : 0, oob);   // several levels only when h varies: posh.w = h
         const uint32_t k = cell * (uint32_t)g.na + aid;
         key[i] = k;
         rank[i] = atomicAdd(&cell_count[k], 1u);
@@ -244,9 +254,9 @@ k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass,
     if (i >= n) return;
     const uint32_t k = key[i];
     const uint32_t d = cell_start[k] + rank[i];
-    float4 p = A.posh[i];
-    float4 v = A.velm[i];
-    const float2 r = A.rp[i];
+    real4 p = A.posh[i];
+    real4 v = A.velm[i];
+    const real2 r = A.rp[i];
     // first sort after the pack (SortedState).  constant h: velm.w <- rho; posh.w <- m, or <- p/rho^2 when the mass is uniform
     if (w_mass == 3) v.w = r.x;                                      // VU layout (variable h): velm.w <- rho, posh.w stays h
     else if (w_mass) { p.w = w_mass == 2 ? r.y : v.w; v.w = r.x; }
@@ -267,12 +277,12 @@ int nnps_key_hist(sph_ctx* c) {
     return SPH_OK;
 }
 
-int nnps_update_key_hist(sph_ctx* c, float dt, bool kick2, bool kick1_drift, bool continuity, bool rekey) {
+int nnps_update_key_hist(sph_ctx* c, real dt, bool kick2, bool kick1_drift, bool continuity, bool rekey) {
     const bool kick_only = kick2 && !kick1_drift;
     const int n = (int)c->n_total;
     UpdateArgs U;
     U.euler = c->prm.integrator == SPH_INTEGRATOR_EULER ? 1 : 0;
-    U.dt_half = U.euler ? dt : 0.5f * dt;              // Euler: the one kick per step is a full dt
+    U.dt_half = U.euler ? dt : real(0.5) * dt;              // Euler: the one kick per step is a full dt
     U.dt = dt; U.kick2 = kick2; U.kick1 = kick1_drift; U.move = c->prm.move;
     U.continuity = continuity; U.rekey = rekey; U.zero_cnt = rekey ? 1 : 0; U.w_rho = (!c->variable_h || c->pc.varh_um) ? 1 : 0; U.w_prr = (!c->variable_h && c->pc.uniform_m) ? 1 : 0;
     for (int a = 0; a < SPH_MAX_ARRAYS; ++a) U.fixed[a] = a < c->na ? c->fixed[a] : 1;
@@ -304,11 +314,11 @@ k_gather_out(SortedState S, int n, uint32_t array, OutPtrs O) {
     const uint32_t meta = S.meta[i];
     if ((meta >> SPH_META_IDX_BITS) != array) return;
     const uint32_t o = meta & SPH_META_IDX_MASK;
-    if (O.x || O.y || O.z) { const float4 p = S.posh[i]; if (O.x) O.x[o] = p.x; if (O.y) O.y[o] = p.y; if (O.z) O.z[o] = p.z; }
-    if (O.u || O.v || O.w) { const float4 v = S.velm[i]; if (O.u) O.u[o] = v.x; if (O.v) O.v[o] = v.y; if (O.w) O.w[o] = v.z; }
-    if (O.rho || O.p) { const float2 r = S.rp[i]; if (O.rho) O.rho[o] = r.x; if (O.p) O.p[o] = r.y * r.x * r.x; }
+    if (O.x || O.y || O.z) { const real4 p = S.posh[i]; if (O.x) O.x[o] = p.x; if (O.y) O.y[o] = p.y; if (O.z) O.z[o] = p.z; }
+    if (O.u || O.v || O.w) { const real4 v = S.velm[i]; if (O.u) O.u[o] = v.x; if (O.v) O.v[o] = v.y; if (O.w) O.w[o] = v.z; }
+    if (O.rho || O.p) { const real2 r = S.rp[i]; if (O.rho) O.rho[o] = r.x; if (O.p) O.p[o] = r.y * r.x * r.x; }
     if (O.ax || O.ay || O.az || O.arho) {
-        const float4 a = S.acc[i];
+        const real4 a = S.acc[i];
         if (O.ax) O.ax[o] = a.x; if (O.ay) O.ay[o] = a.y; if (O.az) O.az[o] = a.z; if (O.arho) O.arho[o] = a.w;
     }
 }
@@ -322,7 +332,7 @@ int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O) {
 // ------------------------------------------------------------------------------------------------
 // neighbour-list export (verification): the same warp-tile walker and predicate code as the pair kernels.
 // ------------------------------------------------------------------------------------------------
-struct NbSrc { float4 pj; uint32_t meta; };
+struct NbSrc { real4 pj; uint32_t meta; };
 
 template <int DIM, bool VARH, bool FILL>
 __global__ void __launch_bounds__(TILE_BLOCK)
@@ -333,21 +343,21 @@ k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __res
     TileWarpSmem& ws = smem[threadIdx.x >> 5];
     const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
     const bool in = i < n;
-    uint32_t meta = 0, ci = 0; float4 pi = make_float4(0, 0, 0, 1);
+    uint32_t meta = 0, ci = 0; real4 pi = make_real4(0, 0, 0, 1);
     if (in) { meta = S.meta[i]; ci = S.cell[i]; pi = S.posh[i]; }
     const bool active = in && (meta >> SPH_META_IDX_BITS) == dest;
     if (!__any_sync(SPH_FULL_MASK, active)) return;
     const uint32_t o = meta & SPH_META_IDX_MASK;
-    const float hi = VARH ? pi.w : pc.h_const, kh = pc.kh;
-    const float cut2c = pair_cut2(kh, pc.h_const, pc.h_const);
+    const real hi = VARH ? pi.w : pc.h_const, kh = sizeof(real) == 8 ? pc.ksup : pc.kh;
+    const real cut2c = pair_cut2(kh, pc.h_const, pc.h_const);
     uint32_t cnt = 0;
     int32_t* out = FILL ? indices + (active ? offsets[o] : 0u) : nullptr;
-    auto load = [&](uint32_t j) { NbSrc s; s.pj = __ldg(S.posh + j); s.meta = __ldg(S.meta + j); return s; };
+    auto load = [&](uint32_t j) { NbSrc s; s.pj = ldg_r(S.posh + j); s.meta = __ldg(S.meta + j); return s; };
     auto compute = [&](const NbSrc& s, bool has, uint32_t code, auto per) {
-        float dx = __fsub_rn(pi.x, s.pj.x), dy = __fsub_rn(pi.y, s.pj.y), dz = DIM == 3 ? __fsub_rn(pi.z, s.pj.z) : 0.0f;
+        real dx = rsub(pi.x, s.pj.x), dy = rsub(pi.y, s.pj.y), dz = DIM == 3 ? rsub(pi.z, s.pj.z) : real(0);
         if (decltype(per)::value) {
-            dx = __fsub_rn(dx, img_shift(code, 0, g.L[0])); dy = __fsub_rn(dy, img_shift(code, 1, g.L[1]));
-            if (DIM == 3) dz = __fsub_rn(dz, img_shift(code, 2, g.L[2]));
+            dx = rsub(dx, img_shift(code, 0, g.Lr[0])); dy = rsub(dy, img_shift(code, 1, g.Lr[1]));
+            if (DIM == 3) dz = rsub(dz, img_shift(code, 2, g.Lr[2]));
         }
         has = has && pair_r2(dx, dy, dz) < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);     // the exact predicate R7
         if (!has || (s.meta >> SPH_META_IDX_BITS) != src) return;
@@ -356,7 +366,7 @@ k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __res
     };
     TileState st; st.reset(); st.tests = 0;
     const uint32_t idle = in ? (uint32_t)i : 0u;
-    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, pi, ci, ws, st, [&]() {
+    tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, to_float4(pi), ci, ws, st, [&]() {
         if (st.shifted) tile_drain<NbSrc, 2, true>(ws, st.nz, idle, load, compute);
         else            tile_drain<NbSrc, 2, false>(ws, st.nz, idle, load, compute);
         st.reset(); });
@@ -417,9 +427,11 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
 // ------------------------------------------------------------------------------------------------
 int nnps_pack(sph_ctx* c, const PackArgs& A) {
     const int n = (int)c->n_total;
-    const int init[4] = { 0x7f7fffff, 0, 0x7f7fffff, 0 };
+    const real big = real(3.0e38);
+    real_bits init[4] = { 0, 0, 0, 0 };
+    memcpy(&init[0], &big, sizeof(real)); memcpy(&init[2], &big, sizeof(real));
     SPH_CUDA_OK(c, cudaMemcpyAsync(c->hminmax, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
-    if (n) SPH_LAUNCH(c, SPH_K_PACK, k_pack, (n + NB - 1) / NB, NB, 0, A, c->S[c->cur], n, c->pc, (int*)c->hminmax);
+    if (n) SPH_LAUNCH(c, SPH_K_PACK, k_pack, (n + NB - 1) / NB, NB, 0, A, c->S[c->cur], n, c->pc, (real_bits*)c->hminmax);
     return SPH_OK;
 }
 
@@ -440,7 +452,7 @@ k_coarse_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ cnt) {
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
     int c[3], nc[3];
-    coarse_coords(g, S.posh[i], c, nc);
+    coarse_coords(g, to_float4(S.posh[i]), c, nc);
     atomicAdd(&cnt[(c[2] * nc[1] + c[1]) * nc[0] + c[0]], 1u);
 }
 __global__ void __launch_bounds__(NB)
@@ -449,7 +461,7 @@ k_coarse_sum(GridDesc g, SortedState S, int n, const uint32_t* __restrict__ cnt,
     unsigned long long sum = 0ull;
     if (i < n) {
         int c[3], nc[3];
-        coarse_coords(g, S.posh[i], c, nc);
+        coarse_coords(g, to_float4(S.posh[i]), c, nc);
         for (int dz = (g.dim == 3 ? -1 : 0); dz <= (g.dim == 3 ? 1 : 0); ++dz)
             for (int dy = -1; dy <= 1; ++dy)
                 for (int dx = -1; dx <= 1; ++dx) {

@@ -16,7 +16,7 @@ k_search_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restri
     const int warp_id = i >> 5;
     const bool in = i < n;
     uint32_t ci = 0; float4 pi = make_float4(0, 0, 0, 1);
-    if (in) { ci = S.cell[i]; pi = __ldg(S.posh + i); }
+    if (in) { ci = S.cell[i]; pi = to_float4(ldg_r(S.posh + i)); }
     TileState st; st.reset(); st.tests = 0;
     TileRecorder rec; rec.init(nl);
     tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, in, in, pi, ci, ws, st,

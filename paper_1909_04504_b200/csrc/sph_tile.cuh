@@ -93,9 +93,10 @@ __device__ __forceinline__ float warp_min_f(float v) { return ord2f(__reduce_min
 __device__ __forceinline__ float warp_max_f(float v) { return ord2f(__reduce_max_sync(SPH_FULL_MASK, f2ord(v))); }
 
 // minimum-image shift of a batch on one axis from its code: d = fl(x_i - x_j) - shift (R7)
-__device__ __forceinline__ float img_shift(uint32_t code, int axis, float L) {
+template <class T>
+__device__ __forceinline__ T img_shift(uint32_t code, int axis, T L) {
     const uint32_t c = (code >> (2 * axis)) & 3u;
-    return c == 1u ? -L : (c == 2u ? L : 0.0f);
+    return c == 1u ? -L : (c == 2u ? L : T(0));
 }
 
 // D = A (16 x 8, tf32, row) * B (8 x 8, tf32, col), fp32 accumulators starting from zero
@@ -111,13 +112,15 @@ __device__ __forceinline__ void mma_tf32_16x8x8(float (&c)[4], const uint32_t (&
 // launch; pi = (x, y, z, h); ci = its cell id (level base + linear cell).
 template <int DIM, bool VARH, class Drain>
 __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& pc,
-                                          const float4* posh, const uint32_t* __restrict__ cell_start,
+                                          const real4* posh, const uint32_t* __restrict__ cell_start,
                                           bool active, bool in, float4 pi, uint32_t ci,
                                           TileWarpSmem& ws, TileState& st, Drain&& drain) {
     const int lane = threadIdx.x & 31, gq = lane >> 2, tq = lane & 3;
     const int na = g.na, nlev = VARH ? g.nlev : 1;
-    const float khsq = pc.kh * pc.kh;
-    const float cut2c = pair_cut2(pc.kh, pc.h_const, pc.h_const);
+    // the search runs in float whatever the real type of the build (see sph_internal.cuh)
+    const float khf = (float)pc.kh, hcf = (float)pc.h_const;
+    const float khsq = khf * khf;
+    const float cut2c = pair_cut2(khf, hcf, hcf);
 
     // own cell -> (level, stencil row, x sub-cell); groups: maximal lane ranges of one level and row without an x
     // gap wider than two coarse cells (a wider gap means the windows of its two sides are disjoint)
@@ -156,7 +159,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
 
     auto load_batch = [&](uint32_t bb, uint32_t ee) -> float4 {
         const uint32_t j = bb + (uint32_t)lane;
-        return j < ee ? ld_state(posh + j) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        return j < ee ? to_float4(ld_state(posh + j)) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     };
     auto pop_run = [&]() -> bool {
         if (!segs) return false;
@@ -177,7 +180,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         const float big = 3.0e38f;
         const float xmin = warp_min_f(ing ? pi.x : big), xmax = warp_max_f(ing ? pi.x : -big);
         const float ymin = warp_min_f(ing ? pi.y : big), ymax = warp_max_f(ing ? pi.y : -big);
-        float zmin = 0.0f, zmax = 0.0f, hg = pc.h_const;
+        float zmin = 0.0f, zmax = 0.0f, hg = hcf;
         if (DIM == 3) { zmin = warp_min_f(ing ? pi.z : big); zmax = warp_max_f(ing ? pi.z : -big); }
         if (VARH) hg = __uint_as_float(__reduce_max_sync(SPH_FULL_MASK, ing ? __float_as_uint(pi.w) : 0u));
         ox = 0.5f * (xmin + xmax); oy = 0.5f * (ymin + ymax); oz = DIM == 3 ? 0.5f * (zmin + zmax) : 0.0f;
@@ -205,7 +208,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
     auto setup_level = [&]() {
         const LevelDesc& Lv = g.lev[b];
         const float xmin = ws.bb[0], xmax = ws.bb[1], ymin = ws.bb[2], ymax = ws.bb[3], zmin = ws.bb[4], zmax = ws.bb[5];
-        const float R = pc.kh * (ws.bb[6] + (VARH ? Lv.hmax : pc.h_const)) * 1.0001f + 16.0f * g.uabs;
+        const float R = khf * (ws.bb[6] + (VARH ? Lv.hmax : hcf)) * 1.0001f + 16.0f * g.uabs;
         const float X = ws.bb[7] + R;                          // bound of every tile-local coordinate that matters
         // filter margin: bounds the tf32 rounding of operands and accumulation
         nsub = (R * X + R * R) * (1.0f / 256.0f) + X * X * (1.0f / 32768.0f) + 64.0f * g.uabs * (R + X) + (VARH ? 0.0f : cut2c);

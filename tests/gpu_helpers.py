@@ -21,7 +21,7 @@ def assert_close(got, want, name, tol=TOL):
 def make_ctx(wl, arrays=None, **over):
     from paper_1909_04504_b200 import binding
     ctx = binding.SphContext.from_workload(wl, **over)
-    arrays = arrays if arrays is not None else binding.device_arrays(wl)
+    arrays = arrays if arrays is not None else binding.device_arrays(wl, precision=over.get("precision", "f32"))
     ctx.nnps_build(arrays, [a.fixed for a in wl.arrays])
     return ctx, arrays
 

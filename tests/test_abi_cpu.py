@@ -13,11 +13,14 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "sph.h")
 
 
-@pytest.fixture(scope="module")
-def lib():
+@pytest.fixture(scope="module", params=["f32", "f64"])
+def lib(request):
+    """libsph_b200.so (sph_real = float) and libsph_b200_f64.so (the same sources with -DSPH_REAL_DOUBLE)"""
     from paper_1909_04504_b200 import build, binding
-    build.build()
-    return binding.load()
+    build.build(precision=request.param)
+    L = binding.load(request.param)
+    assert L.sph_real_size() == (4 if request.param == "f32" else 8)
+    return L
 
 
 def _declared():
