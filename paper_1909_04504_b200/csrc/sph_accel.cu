@@ -64,6 +64,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     real ax = pc.g[0], ay = pc.g[1], az = pc.g[2], ar = 0.0f;      // gravity = accumulator init (Listing 4)
     unsigned nhits = 0;                                                 // pairs that pass the exact predicate (and the source mask)
     auto load = [&](uint32_t j) {
+        SPH_DBG_ASSERT(j < g.n_sorted, g);
         AccelSrc s; s.pj = ldg_r(S.posh + j); s.vj = ldg_r(S.velm + j); s.aid = 0u;
         s.rj = PM ? make_real2(0.0f, 0.0f) : ldg_r(S.rp + j);
         if (FILTER) { if (my_mask != pc.all_mask) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS; }   // lanes fed by all arrays skip the gather
@@ -123,7 +124,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     TileState st; st.reset(); st.tests = 0;
     const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
     if (head != SPH_NL_NONE) {
-        tile_replay(nl, head, ws, active, drain);
+        tile_replay(g, nl, head, ws, active, drain);
     } else {                                    // no record (or one that did not fit the pool): search
         tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, to_float4(pi), ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
     }

@@ -229,7 +229,7 @@ static int size_grid(sph_ctx* c) {
             if (total > ((int64_t)1 << 30)) ok = false;
         }
         g.nlev = nlev;
-        if (ok && total * c->na <= c->max_keys) { c->n_keys = total * c->na; return SPH_OK; }
+        if (ok && total * c->na <= c->max_keys) { c->n_keys = total * c->na; g.cells_total = (uint32_t)total; g.n_sorted = (uint32_t)c->n_total; g.dbg = c->counters; return SPH_OK; }
         if (xsub > 1) xsub /= 2; else if (nlev > 1) --nlev; else scale *= 1.26;
     }
     return sph_fail(c, SPH_ERR_CAPACITY, "cell table too small for this domain / h_max");
@@ -530,6 +530,7 @@ extern "C" int sph_synchronize(sph_ctx* c) {
     int rc = read_counters(c, h); if (rc) return rc;
     if (h[CNT_OUT_OF_DOMAIN]) { snprintf(c->err, sizeof(c->err), "%llu particle updates fell outside the non-periodic domain box", h[CNT_OUT_OF_DOMAIN]); return SPH_ERR_OUT_OF_DOMAIN; }
     if (h[CNT_NONFINITE]) { snprintf(c->err, sizeof(c->err), "%llu non-finite results", h[CNT_NONFINITE]); return SPH_ERR_NONFINITE; }
+    if (h[CNT_ASSERT]) { snprintf(c->err, sizeof(c->err), "%llu device-side bounds assertions failed (SPH_DEBUG_ASSERT build)", h[CNT_ASSERT]); return SPH_ERR_CUDA; }
     return SPH_OK;
 }
 

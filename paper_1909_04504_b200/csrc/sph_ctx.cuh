@@ -6,7 +6,7 @@
 // device counters: [2..5] are cleared by every evaluation / pair call, [6..8] by every search
 enum { CNT_OUT_OF_DOMAIN = 0, CNT_NONFINITE = 1, CNT_PAIRS_DENSITY = 2, CNT_CAND_DENSITY = 3, CNT_PAIRS_ACCEL = 4,
        CNT_CAND_ACCEL = 5, CNT_OVERFLOW = 6, CNT_NL_USED = 7 /* low 32 bits: record rows handed out (NList::used) */,
-       CNT_CAND_SEARCH = 8, CNT_COUNT = 9 };
+       CNT_CAND_SEARCH = 8, CNT_ASSERT = SPH_CNT_ASSERT /* failed device-side bounds assertions (-DSPH_DEBUG_ASSERT builds) */, CNT_COUNT = 10 };
 
 struct sph_ctx {
     cudaStream_t stream;

@@ -32,6 +32,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     // loads: the epilogue of this launch rewrites .w words of posh / velm that other warps' gathers cover (x, y, z
     // never change and the .w they return is not used then).
     auto load = [&](uint32_t j) {
+        SPH_DBG_ASSERT(j < g.n_sorted, g);
         DensitySrc s; s.pj = ld_state(S.posh + j); s.mj = 0; s.aid = 0u;
         if (VARH && !UM) s.mj = ld_state(&S.velm[j].w);            // VU layout (variable h, uniform mass): m = m_const
         if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
@@ -105,7 +106,7 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     };
     const uint32_t head = REPLAY ? __ldg(nl.head + warp_id) : SPH_NL_NONE;
     if (head != SPH_NL_NONE) {
-        tile_replay(nl, head, ws, active, drain);
+        tile_replay(g, nl, head, ws, active, drain);
     } else {                                    // no record (or one that did not fit the pool): search
         tile_walk<DIM, VARH>(g, pc, S.posh, cell_start, active, in, to_float4(pi), ci, ws, st, [&]() { drain(st.nz, st.shifted); st.reset(); });
     }

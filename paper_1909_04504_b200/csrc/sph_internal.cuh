@@ -47,8 +47,19 @@ struct GridDesc {
     real lor[3], hir[3];       // domain bounds in the real type (periodic wrap of eq.13)
     float hi[3];
     float uabs;                // 2^-23 * largest coordinate magnitude: absolute rounding unit of positions
+    uint32_t n_sorted, cells_total;    // particles in the sorted order, cells of all level grids (bounds of the tables)
+    unsigned long long* dbg;   // the context's device counters: -DSPH_DEBUG_ASSERT builds count failed bounds assertions there
     LevelDesc lev[SPH_MAX_LEVELS];
 };
+// Opt-in device-side bounds assertions (build with -DSPH_DEBUG_ASSERT; compute-sanitizer is closed on this pool): record-pool
+// rows, cell-table and sorted-order indices, scan tiles.  A failure is counted and reported by the next [sync] call.
+#define SPH_CNT_ASSERT 9
+#ifdef SPH_DEBUG_ASSERT
+#define SPH_DBG_ASSERT(cond, g) do { if (!(cond)) atomicAdd(&(g).dbg[SPH_CNT_ASSERT], 1ull); } while (0)
+#else
+#define SPH_DBG_ASSERT(cond, g) do { } while (0)
+#endif
+
 __host__ __device__ inline int level_of_h(const GridDesc& g, float h) {
     int l = 0;
     while (l + 1 < g.nlev && h > g.lev[l].hmax) ++l;

@@ -78,6 +78,7 @@ k_key_hist(GridDesc g, SortedState S, int n, uint32_t* __restrict__ key, uint32_
     const float4 p = to_float4(S.posh[i]);                            // posh.w is still h here (k_pack; the layouts change at the sort)
     const uint32_t cell = cell_of(g, p, level_of_h(g, p.w), oob);
     const uint32_t k = cell * (uint32_t)g.na + (S.meta[i] >> SPH_META_IDX_BITS);
+    SPH_DBG_ASSERT(cell < g.cells_total, g);
     key[i] = k;
     rank[i] = atomicAdd(&cell_count[k], 1u);
     if (oob) atomicAdd(&counters[CNT_OUT_OF_DOMAIN], 1ull);
@@ -146,6 +147,7 @@ k_update(GridDesc g, PairConsts pc, SortedState S, int n, UpdateArgs U,
         const float4 posf = to_float4(pos);
         const uint32_t cell = cell_of(g, posf, g.nlev > 1 ? level_of_h(g, posf.w) : 0, oob);   // several levels only when h varies: posh.w = h
         const uint32_t k = cell * (uint32_t)g.na + aid;
+        SPH_DBG_ASSERT(cell < g.cells_total, g);
         key[i] = k;
         rank[i] = atomicAdd(&cell_count[k], 1u);
         if (oob) atomicAdd(&counters[CNT_OUT_OF_DOMAIN], 1ull);
@@ -193,6 +195,9 @@ k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int n
     }
     __syncthreads();
     const uint32_t tile = s_tile, epoch = s_epoch;
+#ifdef SPH_DEBUG_ASSERT
+    if (threadIdx.x == 0 && tile >= (uint32_t)nb) atomicAdd(&state[0], 0ull);   // (a tile beyond the grid cannot happen: tickets == blocks)
+#endif
     const long long i0 = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
     uint32_t v[SCAN_ITEMS], s = 0;
 #pragma unroll
@@ -248,12 +253,13 @@ static int scan_exclusive(sph_ctx* c, uint32_t* in, uint32_t* out, long long n, 
 
 // a3: gather every persistent property into cell order (double buffer A -> B).
 __global__ void __launch_bounds__(NB)
-k_scatter(SortedState A, SortedState B, int n, int na, int with_acc, int w_mass, const uint32_t* __restrict__ key,
+k_scatter(GridDesc g, SortedState A, SortedState B, int n, int na, int with_acc, int w_mass, const uint32_t* __restrict__ key,
           const uint32_t* __restrict__ rank, const uint32_t* __restrict__ cell_start, uint32_t* __restrict__ nl_head) {
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
     const uint32_t k = key[i];
     const uint32_t d = cell_start[k] + rank[i];
+    SPH_DBG_ASSERT(k / (uint32_t)na < g.cells_total && d < (uint32_t)n, g);
     real4 p = A.posh[i];
     real4 v = A.velm[i];
     const real2 r = A.rp[i];
@@ -296,7 +302,7 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     const int n = (int)c->n_total;
     int rc = scan_exclusive(c, c->cell_count, c->cell_start, c->n_keys, true);   // leaves cell_count cleared
     if (rc) return rc;
-    if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
+    if (n) SPH_LAUNCH(c, SPH_K_SCATTER, k_scatter, (n + NB - 1) / NB, NB, 0, c->grid, c->S[c->cur], c->S[c->cur ^ 1], n, c->na,
                       with_acc ? 1 : 0, !with_acc ? 0 : (c->variable_h ? (c->pc.varh_um ? 3 : 0) : (c->pc.uniform_m ? 2 : 1)), c->key, c->rank, c->cell_start, c->nl.head);
     c->heads_fresh = n > 0 && c->nl.head != nullptr;
     c->cur ^= 1;

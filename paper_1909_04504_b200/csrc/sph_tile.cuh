@@ -159,6 +159,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
 
     auto load_batch = [&](uint32_t bb, uint32_t ee) -> float4 {
         const uint32_t j = bb + (uint32_t)lane;
+        SPH_DBG_ASSERT(ee <= g.n_sorted && bb <= ee, g);
         return j < ee ? to_float4(ld_state(posh + j)) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     };
     auto pop_run = [&]() -> bool {
@@ -257,6 +258,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
             else if (kind == 1) { c0 = max(x0 + n0, 0); c1 = n0 - 1; code |= 1u; }
             else                { c0 = 0; c1 = min(x1 - n0, n0 - 1); code |= 2u; }
             const uint32_t rowbase = Lv.base + (uint32_t)((iz * n1 + iy) * n0);
+            SPH_DBG_ASSERT(c0 >= 0 && c0 <= c1 + 1 && c1 < n0 && iy >= 0 && iy < n1 && iz >= 0 && iz < n2 && rowbase + (uint32_t)c1 + 1u <= g.cells_total, g);
             s_ = __ldg(cell_start + (size_t)(rowbase + (uint32_t)c0) * na);
             e_ = __ldg(cell_start + (size_t)(rowbase + (uint32_t)c1 + 1u) * na);
             nonempty = s_ < e_;
@@ -459,7 +461,7 @@ struct TileRecorder {
 
 // drain(nz, shifted) is called once per recorded block with the masks, bases and shift codes in ws
 template <class Drain>
-__device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileWarpSmem& ws, bool active, Drain&& drain) {
+__device__ __forceinline__ void tile_replay(const GridDesc& g, const NList& nl, uint32_t blk, TileWarpSmem& ws, bool active, Drain&& drain) {
     const int lane = threadIdx.x & 31;
     while (blk) {
         const uint32_t* hdr = nl.pool + (size_t)blk * 32;
@@ -468,6 +470,7 @@ __device__ __forceinline__ void tile_replay(const NList& nl, uint32_t blk, TileW
         const uint32_t w1 = __shfl_sync(SPH_FULL_MASK, hw, 1);
         const int M = (int)(w1 & 0xffu);
         const bool shifted = (w1 & 0x100u) != 0u;
+        SPH_DBG_ASSERT(blk < nl.pool_rows && M >= 1 && M <= TILE_MMAX && (unsigned long long)blk + (unsigned)M + 1u + (shifted ? 1u : 0u) <= nl.pool_rows, g);
         const uint32_t* rows0 = hdr + 32;
         __syncwarp();
         if (lane >= 2) ws.base[lane - 2] = hw;
