@@ -195,16 +195,20 @@ k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int n
     }
     __syncthreads();
     const uint32_t tile = s_tile, epoch = s_epoch;
-#ifdef SPH_DEBUG_ASSERT
-    if (threadIdx.x == 0 && tile >= (uint32_t)nb) atomicAdd(&state[0], 0ull);   // (a tile beyond the grid cannot happen: tickets == blocks)
-#endif
     const long long i0 = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
     uint32_t v[SCAN_ITEMS], s = 0;
+    const bool full = i0 + SCAN_ITEMS <= n;                              // 16-byte vector path (SCAN_ITEMS == 4, i0 % 4 == 0)
+    if (full) {
+        const uint4 q = *reinterpret_cast<const uint4*>(in + i0);
+        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w; s = q.x + q.y + q.z + q.w;
+        if (zero_in) *reinterpret_cast<uint4*>(in + i0) = make_uint4(0u, 0u, 0u, 0u);   // the histogram is consumed: leave it cleared for the next step
+    } else {
 #pragma unroll
-    for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (i0 + k < n) ? in[i0 + k] : 0u; s += v[k]; }
-    if (zero_in) {                                                       // the histogram is consumed: leave it cleared for the next step
+        for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (i0 + k < n) ? in[i0 + k] : 0u; s += v[k]; }
+        if (zero_in) {
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS; ++k) if (i0 + k < n) in[i0 + k] = 0u;
+            for (int k = 0; k < SCAN_ITEMS; ++k) if (i0 + k < n) in[i0 + k] = 0u;
+        }
     }
     uint32_t ex = block_exclusive_scan(s, &s_total);
     __syncthreads();
@@ -241,7 +245,12 @@ k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int n
     __syncthreads();
     ex += s_prefix;
 #pragma unroll
-    for (int k = 0; k < SCAN_ITEMS; ++k) { if (i0 + k < n) out[i0 + k] = ex; ex += v[k]; }
+    for (int k = 0; k < SCAN_ITEMS; ++k) { const uint32_t e = ex; ex += v[k]; v[k] = e; }
+    if (full) *reinterpret_cast<uint4*>(out + i0) = make_uint4(v[0], v[1], v[2], v[3]);
+    else {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) if (i0 + k < n) out[i0 + k] = v[k];
+    }
 }
 
 static int scan_exclusive(sph_ctx* c, uint32_t* in, uint32_t* out, long long n, bool zero_in) {
