@@ -4,7 +4,11 @@
 // the records of launch_search (sph_search.cu) and walks nothing; otherwise the warp searches itself.
 #include "sph_tile.cuh"
 
-struct DensitySrc { real4 pj; real mj; uint32_t aid; };
+struct DensitySrc { real4 pj; real mj; uint32_t aid;
+#ifdef SPH_EXP_RED
+    uint32_t j;
+#endif
+};
 
 template <int KERNEL, int DIM, bool VARH, bool FILTER, bool REPLAY, bool UM>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS_DENSITY)
@@ -34,6 +38,9 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
     auto load = [&](uint32_t j) {
         SPH_DBG_ASSERT(j < g.n_sorted, g);
         DensitySrc s; s.pj = ld_state(S.posh + j); s.mj = 0; s.aid = 0u;
+#ifdef SPH_EXP_RED
+        s.j = j;
+#endif
         if (VARH && !UM) s.mj = ld_state(&S.velm[j].w);            // VU layout (variable h, uniform mass): m = m_const
         if (FILTER) s.aid = __ldg(S.meta + j) >> SPH_META_IDX_BITS;
         return s;
@@ -90,6 +97,12 @@ k_density_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restr
         kernel_profile2<KERNEL, DIM>(mul2(r, hinv), f, df);
         mfac = pk(ha ? mfac.x : 0.0f, hb ? mfac.y : 0.0f);              // a candidate that fails contributes nothing
         rho2 = fma2(mfac, f, rho2);
+#ifdef SPH_EXP_RED
+        // EXPERIMENT (DESIGN.md "Tried and dropped" (g)): the cost of ONE red.global.add.f32 per true pair, which a
+        // symmetric once-per-pair density pass would need for the j side (the target word is scratch: acc.w)
+        if (ha) atomicAdd(&S.acc[a.j].w, mfac.x * f.x);
+        if (hb) atomicAdd(&S.acc[b.j].w, mfac.y * f.y);
+#endif
     };
 #endif
 
