@@ -124,9 +124,9 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     SPH_CUDA_OK(c, cudaMalloc(&c->hminmax, 4 * sizeof(long long)));
     if (nl_slots > 0 && tot > 0) {
         const size_t warps = (size_t)(tot + 31) / 32;
-        size_t rows = warps * (size_t)nl_slots + 32;
+        size_t rows = warps * (size_t)nl_slots + 64;      // + slack: a replaying warp always fetches a whole block image (26 rows)
         if (rows > 0xfffffff0ull) rows = 0xfffffff0ull;
-        c->nl.pool_rows = (uint32_t)rows;
+        c->nl.pool_rows = (uint32_t)(rows - 32);          // rows the recorder may hand out; the last 32 are only ever over-read
         SPH_CUDA_OK(c, cudaMalloc(&c->nl.pool, rows * 32 * sizeof(uint32_t)));
         SPH_CUDA_OK(c, cudaMalloc(&c->nl.head, (warps + 2) * sizeof(uint32_t)));
         c->nl.used = (uint32_t*)(c->counters + CNT_NL_USED);

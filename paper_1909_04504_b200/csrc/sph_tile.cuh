@@ -57,9 +57,12 @@ struct __align__(16) TileWarpSmem {
         float2 G[4][34];                   // B operands of one batch: G[t][c] = (feature t, feature t+4) of staged candidate c
         float Af[32 * 9];                  // A operands of a group while the quads exchange them (stride 9: conflict-free)
     };
-    uint32_t mask[TILE_MMAX][32];          // candidate masks, [batch][lane]
-    uint32_t base[32];                     // first sorted index of every batch
+    // the image of one record block, in the layout of the pool (so that a replaying warp fetches a block with ONE
+    // bulk copy): header row, shift-code row, mask rows
+    uint32_t hdr[32];                      // [0] next block, [1] batches | flags, [2 + m] first sorted index of batch m
     uint32_t bcode[32];                    // image-shift code of every batch (2 bits per axis: 1 -> -L, 2 -> +L)
+    uint32_t mask[TILE_MMAX][32];          // candidate masks, [batch][lane]
+    unsigned long long bar;                // mbarrier of the bulk copy
     uint32_t seg_s[32], seg_e[32], seg_c[32];   // candidate runs of the current pass: [s, e) and image-shift code
     // warp-uniform walker state that only the (cold) group / level / pass set-up code touches: kept here, not in
     // registers, so that the batch loop stays within the register budget
@@ -313,7 +316,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         if (!ing) mask = 0u;
         ws.mask[st.M][lane] = mask;
         if (mask) st.nz |= 1u << st.M;
-        if (lane == 0) { ws.base[st.M] = cb0; ws.bcode[st.M] = ccode; }
+        if (lane == 0) { ws.hdr[2 + st.M] = cb0; ws.bcode[st.M] = ccode; }
         if (ing) st.tests += (unsigned)min(32u, ce - cb0);
         ++st.M;
     };
@@ -363,7 +366,7 @@ __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32
     auto pop = [&](bool& has, uint32_t& cd) -> uint32_t {
         const bool refill = cur == 0u && nz != 0u;
         const int m = max(__ffs(nz) - 1, 0);
-        const uint32_t nm = ws.mask[m][lane], nb = ws.base[m];
+        const uint32_t nm = ws.mask[m][lane], nb = ws.hdr[2 + m];
         cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? (nz & (nz - 1u)) : nz;
         if (PER) { const uint32_t nc = ws.bcode[m]; code = refill ? nc : code; }
         has = cur != 0u;
@@ -403,7 +406,7 @@ __device__ __forceinline__ void tile_drain2(TileWarpSmem& ws, uint32_t nz, uint3
     auto pop = [&](bool& has, uint32_t& cd) -> uint32_t {
         const bool refill = cur == 0u && nz != 0u;
         const int m = max(__ffs(nz) - 1, 0);
-        const uint32_t nm = ws.mask[m][lane], nb = ws.base[m];
+        const uint32_t nm = ws.mask[m][lane], nb = ws.hdr[2 + m];
         cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? (nz & (nz - 1u)) : nz;
         if (PER) { const uint32_t nc = ws.bcode[m]; code = refill ? nc : code; }
         has = cur != 0u;
@@ -428,18 +431,24 @@ __device__ __forceinline__ void tile_drain2(TileWarpSmem& ws, uint32_t nz, uint3
     __syncwarp();
 }
 
-// ---- mask records (recorded by the density pass, replayed by the acceleration pass) -----------------------
-// The pool is an array of ROWS of 32 words.  A warp appends BLOCKS: a header row {next block (row index, 0 =
-// end), number of batches M <= TILE_MMAX | 0x100 if a batch came from a periodic image, base[0..M-1]}, then -- only
-// when that flag is set -- one row of shift codes (word = batch), then M rows of masks (word = lane).
-// head[warp] = SPH_NL_NONE marks a warp whose masks did not fit the pool.
+// ---- mask records (recorded by the search, replayed by the pair passes) ------------------------------------
+// The pool is an array of ROWS of 32 words.  A warp appends BLOCKS of 2 + M rows: a header row {next block (row
+// index, 0 = end), number of batches M <= TILE_MMAX | 0x100 if a batch came from a periodic image, base[0..M-1]}, one
+// row of shift codes (word = batch), then M rows of masks (word = lane).  A block is contiguous, so a replaying
+// warp fetches it with ONE bulk copy (cp.async.bulk + mbarrier; SASS UBLKCP) into the same layout in shared
+// memory.  head[warp] = SPH_NL_NONE marks a warp whose masks did not fit the pool.
+#ifndef TILE_BULK_REPLAY
+#define TILE_BULK_REPLAY 1
+#endif
+#define TILE_BLOCK_ROWS (TILE_MMAX + 2)
+
 struct TileRecorder {
     NList nl; uint32_t prev_hdr; bool ok;
     __device__ __forceinline__ void init(const NList& n) { nl = n; prev_hdr = 0u; ok = n.pool != nullptr; }
     __device__ __forceinline__ void append(const TileWarpSmem& ws, int M, bool shifted, int warp_id, unsigned long long* counters) {
         if (!ok || M <= 0) return;
         const int lane = threadIdx.x & 31;
-        const uint32_t rows = (uint32_t)M + 1u + (shifted ? 1u : 0u);
+        const uint32_t rows = (uint32_t)M + 2u;
         uint32_t blk = 0;
         if (lane == 0) blk = atomicAdd(nl.used, rows) + 1u;
         blk = __shfl_sync(SPH_FULL_MASK, blk, 0);
@@ -450,39 +459,57 @@ struct TileRecorder {
         }
         __syncwarp();
         uint32_t* hdr = nl.pool + (size_t)blk * 32;
-        hdr[lane] = lane == 0 ? 0u : (lane == 1 ? ((uint32_t)M | (shifted ? 0x100u : 0u)) : ws.base[lane - 2]);
-        uint32_t* rows0 = hdr + 32;
-        if (shifted) { rows0[lane] = ws.bcode[lane]; rows0 += 32; }
-        for (int m = 0; m < M; ++m) __stcs(rows0 + (size_t)m * 32 + lane, ws.mask[m][lane]);   // streaming: keep the state in L2
+        hdr[lane] = lane == 0 ? 0u : (lane == 1 ? ((uint32_t)M | (shifted ? 0x100u : 0u)) : ws.hdr[lane]);
+        hdr[32 + lane] = ws.bcode[lane];
+        for (int m = 0; m < M; ++m) __stcs(hdr + (size_t)(m + 2) * 32 + lane, ws.mask[m][lane]);   // streaming: keep the state in L2
         if (lane == 0) { if (prev_hdr) nl.pool[(size_t)prev_hdr * 32] = blk; else nl.head[warp_id] = blk; }
         prev_hdr = blk;
     }
 };
 
-// drain(nz, shifted) is called once per recorded block with the masks, bases and shift codes in ws
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// drain(nz, shifted) is called once per recorded block with the header, shift codes and masks in ws
 template <class Drain>
 __device__ __forceinline__ void tile_replay(const GridDesc& g, const NList& nl, uint32_t blk, TileWarpSmem& ws, bool active, Drain&& drain) {
     const int lane = threadIdx.x & 31;
+#if TILE_BULK_REPLAY
+    const uint32_t bar = smem_addr(&ws.bar), dst = smem_addr(ws.hdr);
+    uint32_t phase = 0u;
+    if (lane == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(bar));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+#endif
     while (blk) {
-        const uint32_t* hdr = nl.pool + (size_t)blk * 32;
-        const uint32_t hw = __ldcs(hdr + lane);
-        const uint32_t next = __shfl_sync(SPH_FULL_MASK, hw, 0);
-        const uint32_t w1 = __shfl_sync(SPH_FULL_MASK, hw, 1);
+        SPH_DBG_ASSERT((unsigned long long)blk + TILE_BLOCK_ROWS <= (unsigned long long)nl.pool_rows + TILE_BLOCK_ROWS, g);
+        const uint32_t* src = nl.pool + (size_t)blk * 32;
+        __syncwarp();                                                    // the previous block has been drained
+#if TILE_BULK_REPLAY
+        if (lane == 0) {     // one bulk copy of the whole block image (fixed size: a short block over-reads into the next rows of the pool)
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"((uint32_t)(TILE_BLOCK_ROWS * 128)) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         :: "r"(dst), "l"(src), "r"((uint32_t)(TILE_BLOCK_ROWS * 128)), "r"(bar) : "memory");
+        }
+        uint32_t done = 0u;
+        while (!done)
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(done) : "r"(bar), "r"(phase) : "memory");
+        phase ^= 1u;
+#else
+        ws.hdr[lane] = __ldcs(src + lane); ws.bcode[lane] = __ldcs(src + 32 + lane);
+        __syncwarp();
+        { const int M0 = (int)(ws.hdr[1] & 0xffu); for (int m = 0; m < M0; ++m) ws.mask[m][lane] = __ldcs(src + (size_t)(m + 2) * 32 + lane); }
+#endif
+        const uint32_t next = ws.hdr[0], w1 = ws.hdr[1];
         const int M = (int)(w1 & 0xffu);
         const bool shifted = (w1 & 0x100u) != 0u;
-        SPH_DBG_ASSERT(blk < nl.pool_rows && M >= 1 && M <= TILE_MMAX && (unsigned long long)blk + (unsigned)M + 1u + (shifted ? 1u : 0u) <= nl.pool_rows, g);
-        const uint32_t* rows0 = hdr + 32;
-        __syncwarp();
-        if (lane >= 2) ws.base[lane - 2] = hw;
-        if (shifted) { ws.bcode[lane] = __ldcs(rows0 + lane); rows0 += 32; }
+        SPH_DBG_ASSERT(blk < nl.pool_rows && M >= 1 && M <= TILE_MMAX && (unsigned long long)blk + (unsigned)M + 2u <= nl.pool_rows, g);
         uint32_t nz = 0u;
-        for (int m0 = 0; m0 < M; m0 += 8) {                              // 8 independent loads in flight
-            uint32_t w[8];
-#pragma unroll
-            for (int k = 0; k < 8; ++k) w[k] = (m0 + k < M && active) ? __ldcs(rows0 + (size_t)(m0 + k) * 32 + lane) : 0u;   // a lane that is no destination of this pass drops its masks
-#pragma unroll
-            for (int k = 0; k < 8; ++k) if (m0 + k < M) { ws.mask[m0 + k][lane] = w[k]; if (w[k]) nz |= 1u << (m0 + k); }
-        }
+        if (active)                                                      // a lane that is no destination of this pass drops its masks
+            for (int m = 0; m < M; ++m) if (ws.mask[m][lane]) nz |= 1u << m;
         drain(nz, shifted);
         blk = next;
     }
