@@ -354,8 +354,9 @@ __global__ void __launch_bounds__(TILE_BLOCK)
 k_neighbors_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
                  uint32_t dest, uint32_t src, uint32_t* __restrict__ counts, const uint32_t* __restrict__ offsets,
                  int32_t* __restrict__ indices) {
-    __shared__ TileWarpSmem smem[TILE_WARPS];
-    TileWarpSmem& ws = smem[threadIdx.x >> 5];
+    typedef TileWarpSmemT<TILE_MMAX_OF(VARH)> WS;
+    __shared__ WS smem[TILE_WARPS];
+    WS& ws = smem[threadIdx.x >> 5];
     const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
     const bool in = i < n;
     uint32_t meta = 0, ci = 0; real4 pi = make_real4(0, 0, 0, 1);

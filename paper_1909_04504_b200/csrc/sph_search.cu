@@ -10,8 +10,9 @@ template <int DIM, bool VARH>
 __global__ void __launch_bounds__(TILE_BLOCK, TILE_MIN_BLOCKS)
 k_search_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restrict__ cell_start, int n,
               NList nl, unsigned long long* __restrict__ counters) {
-    __shared__ TileWarpSmem smem[TILE_WARPS];
-    TileWarpSmem& ws = smem[threadIdx.x >> 5];
+    typedef TileWarpSmemT<TILE_MMAX_OF(VARH)> WS;
+    __shared__ WS smem[TILE_WARPS];
+    WS& ws = smem[threadIdx.x >> 5];
     const int i = blockIdx.x * TILE_BLOCK + threadIdx.x;
     const int warp_id = i >> 5;
     const bool in = i < n;

@@ -48,11 +48,20 @@
 #ifndef TILE_DRAIN_DEPTH_DENSITY
 #define TILE_DRAIN_DEPTH_DENSITY 2        // PAIRS of candidates in flight in the density drain
 #endif
-#ifndef TILE_MMAX
-#define TILE_MMAX 24                      // masks per warp before a forced drain (<= 30: 30 bases + 2 words = one header row)
+// masks per warp before a forced drain / per record block (<= 30: 30 bases + 2 words = one header row).  Constant h:
+// 24 (a C3 / C4 tile streams ~22 batches; 30 costs a shared-memory carve-out step: C4 momentum 1.21 -> 1.36 ms);
+// variable h: 30 (a C5 tile streams ~33: C5 13.6 -> 13.0 ms/step)
+#ifndef TILE_MMAX_CONSTH
+#define TILE_MMAX_CONSTH 24
 #endif
+#ifndef TILE_MMAX_VARH
+#define TILE_MMAX_VARH 30
+#endif
+#define TILE_MMAX_OF(VARH) ((VARH) ? TILE_MMAX_VARH : TILE_MMAX_CONSTH)
 
-struct __align__(16) TileWarpSmem {
+template <int MM>
+struct __align__(16) TileWarpSmemT {
+    static constexpr int MMAX = MM;
     union {
         float2 G[4][34];                   // B operands of one batch: G[t][c] = (feature t, feature t+4) of staged candidate c
         float Af[32 * 9];                  // A operands of a group while the quads exchange them (stride 9: conflict-free)
@@ -61,7 +70,7 @@ struct __align__(16) TileWarpSmem {
     // bulk copy): header row, shift-code row, mask rows
     uint32_t hdr[32];                      // [0] next block, [1] batches | flags, [2 + m] first sorted index of batch m
     uint32_t bcode[32];                    // image-shift code of every batch (2 bits per axis: 1 -> -L, 2 -> +L)
-    uint32_t mask[TILE_MMAX][32];          // candidate masks, [batch][lane]
+    uint32_t mask[MM][32];                 // candidate masks, [batch][lane]
     unsigned long long bar;                // mbarrier of the bulk copy
     uint32_t seg_s[32], seg_e[32], seg_c[32];   // candidate runs of the current pass: [s, e) and image-shift code
     // warp-uniform walker state that only the (cold) group / level / pass set-up code touches: kept here, not in
@@ -110,14 +119,14 @@ __device__ __forceinline__ void mma_tf32_16x8x8(float (&c)[4], const uint32_t (&
 }
 
 // Walks every candidate run of the warp's 32 particles.  `drain()` is called (warp-uniformly, from ONE site)
-// whenever the mask store holds TILE_MMAX batches, and once at the end; it must consume the masks and call
+// whenever the mask store holds WS::MMAX batches, and once at the end; it must consume the masks and call
 // st.reset().  All 32 lanes must call this.   in: the lane holds a particle; active: it is a destination of this
 // launch; pi = (x, y, z, h); ci = its cell id (level base + linear cell).
-template <int DIM, bool VARH, class Drain>
+template <int DIM, bool VARH, class WS, class Drain>
 __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& pc,
                                           const real4* posh, const uint32_t* __restrict__ cell_start,
                                           bool active, bool in, float4 pi, uint32_t ci,
-                                          TileWarpSmem& ws, TileState& st, Drain&& drain) {
+                                          WS& ws, TileState& st, Drain&& drain) {
     const int lane = threadIdx.x & 31, gq = lane >> 2, tq = lane & 3;
     const int na = g.na, nlev = VARH ? g.nlev : 1;
     // the search runs in float whatever the real type of the build (see sph_internal.cuh)
@@ -324,7 +333,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
     // streams batches until the mask store is full (true) or every group is done (false)
     auto fill = [&]() -> bool {
         for (;;) {
-            if (st.M >= TILE_MMAX) return true;
+            if (st.M >= WS::MMAX) return true;
             if (!have) {
                 if (pop_run()) { pjn = load_batch(nb0, ne); have = true; continue; }
                 if (grp) {
@@ -358,8 +367,8 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
 // arithmetic.  A lane that has run out keeps executing with has = false and the harmless index `idle` (its own
 // particle) until the slowest lane of the warp is done; compute(src, has, code, per) must apply the exact
 // predicate and contribute nothing when it fails or has is false.  PER: some batch is a periodic image (code != 0).
-template <class Src, int DEPTH, bool PER, class Load, class Compute>
-__device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
+template <class Src, int DEPTH, bool PER, class WS, class Load, class Compute>
+__device__ __forceinline__ void tile_drain(WS& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
     const int lane = threadIdx.x & 31;
     __syncwarp();
     uint32_t cur = 0u, b = 0u, code = 0u;
@@ -398,8 +407,8 @@ __device__ __forceinline__ void tile_drain(TileWarpSmem& ws, uint32_t nz, uint32
 // false and the harmless index `idle` (its own particle) until the slowest lane of the warp is done;
 // compute(srcA, srcB, hasA, hasB, codeA, codeB, per) must apply the exact predicate and contribute nothing where
 // it fails or has is false.  PER: some batch is a periodic image (code != 0).
-template <class Src, int DEPTH, bool PER, class Load, class Compute>
-__device__ __forceinline__ void tile_drain2(TileWarpSmem& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
+template <class Src, int DEPTH, bool PER, class WS, class Load, class Compute>
+__device__ __forceinline__ void tile_drain2(WS& ws, uint32_t nz, uint32_t idle, Load&& load, Compute&& compute) {
     const int lane = threadIdx.x & 31;
     __syncwarp();
     uint32_t cur = 0u, b = 0u, code = 0u;
@@ -433,19 +442,19 @@ __device__ __forceinline__ void tile_drain2(TileWarpSmem& ws, uint32_t nz, uint3
 
 // ---- mask records (recorded by the search, replayed by the pair passes) ------------------------------------
 // The pool is an array of ROWS of 32 words.  A warp appends BLOCKS of 2 + M rows: a header row {next block (row
-// index, 0 = end), number of batches M <= TILE_MMAX | 0x100 if a batch came from a periodic image, base[0..M-1]}, one
+// index, 0 = end), number of batches M <= WS::MMAX | 0x100 if a batch came from a periodic image, base[0..M-1]}, one
 // row of shift codes (word = batch), then M rows of masks (word = lane).  A block is contiguous, so a replaying
 // warp fetches it with ONE bulk copy (cp.async.bulk + mbarrier; SASS UBLKCP) into the same layout in shared
 // memory.  head[warp] = SPH_NL_NONE marks a warp whose masks did not fit the pool.
 #ifndef TILE_BULK_REPLAY
 #define TILE_BULK_REPLAY 1
 #endif
-#define TILE_BLOCK_ROWS (TILE_MMAX + 2)
 
 struct TileRecorder {
     NList nl; uint32_t prev_hdr; bool ok;
     __device__ __forceinline__ void init(const NList& n) { nl = n; prev_hdr = 0u; ok = n.pool != nullptr; }
-    __device__ __forceinline__ void append(const TileWarpSmem& ws, int M, bool shifted, int warp_id, unsigned long long* counters) {
+    template <class WS>
+    __device__ __forceinline__ void append(const WS& ws, int M, bool shifted, int warp_id, unsigned long long* counters) {
         if (!ok || M <= 0) return;
         const int lane = threadIdx.x & 31;
         const uint32_t rows = (uint32_t)M + 2u;
@@ -470,9 +479,10 @@ struct TileRecorder {
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 // drain(nz, shifted) is called once per recorded block with the header, shift codes and masks in ws
-template <class Drain>
-__device__ __forceinline__ void tile_replay(const GridDesc& g, const NList& nl, uint32_t blk, TileWarpSmem& ws, bool active, Drain&& drain) {
+template <class WS, class Drain>
+__device__ __forceinline__ void tile_replay(const GridDesc& g, const NList& nl, uint32_t blk, WS& ws, bool active, Drain&& drain) {
     const int lane = threadIdx.x & 31;
+    constexpr int TILE_BLOCK_ROWS = WS::MMAX + 2;
 #if TILE_BULK_REPLAY
     const uint32_t bar = smem_addr(&ws.bar), dst = smem_addr(ws.hdr);
     uint32_t phase = 0u;
@@ -506,7 +516,7 @@ __device__ __forceinline__ void tile_replay(const GridDesc& g, const NList& nl, 
         const uint32_t next = ws.hdr[0], w1 = ws.hdr[1];
         const int M = (int)(w1 & 0xffu);
         const bool shifted = (w1 & 0x100u) != 0u;
-        SPH_DBG_ASSERT(blk < nl.pool_rows && M >= 1 && M <= TILE_MMAX && (unsigned long long)blk + (unsigned)M + 2u <= nl.pool_rows, g);
+        SPH_DBG_ASSERT(blk < nl.pool_rows && M >= 1 && M <= WS::MMAX && (unsigned long long)blk + (unsigned)M + 2u <= nl.pool_rows, g);
         uint32_t nz = 0u;
         if (active)                                                      // a lane that is no destination of this pass drops its masks
             for (int m = 0; m < M; ++m) if (ws.mask[m][lane]) nz |= 1u << m;
