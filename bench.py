@@ -430,6 +430,7 @@ def report(name, r, K, world, ms_max, units, e2e_agg, fp32_peak, hbm_peak, hbm_s
         e_ms, e_units = e2e_agg
         out["e2e"] = {"value": e_units / (e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": r["e2e"]["h2d"], "d2h_bytes_per_step": r["e2e"]["d2h"],
                       "steps": r["e2e"]["steps"], "ms_per_step": e_ms / r["e2e"]["steps"],
+                      "pcie_gbs": (r["e2e"]["h2d"] + r["e2e"]["d2h"]) * r["e2e"]["steps"] / (e_ms * 1e-3) / 1e9,
                       "what": "sph_nnps_build(host pinned arrays + a^n) + sph_pc_step(dt,1) + sph_sync_state(host) per step"}
     return out
 

@@ -24,7 +24,9 @@
  *                  reallocates caller memory.  Arrays must be contiguous; z,w may be NULL when dim == 2.
  *   ownership      sph_ctx is opaque and LIBRARY-OWNED; it holds all workspace (cell tables, the
  *                  cell-sorted mirror of the particle state), allocated once in sph_create from
- *                  `capacity`.  No call allocates device memory after sph_create.
+ *                  `capacity`.  No call of the path allocates device memory after sph_create; the one exception is
+ *                  the verification export sph_nnps_get_neighbors with HOST pointers, which allocates and frees two
+ *                  temporary device buffers for its result.
  *   asynchrony     all work is enqueued on the stream given to sph_create.  Calls marked [sync]
  *                  synchronise that stream before returning; the others do not.
  *   errors         every call returns 0 (SPH_OK) or a negative sph_error.  Argument errors are detected
@@ -107,10 +109,11 @@ typedef struct sph_params {
                                  * of a class <= ~1.6 (at most 8); 1 = the paper's single grid sized by h_max      */
     int nlist_slots;            /* record pool of the pair passes, in rows of 32 words per warp (32 particles) of
                                  * capacity (default 192, i.e. 768 B per particle of capacity; < 0: no pool, every
-                                 * pair pass searches).  The summation-density pass records one 32-bit hit mask
-                                 * per particle and batch of 32 candidates; the momentum pass of the same
-                                 * evaluation replays them instead of searching again.  A warp whose masks do
-                                 * not fit simply searches again (sph_stats.nlist_fallback_warps counts them). */
+                                 * pair pass searches itself).  ONE search per sorted order records one 32-bit
+                                 * candidate mask per particle and batch of 32 candidates; the density and momentum
+                                 * passes that follow replay them (and apply the exact predicate).  A warp whose
+                                 * masks do not fit is searched again by the pair passes
+                                 * (sph_stats.nlist_fallback_warps counts them). */
 } sph_params;
 
 typedef struct sph_array {      /* one named particle array (L316) */

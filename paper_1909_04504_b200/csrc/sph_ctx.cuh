@@ -40,6 +40,7 @@ struct sph_ctx {
     // neighbour rows recorded by a density launch for the acceleration launch that follows it
     NList nl;                  // nl.pool == nullptr: recording disabled
     bool nl_valid;             // the records match the current sorted order (launch_search ran since the last sort)
+    bool inv_valid;            // rank[] holds the inverse permutation (caller order -> sorted index) of the current order
     bool last_used_rows;       // the last acceleration launch replayed recorded rows
     bool counters_fresh;       // k_update has just cleared the counters of the search and the pair passes (consumed by evaluate)
     bool heads_fresh;          // k_scatter has just cleared the record heads (consumed by launch_search)

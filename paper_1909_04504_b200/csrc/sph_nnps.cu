@@ -316,19 +316,28 @@ int nnps_sort_from_keys(sph_ctx* c, bool with_acc) {
     c->heads_fresh = n > 0 && c->nl.head != nullptr;
     c->cur ^= 1;
     c->nl_valid = false;                 // recorded neighbour rows index the previous sorted order
+    c->inv_valid = false;
     return SPH_OK;
 }
 
 // ------------------------------------------------------------------------------------------------
 // caller-order outputs
 // ------------------------------------------------------------------------------------------------
+// inv[base(array) + original index] = sorted index: the caller-order outputs then WRITE coalesced (one thread per
+// caller-order particle) instead of scattering 4-byte words (8x write amplification at 32-byte sectors)
 __global__ void __launch_bounds__(NB)
-k_gather_out(SortedState S, int n, uint32_t array, OutPtrs O) {
+k_inverse(SortedState S, int n, PackArgs A, uint32_t* __restrict__ inv) {
     const int i = blockIdx.x * NB + threadIdx.x;
     if (i >= n) return;
     const uint32_t meta = S.meta[i];
-    if ((meta >> SPH_META_IDX_BITS) != array) return;
-    const uint32_t o = meta & SPH_META_IDX_MASK;
+    inv[A.base[meta >> SPH_META_IDX_BITS] + (long long)(meta & SPH_META_IDX_MASK)] = (uint32_t)i;
+}
+
+__global__ void __launch_bounds__(NB)
+k_gather_out(SortedState S, int n_array, const uint32_t* __restrict__ inv, OutPtrs O) {
+    const int o = blockIdx.x * NB + threadIdx.x;
+    if (o >= n_array) return;
+    const uint32_t i = inv[o];
     if (O.x || O.y || O.z) { const real4 p = S.posh[i]; if (O.x) O.x[o] = p.x; if (O.y) O.y[o] = p.y; if (O.z) O.z[o] = p.z; }
     if (O.u || O.v || O.w) { const real4 v = S.velm[i]; if (O.u) O.u[o] = v.x; if (O.v) O.v[o] = v.y; if (O.w) O.w[o] = v.z; }
     if (O.rho || O.p) { const real2 r = S.rp[i]; if (O.rho) O.rho[o] = r.x; if (O.p) O.p[o] = r.y * r.x * r.x; }
@@ -340,7 +349,16 @@ k_gather_out(SortedState S, int n, uint32_t array, OutPtrs O) {
 
 int nnps_gather_out(sph_ctx* c, int array, const OutPtrs& O) {
     const int n = (int)c->n_total;
-    if (n) SPH_LAUNCH(c, SPH_K_OUTPUT, k_gather_out, (n + NB - 1) / NB, NB, 0, c->S[c->cur], n, (uint32_t)array, O);
+    if (n == 0 || c->n[array] == 0) return SPH_OK;
+    if (!c->inv_valid) {                       // once per sorted order (rank is idle between sorts)
+        PackArgs A; memset(&A, 0, sizeof(A));
+        A.na = c->na;
+        for (int a = 0; a <= c->na; ++a) A.base[a] = c->base[a];
+        SPH_LAUNCH(c, SPH_K_OUTPUT, k_inverse, (n + NB - 1) / NB, NB, 0, c->S[c->cur], n, A, c->rank);
+        c->inv_valid = true;
+    }
+    const int na_ = (int)c->n[array];
+    SPH_LAUNCH(c, SPH_K_OUTPUT, k_gather_out, (na_ + NB - 1) / NB, NB, 0, c->S[c->cur], na_, c->rank + c->base[array], O);
     return SPH_OK;
 }
 
@@ -405,6 +423,7 @@ int nnps_export_neighbors(sph_ctx* c, int dest, int src, int64_t* offsets, int32
     const long long nd = c->n[dest];
     uint32_t* counts = c->key;            // scratch: key/rank are dead between sorts
     uint32_t* off32 = c->rank;
+    c->inv_valid = false;                 // (rank also holds the inverse permutation of the caller-order outputs)
     SPH_CUDA_OK(c, cudaMemsetAsync(counts, 0, (size_t)(nd + 1) * sizeof(uint32_t), c->stream));
     SortedState& S = c->S[c->cur];
     const int tgrid = (n + TILE_BLOCK - 1) / TILE_BLOCK;
