@@ -178,3 +178,53 @@ def test_variable_h_sets_do_not_depend_on_the_number_of_levels(O, WL, levels):
     assert_close(rho.cpu().numpy(), orho, f"rho levels={levels}")
     ctx.synchronize()
     ctx.close()
+
+
+@pytest.mark.parametrize("offset", [0.0, 1000.0])
+def test_filter_has_no_false_negatives_at_the_cutoff(O, WL, offset):
+    """Stress of the conservative tensor-core filter: many pairs at r = cut (1 +- 1e-6 ... 1e-3) in random directions,
+    constant and variable h, in a box far from the origin (coordinates ~1000: the float rounding unit of positions is
+    6e-5, a third of a per cent of h).  Sets must stay bit-exact with the oracle's float predicate."""
+    rng = np.random.default_rng(123 + int(offset))
+    for variable_h in (False, True):
+        n_pairs = 1500
+        wl = WL.random_box(n=2 * n_pairs, dim=3, periodic=True, seed=97, kernel="wendland_c2", variable_h=variable_h, h_mean=0.04)
+        A = wl.arrays[0]
+        h = A.h.astype(np.float64)
+        ctr = rng.random((n_pairs, 3))
+        d = rng.standard_normal((n_pairs, 3)); d /= np.linalg.norm(d, axis=1)[:, None]
+        cut = (h[0::2] + h[1::2])                                   # k/2 = 1 for Wendland-C2
+        rel = 1.0 + rng.choice([-1.0, 1.0], n_pairs) * 10.0 ** rng.uniform(-6.5, -3.0, n_pairs)
+        p0 = ctr - 0.5 * d * (cut * rel)[:, None]; p1 = ctr + 0.5 * d * (cut * rel)[:, None]
+        pos = np.empty((2 * n_pairs, 3)); pos[0::2] = p0; pos[1::2] = p1
+        pos = np.mod(pos, 1.0) + offset
+        for k, c in enumerate("xyz"):
+            v = pos[:, k].astype(np.float32)
+            v[v >= np.float32(offset + 1.0)] = np.float32(offset)
+            setattr(A, c, np.ascontiguousarray(v))
+        wl.lo = (offset, offset, offset); wl.hi = (offset + 1.0, offset + 1.0, offset + 1.0)
+        ctx, _ = make_ctx(wl)
+        f = {c: getattr(A, c) for c in "xyzh"}
+        off, idx = ctx.nnps_get_neighbors(0, 0)
+        ooff, oidx = O.neighbors(wl, f, f, pred32=True)
+        assert np.array_equal(off, ooff) and np.array_equal(idx.astype(np.int64), oidx), (offset, variable_h)
+        near = np.diff(ooff).sum() - len(ooff) + 1
+        assert near > n_pairs // 4                                   # a good share of the constructed pairs are neighbours
+        rho, _ = ctx.summation_density(0, 1)
+        assert ctx.get_stats().pairs_density == int(ooff[-1])
+        ctx.synchronize()
+        ctx.close()
+
+
+def test_c5_pair_totals_do_not_depend_on_the_tiling(WL):
+    """Full-size consistency of the filter: different level counts / x sub-cells give different groups, tile origins and
+    margins; a false negative of the filter would have to repeat in all of them for the totals to agree."""
+    wl = WL.gaussian_mixture_3d()
+    totals = []
+    for over in (dict(), dict(levels=2, xsub=8), dict(levels=5, xsub=2)):
+        ctx, _ = make_ctx(wl, **over)
+        ctx.summation_density(0, 1, want_p=False)
+        ctx.synchronize()
+        totals.append(int(ctx.get_stats().pairs_density))
+        ctx.close()
+    assert totals[0] == totals[1] == totals[2], totals
