@@ -103,7 +103,7 @@ typedef struct sph_params {
                                  * nu = 0 (default): term off.  eta: the paper's regulariser (0.01 is customary) */
     int integrator;             /* enum sph_integrator: what sph_pc_step steps with */
     /* Tuning knobs of the neighbour search; results do not depend on them (0 = default). */
-    int xsub;                   /* x sub-cells per support radius (1..16; default 0 = 6, or 4 when h varies)       */
+    int xsub;                   /* x sub-cells per support radius (1..16; default 0 = 6)                           */
     int levels;                 /* variable h: number of h classes, each with its own cell grid (PAPER.md L158-160,
                                  * L171: one grid sized by h_max "becomes inefficient"); 0 = as many as keep the h ratio
                                  * of a class <= ~1.6 (at most 8); 1 = the paper's single grid sized by h_max      */

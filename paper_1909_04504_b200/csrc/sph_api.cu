@@ -94,7 +94,6 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     default_tables(c);
     set_consts(c);
     c->xsub = params->xsub ? params->xsub : 6;
-    c->xsub_auto = params->xsub == 0;
     const int nl_slots = params->nlist_slots ? params->nlist_slots : 192;
     *out = c;                                  // so the caller can read sph_last_error / destroy on failure
     SPH_CUDA_OK(c, cudaGetDevice(&c->device));
@@ -192,7 +191,6 @@ static int size_grid(sph_ctx* c) {
         nlev = nlev < 1 ? 1 : (nlev > SPH_MAX_LEVELS ? SPH_MAX_LEVELS : nlev);
     }
     int xsub = c->xsub;
-    if (c->xsub_auto && c->variable_h) xsub = 4;
     double scale = 1.0;
     for (int iter = 0; iter < 96; ++iter) {
         int64_t total = 0; bool ok = true;

@@ -46,7 +46,6 @@ struct sph_ctx {
     bool heads_fresh;          // k_scatter has just cleared the record heads (consumed by launch_search)
     // CUDA graph of two consecutive steps of sph_pc_step (the state buffers flip every step), replayed for long runs
     cudaGraphExec_t step_graph; real graph_dt; int graph_cont, graph_cur, graph_nodes; bool graph_off;
-    bool xsub_auto;            // xsub was not given: 6, or 16 when h varies
     int xsub;                  // x sub-cells per support radius requested (GridDesc::xsub is what the grid got)
 
     int64_t launches, steps_done;
