@@ -66,10 +66,9 @@ __host__ __device__ inline int level_of_h(const GridDesc& g, float h) {
     return l;
 }
 
-// Neighbour rows recorded by the density pass and replayed by the acceleration pass.
-// The pool is an array of ROWS of 32 words (one word per lane of the warp that owns the row).  A warp appends
-// BLOCKS: a header row {next block (row index, 0 = end), number of rows} followed by that many rows of sorted
-// particle indices, SPH_NL_NONE where a lane has no entry.
+// Candidate-mask records written by the search and replayed by the pair passes (sph_tile.cuh "mask records").  The
+// pool is an array of ROWS of 32 words (one word per lane of the warp that owns the row); a warp appends contiguous
+// BLOCKS: header row, shift-code row, one mask row per batch.
 #define SPH_NL_NONE 0xffffffffu
 struct NList {
     uint32_t* pool;            // pool_rows * 32 words

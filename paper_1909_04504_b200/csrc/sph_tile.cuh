@@ -18,15 +18,15 @@
 // of DESIGN.md R7, so the tensor-core result is only a CONSERVATIVE filter: a margin that bounds the rounding
 // (derived in DESIGN.md "Tensor-core filter") is subtracted on the candidate side, the sign bits of the
 // accumulators are collected with one funnel shift each, and a 4 x 4 byte transpose inside every quad gives each
-// lane the 32-bit mask of ITS particle for the batch: a superset of its neighbours (+ ~4 %).
+// lane the 32-bit mask of ITS particle for the batch: a superset of its neighbours (+ 2-4 %).
 // Phase 2 (evaluation).  When the mask store is full, and once at the end, the warp drains it: every lane pops its
 // own candidates in order, applies the EXACT float predicate R7 (image-specific shift, fl(x_i - x_j), fma chain,
 // r2 < cut2) and runs the expensive body (kernel, EOS terms, viscosity) on the true neighbours, so the body runs at
 // mean/max neighbour-count lane utilisation instead of the hit rate of the tests.  Set membership is therefore
 // decided by exactly the expression the oracle uses; the filter only has to have no false negatives.
-// Records.  A recording pass also copies the masks, bases and shift codes (not the hit indices: 4 B per 32 tests
-// instead of 4 B per hit) to the record pool; the acceleration pass of the same evaluation replays them
-// (tile_replay), applies the same exact predicate and walks nothing.
+// Records.  The search kernel (sph_search.cu) copies the masks, bases and shift codes (not the hit indices: 4 B per
+// 32 tests instead of 4 B per hit) to the record pool, once per sorted order; the density and momentum passes
+// replay them (tile_replay: one bulk copy per block), apply the exact predicate and walk nothing.
 #pragma once
 #include "sph_ctx.cuh"
 #include <type_traits>
