@@ -261,6 +261,30 @@ int sph_fp32_probe(sph_ctx* ctx, int packed, int iters, double* tflops, double* 
  * this library really tests (sph_stats.candidates*).  Positions in the cell-sorted mirror are used.  [sync] */
 int sph_stencil_candidates(sph_ctx* ctx, int64_t* out);
 
+/* Allocation-free cell offsets (Sec.2.2: the start of every cell's run in the cell-sorted order = the
+ * exclusive prefix sum of the per-cell particle counts), for callers that may not call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it).  It needs no context: it is the single-pass
+ * look-back scan of the sort (k_scan) with its look-back table in a file-scope device array of the library instead
+ * of in memory the context allocates.
+ *   d_counts   DEVICE pointer, n uint32 (read only, caller-owned)
+ *   d_offsets  DEVICE pointer, n + 1 uint32 (written; [n] = the total, which must fit 32 bits), caller-owned,
+ *              must not overlap d_counts
+ *   n          0 <= n <= SPH_STATIC_SCAN_MAX_N; n == 0 writes d_offsets[0] = 0
+ *   stream     a cudaStream_t of the CURRENT device (NULL = the default stream); the call is asynchronous on it
+ * The call issues one cudaMemsetAsync and one kernel and calls no cudaMalloc / cudaFree / allocating routine.  The
+ * first call on each device looks up the device address of the array (cudaGetSymbolAddress): make that first call
+ * (n = 0 will do) outside stream capture.  The array (SPH_STATIC_SCAN_BYTES, about 128 KiB) is held by every GPU
+ * that loads the library until the process exits, and is SHARED by all calls on that GPU: each call clears the
+ * part it uses, so calls in stream order are independent of one another, but two calls that overlap on the GPU
+ * (different streams, no dependency between them) race on it and give wrong offsets.
+ * Errors: SPH_ERR_NULL (a pointer is NULL and n > 0, or d_offsets is NULL), SPH_ERR_BAD_ARG (n < 0),
+ * SPH_ERR_CAPACITY (n > SPH_STATIC_SCAN_MAX_N), SPH_ERR_CUDA; sph_static_last_error() gives the message of the
+ * calling thread's last failure (there is no context to hold it). */
+#define SPH_STATIC_SCAN_MAX_N  67108864LL                           /* 2^26 counts per call */
+#define SPH_STATIC_SCAN_BYTES  (256 + 8 * (SPH_STATIC_SCAN_MAX_N / 4096))   /* header + one word per 4096-count tile */
+int sph_cell_offsets_static(const uint32_t* d_counts, int64_t n, uint32_t* d_offsets, void* stream);
+const char* sph_static_last_error(void);
+
 const char* sph_strerror(int code);
 const char* sph_last_error(const sph_ctx* ctx);
 int sph_abi_version(void);

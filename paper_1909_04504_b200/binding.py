@@ -28,7 +28,7 @@ EXPORTS = ["sph_create", "sph_destroy", "sph_set_tables", "sph_nnps_build", "sph
            "sph_wcsph_accel", "sph_pc_step", "sph_sync_state", "sph_get_accel", "sph_nnps_get_neighbors",
            "sph_get_stats", "sph_synchronize", "sph_strerror", "sph_last_error", "sph_abi_version",
            "sph_set_profiling", "sph_get_profile", "sph_kernel_name", "sph_fp32_probe", "sph_stencil_candidates",
-           "sph_real_size"]
+           "sph_real_size", "sph_cell_offsets_static", "sph_static_last_error"]
 
 _FP = C.POINTER(C.c_float)
 FIELD_NAMES = ("x", "y", "z", "u", "v", "w", "h", "m", "rho", "p", "ax", "ay", "az", "arho")
@@ -107,10 +107,34 @@ def load(precision: str = "f32") -> C.CDLL:
         for name in EXPORTS:
             if name not in ("sph_strerror", "sph_last_error", "sph_kernel_name"):
                 getattr(L, name).restype = i32
+        L.sph_static_last_error.argtypes = []; L.sph_static_last_error.restype = C.c_char_p
+        L.sph_cell_offsets_static.argtypes = [vp, C.c_int64, vp, vp]
         if L.sph_real_size() != (4 if precision == "f32" else 8):
             raise ImportError(f"{path}: sph_real_size() does not match precision {precision}")
         _libs[precision] = L
     return _libs[precision]
+
+
+STATIC_SCAN_MAX_N = 1 << 26       # SPH_STATIC_SCAN_MAX_N of include/sph.h
+
+
+def cell_offsets_static(counts, offsets, stream=None, precision: str = "f32", n: Optional[int] = None):
+    """sph_cell_offsets_static (include/sph.h): offsets[0..n] = exclusive prefix sum of counts[0..n) on the GPU,
+    with the scan's scratch in the library's static device array -- the call allocates nothing.  `counts` (n) and
+    `offsets` (>= n + 1) are CUDA tensors of a 32-bit integer type on the current device; `stream` a torch stream
+    (default: the current one).  Argument marshalling only; raises SphError (n beyond the limit -> code -3)."""
+    import torch
+    L = load(precision)
+    n = int(counts.numel()) if n is None else int(n)
+    for t in (counts, offsets):
+        assert t.is_cuda and t.is_contiguous() and t.element_size() == 4 and not t.dtype.is_floating_point
+    assert n > STATIC_SCAN_MAX_N or (counts.numel() >= n and offsets.numel() >= n + 1)
+    st = torch.cuda.current_stream(counts.device) if stream is None else stream
+    with torch.cuda.device(counts.device):
+        rc = L.sph_cell_offsets_static(counts.data_ptr(), n, offsets.data_ptr(), st.cuda_stream)
+    if rc != 0:
+        raise SphError(rc, L.sph_static_last_error().decode())
+    return offsets
 
 
 def _ptr_and_mem(t, real_size=4):

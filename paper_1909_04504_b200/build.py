@@ -24,7 +24,7 @@ OBJ = os.path.join(HERE, "build" if not os.environ.get("SPH_B200_LIB") else
 # (source, extra defines, object): sph_accel.cu is compiled once per smoothing kernel (its instantiations dominate
 # the build time) and once as the dispatcher
 SOURCES = [("sph_api.cu", [], "sph_api.o"), ("sph_nnps.cu", [], "sph_nnps.o"), ("sph_density.cu", [], "sph_density.o"), ("sph_search.cu", [], "sph_search.o"),
-           ("sph_probe.cu", [], "sph_probe.o"), ("sph_accel.cu", [], "sph_accel.o"),
+           ("sph_probe.cu", [], "sph_probe.o"), ("sph_static.cu", [], "sph_static.o"), ("sph_accel.cu", [], "sph_accel.o"),
            ("sph_accel.cu", ["-DSPH_ACCEL_KERNEL=0"], "sph_accel_k0.o"),
            ("sph_accel.cu", ["-DSPH_ACCEL_KERNEL=1"], "sph_accel_k1.o"),
            ("sph_accel.cu", ["-DSPH_ACCEL_KERNEL=2"], "sph_accel_k2.o")]
