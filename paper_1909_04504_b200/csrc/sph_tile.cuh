@@ -29,6 +29,7 @@
 // replay them (tile_replay: one bulk copy per block), apply the exact predicate and walk nothing.
 #pragma once
 #include "sph_ctx.cuh"
+#include <cstddef>
 #include <type_traits>
 
 #define TILE_BLOCK 128
@@ -62,15 +63,19 @@
 template <int MM>
 struct __align__(16) TileWarpSmemT {
     static constexpr int MMAX = MM;
-    union {
-        float2 G[4][34];                   // B operands of one batch: G[t][c] = (feature t, feature t+4) of staged candidate c
-        float Af[32 * 9];                  // A operands of a group while the quads exchange them (stride 9: conflict-free)
-    };
     // the image of one record block, in the layout of the pool (so that a replaying warp fetches a block with ONE
     // bulk copy): header row, shift-code row, mask rows
     uint32_t hdr[32];                      // [0] next block, [1] batches | flags, [2 + m] first sorted index of batch m
     uint32_t bcode[32];                    // image-shift code of every batch (2 bits per axis: 1 -> -L, 2 -> +L)
-    uint32_t mask[MM][32];                 // candidate masks, [batch][lane]
+    uint32_t mask[MM][32];                 // candidate masks, [batch][lane]: bit 31 - c = candidate c of the batch (most
+                                           // significant bit first, so that a pop is one count-leading-zeros)
+    // Directly behind the masks, so that zero_row is "mask row MM": the row the sentinel bit of nz points at.  The
+    // drains clear it when they start; G / Af are dead while a drain runs (every batch stages G anew).
+    union {
+        float2 G[4][34];                   // B operands of one batch: G[t][c] = (feature t, feature t+4) of the candidate in column c
+        float Af[32 * 9];                  // A operands of a group while the quads exchange them (stride 9: conflict-free)
+        uint32_t zero_row[32];
+    };
     unsigned long long bar;                // mbarrier of the bulk copy
     uint32_t seg_s[32], seg_e[32], seg_c[32];   // candidate runs of the current pass: [s, e) and image-shift code
     // warp-uniform walker state that only the (cold) group / level / pass set-up code touches: kept here, not in
@@ -78,11 +83,18 @@ struct __align__(16) TileWarpSmemT {
     float bb[8];                           // group bounding box xmin, xmax, ymin, ymax, zmin, zmax, largest h, half extent
     int lv[8];                             // level ranges x0, x1, y0, z0, ny, entries, nparts | low << 8 | high << 9
     float inv_ny;
+    // mask row m of this lane, m in [0, MM]; row MM is the zero row
+    __device__ __forceinline__ uint32_t mask_row(int m, int lane) const { return (&mask[0][0])[m * 32 + lane]; }
 };
+
+static_assert(offsetof(TileWarpSmemT<TILE_MMAX_VARH>, zero_row) == offsetof(TileWarpSmemT<TILE_MMAX_VARH>, mask) + TILE_MMAX_VARH * 128 &&
+              offsetof(TileWarpSmemT<TILE_MMAX_CONSTH>, zero_row) == offsetof(TileWarpSmemT<TILE_MMAX_CONSTH>, mask) + TILE_MMAX_CONSTH * 128 &&
+              offsetof(TileWarpSmemT<TILE_MMAX_VARH>, hdr) == 0 && TILE_MMAX_VARH <= 30 && TILE_MMAX_CONSTH <= 30,
+              "record block image at offset 0; the zero row directly behind the mask rows");
 
 struct TileState {
     int M;                                 // masks stored since the last drain (warp-uniform)
-    uint32_t nz;                           // bit m: this lane's mask m is not empty
+    uint32_t nz;                           // bit 31 - m: this lane's mask m is not empty
     bool shifted;                          // some stored batch came from a periodic image (warp-uniform)
     unsigned tests;                        // candidates streamed for this lane's particle
     __device__ __forceinline__ void reset() { M = 0; nz = 0u; shifted = false; }
@@ -103,6 +115,11 @@ __device__ __forceinline__ float ord2f(uint32_t o) {
 }
 __device__ __forceinline__ float warp_min_f(float v) { return ord2f(__reduce_min_sync(SPH_FULL_MASK, f2ord(v))); }
 __device__ __forceinline__ float warp_max_f(float v) { return ord2f(__reduce_max_sync(SPH_FULL_MASK, f2ord(v))); }
+
+// x >> s with the hardware's semantics for s >= 32 (0), which C++ leaves undefined
+__device__ __forceinline__ uint32_t shr_u32(uint32_t x, int s) {
+    uint32_t r; asm("shr.u32 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(s)); return r;
+}
 
 // minimum-image shift of a batch on one axis from its code: d = fl(x_i - x_j) - shift (R7)
 template <class T>
@@ -296,8 +313,9 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         n = valid ? n : 1.0e30f;                                // padding never passes
         const float nh = tf32r(n), nl = tf32r(n - nh);
         __syncwarp();                                           // readers of the previous batch are done
-        ws.G[0][lane] = make_float2(xt, 1.0f); ws.G[1][lane] = make_float2(yt, 1.0f);
-        ws.G[2][lane] = make_float2(zt, nh);   ws.G[3][lane] = make_float2(ht, nl);
+        const int slot = 31 - lane;                              // candidate c -> column 31 - c -> bit 31 - c of the masks
+        ws.G[0][slot] = make_float2(xt, 1.0f); ws.G[1][slot] = make_float2(yt, 1.0f);
+        ws.G[2][slot] = make_float2(zt, nh);   ws.G[3][slot] = make_float2(ht, nl);
         __syncwarp();
         uint32_t pm0 = 0u, pm1 = 0u, pm2 = 0u, pm3 = 0u;        // sign bits of the quad's particles 0..3 (this thread's columns)
 #pragma unroll
@@ -324,7 +342,7 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         uint32_t mask = __byte_perm(__byte_perm(P, s1, selA), __byte_perm(s2, s3, selB), selC);
         if (!ing) mask = 0u;
         ws.mask[st.M][lane] = mask;
-        if (mask) st.nz |= 1u << st.M;
+        if (mask) st.nz |= 0x80000000u >> st.M;
         if (lane == 0) { ws.hdr[2 + st.M] = cb0; ws.bcode[st.M] = ccode; }
         if (ing) st.tests += (unsigned)min(32u, ce - cb0);
         ++st.M;
@@ -362,7 +380,8 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
 }
 
 // Every lane pops its own candidates of the stored batches in order (nz: the lane's non-empty masks) and evaluates
-// them.  Branch-free and software-pipelined: DEPTH candidates are in flight, the source data of a later one is
+// them.  A pop is two count-leading-zeros: masks and nz are stored most significant bit first, nz carries a
+// sentinel bit that points at an all-zero mask row, so a lane that has run out needs no test of its own.  Branch-free and software-pipelined: DEPTH candidates are in flight, the source data of a later one is
 // gathered (Src = load(sorted index)) before the current one is computed, so the gather latency overlaps the
 // arithmetic.  A lane that has run out keeps executing with has = false and the harmless index `idle` (its own
 // particle) until the slowest lane of the warp is done; compute(src, has, code, per) must apply the exact
@@ -372,15 +391,19 @@ __device__ __forceinline__ void tile_drain(WS& ws, uint32_t nz, uint32_t idle, L
     const int lane = threadIdx.x & 31;
     __syncwarp();
     uint32_t cur = 0u, b = 0u, code = 0u;
+    constexpr uint32_t SENT = 0x80000000u >> WS::MMAX;      // sentinel: when the lane's masks are used up m = MMAX, the zero row
+    ws.zero_row[lane] = 0u;                                 // (a lane reads its own column only: no warp sync needed)
+    nz |= SENT;
     auto pop = [&](bool& has, uint32_t& cd) -> uint32_t {
-        const bool refill = cur == 0u && nz != 0u;
-        const int m = max(__ffs(nz) - 1, 0);
-        const uint32_t nm = ws.mask[m][lane], nb = ws.hdr[2 + m];
-        cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? (nz & (nz - 1u)) : nz;
+        const bool refill = cur == 0u;
+        const int m = __clz(nz);                            // the lane's next non-empty mask (bits are most significant first)
+        const uint32_t nm = ws.mask_row(m, lane), nb = ws.hdr[2 + m];   // (m = MMAX: nb is a word of the next row, unused)
+        cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? ((nz & shr_u32(0x7fffffffu, m)) | SENT) : nz;
         if (PER) { const uint32_t nc = ws.bcode[m]; code = refill ? nc : code; }
         has = cur != 0u;
-        const uint32_t j = has ? b + (uint32_t)(__ffs(cur) - 1) : idle;
-        cur &= cur - 1u;                        // stays 0 when it is 0
+        const int t = __clz(cur);                           // its next candidate; 32 when there is none
+        const uint32_t j = has ? b + (uint32_t)t : idle;
+        cur &= shr_u32(0x7fffffffu, t);                     // stays 0 when it is 0
         cd = code;
         return j;
     };
@@ -412,15 +435,19 @@ __device__ __forceinline__ void tile_drain2(WS& ws, uint32_t nz, uint32_t idle, 
     const int lane = threadIdx.x & 31;
     __syncwarp();
     uint32_t cur = 0u, b = 0u, code = 0u;
+    constexpr uint32_t SENT = 0x80000000u >> WS::MMAX;      // sentinel: when the lane's masks are used up m = MMAX, the zero row
+    ws.zero_row[lane] = 0u;                                 // (a lane reads its own column only: no warp sync needed)
+    nz |= SENT;
     auto pop = [&](bool& has, uint32_t& cd) -> uint32_t {
-        const bool refill = cur == 0u && nz != 0u;
-        const int m = max(__ffs(nz) - 1, 0);
-        const uint32_t nm = ws.mask[m][lane], nb = ws.hdr[2 + m];
-        cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? (nz & (nz - 1u)) : nz;
+        const bool refill = cur == 0u;
+        const int m = __clz(nz);                            // the lane's next non-empty mask (bits are most significant first)
+        const uint32_t nm = ws.mask_row(m, lane), nb = ws.hdr[2 + m];   // (m = MMAX: nb is a word of the next row, unused)
+        cur = refill ? nm : cur; b = refill ? nb : b; nz = refill ? ((nz & shr_u32(0x7fffffffu, m)) | SENT) : nz;
         if (PER) { const uint32_t nc = ws.bcode[m]; code = refill ? nc : code; }
         has = cur != 0u;
-        const uint32_t j = has ? b + (uint32_t)(__ffs(cur) - 1) : idle;
-        cur &= cur - 1u;                        // stays 0 when it is 0
+        const int t = __clz(cur);                           // its next candidate; 32 when there is none
+        const uint32_t j = has ? b + (uint32_t)t : idle;
+        cur &= shr_u32(0x7fffffffu, t);                     // stays 0 when it is 0
         cd = code;
         return j;
     };
@@ -519,7 +546,7 @@ __device__ __forceinline__ void tile_replay(const GridDesc& g, const NList& nl, 
         SPH_DBG_ASSERT(blk < nl.pool_rows && M >= 1 && M <= WS::MMAX && (unsigned long long)blk + (unsigned)M + 2u <= nl.pool_rows, g);
         uint32_t nz = 0u;
         if (active)                                                      // a lane that is no destination of this pass drops its masks
-            for (int m = 0; m < M; ++m) if (ws.mask[m][lane]) nz |= 1u << m;
+            for (int m = 0; m < M; ++m) if (ws.mask[m][lane]) nz |= 0x80000000u >> m;
         drain(nz, shifted);
         blk = next;
     }
