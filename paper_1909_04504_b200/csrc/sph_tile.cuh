@@ -124,8 +124,8 @@ __device__ __forceinline__ uint32_t shr_u32(uint32_t x, int s) {
 // minimum-image shift of a batch on one axis from its code: d = fl(x_i - x_j) - shift (R7)
 template <class T>
 __device__ __forceinline__ T img_shift(uint32_t code, int axis, T L) {
-    const uint32_t c = (code >> (2 * axis)) & 3u;
-    return c == 1u ? -L : (c == 2u ? L : T(0));
+    const T lo = (code & (1u << (2 * axis))) ? -L : T(0);           // two selects on single bits: no branch per candidate
+    return (code & (2u << (2 * axis))) ? L : lo;
 }
 
 // D = A (16 x 8, tf32, row) * B (8 x 8, tf32, col), fp32 accumulators starting from zero
