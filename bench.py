@@ -161,6 +161,21 @@ def ncu_traffic(kernel: str, workload: str):
     return None, "no committed ncu capture of this kernel on this workload"
 
 
+def ncu_limiter(kernel: str, workload: str):
+    """What the committed ncu capture shows to hold the kernel (columns 6-7 of profiles/r2_dram_traffic.csv:
+    l1tex__data_pipe_lsu_wavefronts and smsp__issue_active, % of peak); not measured in this run."""
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 7 and f[0] == kernel and f[1] == workload:
+                return {"l1_lsu_data_pipe_pct_of_peak": float(f[5]), "issue_slots_pct_of_peak": float(f[6]), "source": f[4] + "; not measured in this run",
+                        "note": "the replaying pair kernels are held by the L1 LSU data pipe (one cycle per 128-byte line a gather touches) "
+                                "with the issue slots close behind; the search by issue / the ALU pipe (DESIGN.md 'What bounds them')"}
+    except (OSError, ValueError):
+        pass
+    return None
+
+
 def aggregate(elapsed_ms: float, units: float, world: int):
     """max-over-ranks time and summed units (replicas): returns (ms, total_units).  gloo/nccl all_reduce."""
     if world <= 1:
@@ -389,7 +404,7 @@ def report(name, r, K, world, ms_max, units, e2e_agg, fp32_peak, hbm_peak, hbm_s
         tot_ms = sum(kprof[k]["ms"] / K for k in alu)
         roofline = {"kernel": dom, "bound": "alu", "achieved": alu[dom]["tflops"], "peak": peak_tf, "unit": "TFLOP/s",
                     "frac": alu[dom]["frac"], "traffic": traffic, "traffic_source": tsrc, "peak_source": peak_src,
-                    "algorithmic_flops_per_launch": alu[dom]["flops"],
+                    "algorithmic_flops_per_launch": alu[dom]["flops"], "ncu_limiter": ncu_limiter(dom, name),
                     "counts": "k_search: min(candidates of the paper's cell-list search (sph_stencil_candidates on this state: "
                               f"{r['stencil']} = {r['stencil'] / max(N, 1):.0f} per particle), candidates streamed) x {c_test} flop; pair passes: true pairs x "
                               f"{pair_d} (density) / {pair_a} (momentum) flop; this library streamed {stats.candidates} candidates "
