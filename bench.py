@@ -426,9 +426,13 @@ def report(name, r, K, world, ms_max, units, e2e_agg, fp32_peak, hbm_peak, hbm_s
             hbm[k] = {"bytes_per_particle": bpp, "achieved_gbs": gbs, "peak_gbs": hbm_peak, "frac": gbs / hbm_peak, "peak_source": hbm_src,
                       "l2_resident": bool(state_bytes < L2_BYTES)}
     if "k_scan" in kernels:
-        gbs = 12.0 * stats.n_keys / (kernels["k_scan"]["ms_per_launch"] * 1e-3) / 1e9
+        # tables of >= 1024 tiles are scanned by three launches (tile sums, their scan, the pass that applies them: the
+        # table is read twice); the algorithmic bytes stay 12 per key (counts read, offsets written, counts cleared)
+        parts = [k for k in ("k_scan_reduce", "k_scan_tiles", "k_scan") if k in kernels]
+        scan_ms = sum(kernels[k]["ms_per_launch"] for k in parts)
+        gbs = 12.0 * stats.n_keys / (scan_ms * 1e-3) / 1e9
         hbm["k_scan"] = {"bytes_per_key": 12, "keys": int(stats.n_keys), "achieved_gbs": gbs, "peak_gbs": hbm_peak, "frac": gbs / hbm_peak,
-                         "peak_source": hbm_src, "l2_resident": bool(12.0 * stats.n_keys < L2_BYTES)}
+                         "peak_source": hbm_src, "l2_resident": bool(12.0 * stats.n_keys < L2_BYTES), "launches": parts, "ms": scan_ms}
     pairs_per_step = stats.pairs_density + stats.pairs_accel
     out = {"workload": workload_label(name), "particles_per_gpu": N, "density_mode": r["mode"], "kernel": wl.kernel, "dim": wl.dim,
            "value": units / (ms_max * 1e-3), "unit": UNIT, "ms_per_step": ms_max / K,

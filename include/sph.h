@@ -169,6 +169,8 @@ enum sph_kernel_id {
     SPH_K_SEARCH = 10,          /* neighbour search of one sorted order: tensor-core filter -> mask records */
     SPH_K_DENSITY_LIST = 11,    /* a4 + a5 replayed over the candidate masks recorded by the search */
     SPH_K_UPDATE_KICK = 12,     /* a8, eq.14 only (the launch that ends a sph_pc_step call): no drift, no key */
+    SPH_K_SCAN_REDUCE = 13,     /* a2, tables of >= 1024 tiles: per-tile sums (SPH_K_SCAN is then the pass that applies them) */
+    SPH_K_SCAN_TILES = 14,      /* a2, tables of >= 1024 tiles: exclusive scan of the tile sums (one block)     */
     SPH_K_COUNT = 16
 };
 typedef struct sph_profile {

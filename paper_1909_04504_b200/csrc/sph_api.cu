@@ -116,6 +116,8 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_dom
     const size_t scan_n = (size_t)(c->max_keys > tot ? c->max_keys : tot) + 2;
     SPH_CUDA_OK(c, cudaMalloc(&c->scan_state, (scan_n / 2048 + 4) * sizeof(unsigned long long)));
     SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_state, 0, (scan_n / 2048 + 4) * sizeof(unsigned long long), c->stream));
+    c->scan_tiles_cap = (int)(scan_n / 4096 + 2);
+    SPH_CUDA_OK(c, cudaMalloc(&c->scan_tiles, 2 * (size_t)(c->scan_tiles_cap + 1) * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMalloc(&c->scan_ticket, 2 * sizeof(uint32_t)));
     SPH_CUDA_OK(c, cudaMemsetAsync(c->scan_ticket, 0, 2 * sizeof(uint32_t), c->stream));
     SPH_CUDA_OK(c, cudaMalloc(&c->staging, N * N_STAGE_FIELDS * sizeof(real)));
@@ -144,7 +146,7 @@ extern "C" int sph_destroy(sph_ctx* c) {
     }
     cudaFree(c->S[0].acc); cudaFree(c->S[1].acc); cudaFree(c->key); cudaFree(c->rank); cudaFree(c->cell_count); cudaFree(c->cell_start);
     cudaFree(c->nl.pool); cudaFree(c->nl.head);
-    cudaFree(c->scan_state); cudaFree(c->scan_ticket); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
+    cudaFree(c->scan_state); cudaFree(c->scan_ticket); cudaFree(c->scan_tiles); cudaFree(c->staging); cudaFree(c->counters); cudaFree(c->hminmax);
     if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
     for (int k = 0; k < c->prof_cap; ++k) { cudaEventDestroy(c->prof[k].a); cudaEventDestroy(c->prof[k].b); }
     free(c->prof);
@@ -617,6 +619,8 @@ extern "C" const char* sph_kernel_name(int id) {
         case SPH_K_KEY: return "k_key_hist";
         case SPH_K_UPDATE: return "k_update";
         case SPH_K_SCAN: return "k_scan";
+        case SPH_K_SCAN_REDUCE: return "k_scan_reduce";
+        case SPH_K_SCAN_TILES: return "k_scan_tiles";
         case SPH_K_SCATTER: return "k_scatter";
         case SPH_K_DENSITY: return "k_density";
         case SPH_K_ACCEL: return "k_accel";

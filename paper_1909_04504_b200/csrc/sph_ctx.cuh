@@ -33,6 +33,7 @@ struct sph_ctx {
     uint32_t *key, *rank;      // per particle, pre-sort order
     uint32_t *cell_count, *cell_start;
     unsigned long long* scan_state; uint32_t* scan_ticket;   // k_scan look-back table; scan_ticket[0] = ticket, [1] = epoch
+    uint32_t* scan_tiles; int scan_tiles_cap;                // two-level scan of large tables: tile sums [cap + 1] and tile prefixes [cap + 1]
     real* staging;             // host<->device staging for SPH_MEM_HOST (14 reals per particle of capacity)
     unsigned long long* counters;     // device, CNT_COUNT entries
     void* hminmax;             // device, 4 x 8 bytes: h min/max, |m| min/max as ordered integers of the real type

@@ -261,9 +261,103 @@ k_scan(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, int n
     }
 }
 
+// Large tables (>= SCAN_TWO_LEVEL_TILES tiles): reduce -> scan of the tile sums -> scan with the known tile prefix.
+// It reads the table twice (16 B per key with the clearing instead of 12) but has no look-back: in the single-pass
+// kernel a tile holds its SM slot for ~11 us, 7 of them waiting for the flags of its predecessors (ncu: `barrier`
+// stalls; a microbenchmark of the same kernel without the look-back runs at 4.9 TB/s, with it at 2.0), whatever the
+// width of the look-back window.  Small tables keep the single launch.
+#ifndef SCAN_TWO_LEVEL_TILES
+#define SCAN_TWO_LEVEL_TILES 1024
+#endif
+__global__ void __launch_bounds__(SCAN_T)
+k_scan_reduce(const uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ tile_sum) {
+    __shared__ uint32_t s_w[SCAN_T / 32];
+    const long long i0 = (long long)blockIdx.x * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
+    uint32_t s = 0;
+    if (i0 + SCAN_ITEMS <= n) {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; k += 4) { const uint4 q = *reinterpret_cast<const uint4*>(in + i0 + k); s += q.x + q.y + q.z + q.w; }
+    } else {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) s += (i0 + k < n) ? in[i0 + k] : 0u;
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(SPH_FULL_MASK, s, o);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        uint32_t t = threadIdx.x < SCAN_T / 32 ? s_w[threadIdx.x] : 0u;
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(SPH_FULL_MASK, t, o);
+        if (threadIdx.x == 0) tile_sum[blockIdx.x] = t;
+    }
+}
+
+// one block: tile_prefix[t] = sum of tile_sum[0..t), tile_prefix[nb] = total (nb <= 1024 * 64)
+__global__ void __launch_bounds__(1024)
+k_scan_tiles(const uint32_t* __restrict__ tile_sum, int nb, uint32_t* __restrict__ tile_prefix) {
+    __shared__ uint32_t s_w[32];
+    const int per = (nb + 1023) / 1024, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int b = threadIdx.x * per, e = min(b + per, nb);
+    uint32_t s = 0;
+    for (int k = b; k < e; ++k) s += tile_sum[k];
+    uint32_t inc = s;
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(SPH_FULL_MASK, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) s_w[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        const uint32_t v = s_w[lane]; uint32_t vi = v;
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(SPH_FULL_MASK, vi, o); if (lane >= o) vi += t; }
+        s_w[lane] = vi - v;
+        if (lane == 31) tile_prefix[nb] = vi;
+    }
+    __syncthreads();
+    uint32_t run = s_w[w] + inc - s;
+    for (int k = b; k < e; ++k) { tile_prefix[k] = run; run += tile_sum[k]; }
+}
+
+__global__ void __launch_bounds__(SCAN_T)
+k_scan_apply(uint32_t* __restrict__ in, long long n, uint32_t* __restrict__ out, const uint32_t* __restrict__ tile_prefix, int nb, int zero_in) {
+    __shared__ uint32_t s_total;
+    const long long i0 = (long long)blockIdx.x * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
+    uint32_t v[SCAN_ITEMS], s = 0;
+    const bool full = i0 + SCAN_ITEMS <= n;
+    if (full) {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; k += 4) {
+            const uint4 q = *reinterpret_cast<const uint4*>(in + i0 + k);
+            v[k] = q.x; v[k + 1] = q.y; v[k + 2] = q.z; v[k + 3] = q.w; s += q.x + q.y + q.z + q.w;
+            if (zero_in) *reinterpret_cast<uint4*>(in + i0 + k) = make_uint4(0u, 0u, 0u, 0u);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (i0 + k < n) ? in[i0 + k] : 0u; s += v[k]; }
+        if (zero_in) {
+#pragma unroll
+            for (int k = 0; k < SCAN_ITEMS; ++k) if (i0 + k < n) in[i0 + k] = 0u;
+        }
+    }
+    uint32_t ex = block_exclusive_scan(s, &s_total) + __ldg(tile_prefix + blockIdx.x);
+    if ((int)blockIdx.x == nb - 1 && threadIdx.x == 0) out[n] = __ldg(tile_prefix + nb);
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { const uint32_t e = ex; ex += v[k]; v[k] = e; }
+    if (full) {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; k += 4) *reinterpret_cast<uint4*>(out + i0 + k) = make_uint4(v[k], v[k + 1], v[k + 2], v[k + 3]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) if (i0 + k < n) out[i0 + k] = v[k];
+    }
+}
+
 static int scan_exclusive(sph_ctx* c, uint32_t* in, uint32_t* out, long long n, bool zero_in) {
     const int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
     if (nb == 0) { SPH_CUDA_OK(c, cudaMemsetAsync(out, 0, sizeof(uint32_t), c->stream)); return SPH_OK; }
+    if (nb >= SCAN_TWO_LEVEL_TILES && nb <= c->scan_tiles_cap) {
+        uint32_t* tile_sum = c->scan_tiles; uint32_t* tile_prefix = c->scan_tiles + c->scan_tiles_cap + 1;
+        SPH_LAUNCH(c, SPH_K_SCAN_REDUCE, k_scan_reduce, nb, SCAN_T, 0, in, n, tile_sum);
+        SPH_LAUNCH(c, SPH_K_SCAN_TILES, k_scan_tiles, 1, 1024, 0, tile_sum, nb, tile_prefix);
+        SPH_LAUNCH(c, SPH_K_SCAN, k_scan_apply, nb, SCAN_T, 0, in, n, out, tile_prefix, nb, zero_in ? 1 : 0);
+        return SPH_OK;
+    }
     SPH_LAUNCH(c, SPH_K_SCAN, k_scan, nb, SCAN_T, 0, in, n, out, nb, c->scan_state, c->scan_ticket, zero_in ? 1 : 0);
     return SPH_OK;
 }
