@@ -53,6 +53,7 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const real visc = pc.visc, eps = pc.eps, nu4 = pc.nu4, eta = pc.eta;
     const real hi = VARH ? pi.w : h_c;
     const real cut2c = pair_cut2(kh, h_c, h_c);
+    const real sigma5 = real(-5) * sigma, cw_c = real(-5) * fac_c * hinv_c * hinv_c;   // Wendland-C2: sigma h^-(d+2) f'(q)/q = cw (1 - q/2)^3
     // PM: where the neighbour's rho and p/rho^2 come from (the loop is L1-gather bound: fewer gathers pay).
     //   0  gathered from rp (caller-supplied p, gamma != 7 ...): three gathers
     //   1  gamma = 7, every p is the EOS of its rho, and velm.w carries rho (constant h, or variable h with uniform
@@ -84,15 +85,22 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         nhits += has ? 1u : 0u;
         const real rinv = r2 > 0.0f ? rsqrt_approx(r2) : real(0);       // grad W := 0 at r = 0 (R18): rinv = 0
         const real r = r2 * rinv;
-        real hij, hinv, fac;
-        if (VARH) {
-            hij = 0.5f * (hi + s.pj.w);
-            hinv = rcp_approx(hij);
-            fac = sigma * hinv * hinv * (DIM == 3 ? hinv : real(1));
-        } else { hij = h_c; hinv = hinv_c; fac = fac_c; }
-        real f, df;
-        kernel_profile<KERNEL, DIM>(r * hinv, f, df);
-        const real gc = fac * hinv * df * rinv;                        // grad_i W_ij = gc * (dx,dy,dz)
+        real hij, hinv;
+        if (VARH) { hij = 0.5f * (hi + s.pj.w); hinv = rcp_approx(hij); } else { hij = h_c; hinv = hinv_c; }
+        real gc;                                                        // grad_i W_ij = gc * (dx,dy,dz)
+        if (KERNEL == SPH_KERNEL_WENDLAND_C2 && DIM > 1) {
+            // f'(q)/q = -5 (1 - q/2)^3 is a polynomial, so gc = sigma h^-(d+2) f'(q)/q needs no 1/r (at r = 0 the
+            // term vanishes with dx = dy = dz = 0, R18)
+            const real t = rmax(rfma(real(-0.5), r * hinv, real(1)), real(0));
+            const real hinv2 = hinv * hinv;
+            const real cw = VARH ? sigma5 * (hinv2 * hinv2) * (DIM == 3 ? hinv : real(1)) : cw_c;
+            gc = cw * (t * t * t);
+        } else {
+            const real fac = VARH ? sigma * hinv * hinv * (DIM == 3 ? hinv : real(1)) : fac_c;
+            real f, df;
+            kernel_profile<KERNEL, DIM>(r * hinv, f, df);
+            gc = fac * hinv * df * rinv;
+        }
         const real vx = vi.x - s.vj.x, vy = vi.y - s.vj.y;
         real vr = rfma(vy, dy, vx * dx);
         if (DIM == 3) vr = rfma(vi.z - s.vj.z, dz, vr);
