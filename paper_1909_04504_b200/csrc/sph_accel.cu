@@ -53,7 +53,10 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
     const real visc = pc.visc, eps = pc.eps, nu4 = pc.nu4, eta = pc.eta;
     const real hi = VARH ? pi.w : h_c;
     const real cut2c = pair_cut2(kh, h_c, h_c);
-    const real sigma5 = real(-5) * sigma, cw_c = real(-5) * fac_c * hinv_c * hinv_c;   // Wendland-C2: sigma h^-(d+2) f'(q)/q = cw (1 - q/2)^3
+    // Wendland-C2: sigma h^-(d+2) f'(q)/q = cw (1 - q/2)^3, times the mass where every particle has the same one
+    constexpr bool MCONST = PM == 2 || (VARH && PM == 1);
+    const real mw = MCONST ? pc.m_const : real(1);
+    const real sigma5 = real(-5) * sigma * mw, cw_c = real(-5) * fac_c * hinv_c * hinv_c * mw;
     // PM: where the neighbour's rho and p/rho^2 come from (the loop is L1-gather bound: fewer gathers pay).
     //   0  gathered from rp (caller-supplied p, gamma != 7 ...): three gathers
     //   1  gamma = 7, every p is the EOS of its rho, and velm.w carries rho (constant h, or variable h with uniform
@@ -83,35 +86,35 @@ k_accel_tile(GridDesc g, PairConsts pc, SortedState S, const uint32_t* __restric
         has = has && r2 < (VARH ? pair_cut2(kh, hi, s.pj.w) : cut2c);
         if (FILTER) has = has && (my_mask == pc.all_mask || ((my_mask >> s.aid) & 1u));
         nhits += has ? 1u : 0u;
-        const real rinv = r2 > 0.0f ? rsqrt_approx(r2) : real(0);       // grad W := 0 at r = 0 (R18): rinv = 0
-        const real r = r2 * rinv;
         real hij, hinv;
         if (VARH) { hij = 0.5f * (hi + s.pj.w); hinv = rcp_approx(hij); } else { hij = h_c; hinv = hinv_c; }
-        real gc;                                                        // grad_i W_ij = gc * (dx,dy,dz)
+        // SortedState layouts: where m, rho and p/rho^2 of the neighbour ride
+        const real mj = PM == 2 ? m_const : (VARH ? (PM == 1 ? m_const : s.vj.w) : s.pj.w);
+        real mgc;                                                       // m_j grad_i W_ij = mgc * (dx,dy,dz)
         if (KERNEL == SPH_KERNEL_WENDLAND_C2 && DIM > 1) {
-            // f'(q)/q = -5 (1 - q/2)^3 is a polynomial, so gc = sigma h^-(d+2) f'(q)/q needs no 1/r (at r = 0 the
-            // term vanishes with dx = dy = dz = 0, R18)
-            const real t = rmax(rfma(real(-0.5), r * hinv, real(1)), real(0));
+            // f'(q)/q = -5 (1 - q/2)^3 is a polynomial, so sigma h^-(d+2) f'(q)/q needs no 1/r (at r = 0 the term
+            // vanishes with dx = dy = dz = 0, R18); a uniform mass rides in the constant
+            const real t = rmax(rfma(real(-0.5), sqrt_approx(r2) * hinv, real(1)), real(0));
             const real hinv2 = hinv * hinv;
             const real cw = VARH ? sigma5 * (hinv2 * hinv2) * (DIM == 3 ? hinv : real(1)) : cw_c;
-            gc = cw * (t * t * t);
+            mgc = cw * (t * t * t);
+            if (!MCONST) mgc *= mj;
         } else {
+            const real rinv = r2 > 0.0f ? rsqrt_approx(r2) : real(0);   // grad W := 0 at r = 0 (R18): rinv = 0
             const real fac = VARH ? sigma * hinv * hinv * (DIM == 3 ? hinv : real(1)) : fac_c;
             real f, df;
-            kernel_profile<KERNEL, DIM>(r * hinv, f, df);
-            gc = fac * hinv * df * rinv;
+            kernel_profile<KERNEL, DIM>(r2 * rinv * hinv, f, df);
+            mgc = mj * (fac * hinv * df * rinv);
         }
         const real vx = vi.x - s.vj.x, vy = vi.y - s.vj.y;
         real vr = rfma(vy, dy, vx * dx);
         if (DIM == 3) vr = rfma(vi.z - s.vj.z, dz, vr);
-        // SortedState layouts: where m, rho and p/rho^2 of the neighbour ride
-        const real mj = PM == 2 ? m_const : (VARH ? (PM == 1 ? m_const : s.vj.w) : s.pj.w);
         const real rho_j = PM ? s.vj.w : s.rj.x;
         const real pr_j = PM == 2 ? s.pj.w : (PM == 1 ? eos7_p_over_rho2(rho_j, rho0, inv_rho0, Beos) : s.rj.y);
         // Pi_ij = -alpha c0 mu / rhobar, mu = h vr/(r^2 + eps h^2), rhobar = (rho_i+rho_j)/2, only if vr < 0
         const real den = rfma(eps * hij, hij, r2) * (rho_i + rho_j);
         const real Pi = vr < real(0) ? visc * hij * vr * rcp_approx(den) : real(0);
-        const real mg = has ? mj * gc : real(0);                          // a lane that has run out contributes nothing
+        const real mg = has ? mgc : real(0);                              // a lane that has run out contributes nothing
         const real sc = -mg * (pr_i + pr_j + Pi);
         ax = rfma(sc, dx, ax); ay = rfma(sc, dy, ay);
         if (DIM == 3) az = rfma(sc, dz, az);

@@ -120,6 +120,8 @@ struct SortedState {
 __device__ __forceinline__ float rcp_approx(float x)  { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_approx(float x){ float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
+__device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ double sqrt_approx(double x) { return sqrt(x); }
 __device__ __forceinline__ double rcp_approx(double x)  { return 1.0 / x; }
 __device__ __forceinline__ double rsqrt_approx(double x){ return 1.0 / sqrt(x); }
 __device__ __forceinline__ float  rfma(float a, float b, float c)    { return fmaf(a, b, c); }

@@ -166,11 +166,8 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
     const unsigned brkmask = __ballot_sync(SPH_FULL_MASK, brk);
     unsigned remaining = __ballot_sync(SPH_FULL_MASK, active);
 
-    // per-thread constants of the mask transpose and of the B-operand fetch
-    const uint32_t selA = ((uint32_t)tq << (4 * tq)) | ((uint32_t)(4 + tq) << (4 * (tq ^ 1)));
-    const uint32_t selB = ((uint32_t)tq << (4 * (tq ^ 2))) | ((uint32_t)(4 + tq) << (4 * (tq ^ 3)));
-    const uint32_t selC = ((uint32_t)tq << (4 * tq)) | ((uint32_t)(tq ^ 1) << (4 * (tq ^ 1))) |
-                          ((uint32_t)(4 + (tq ^ 2)) << (4 * (tq ^ 2))) | ((uint32_t)(4 + (tq ^ 3)) << (4 * (tq ^ 3)));
+    // per-thread constants of the mask transpose (two butterfly rounds inside the quad) and of the B-operand fetch
+    const uint32_t sel1 = (tq & 1) ? 0x3715u : 0x6240u, sel2 = (tq & 2) ? 0x3276u : 0x5410u;
     const int cidx = 8 * (gq >> 1) + 7 - (gq & 1);           // column g of N-tile nt holds staged candidate cidx - 2 nt
 
     // ---- group state (warp-uniform unless noted); the cold part lives in ws.bb / ws.lv
@@ -298,8 +295,11 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
         __syncwarp();
     };
 
-    // one batch of <= 32 candidates [cb0, min(cb0 + 32, ce)) against the warp's 32 particles
-    auto process = [&](uint32_t cb0, uint32_t ce, uint32_t ccode, float4 pj) {
+    // one batch of <= 32 candidates [cb0, min(cb0 + 32, ce)) against the warp's 32 particles, in two parts so that the
+    // prefetch of the next batch can overwrite the run state in place (no register copies of cb0 / ce / code / pj):
+    // features(): this lane's candidate -> B-operand features + the batch's header words; filter(): staging, MMAs, masks
+    struct Feat { float xt, yt, zt, ht, nh, nl; };
+    auto features = [&](uint32_t cb0, uint32_t ce, uint32_t ccode, float4 pj) -> Feat {
         const bool valid = cb0 + (uint32_t)lane < ce;
         float xr = pj.x, yr = pj.y, zr = pj.z;
         if (ccode) {                                            // the image of the candidate next to the group: x_j + shift
@@ -307,15 +307,21 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
             if (DIM == 3) zr += img_shift(ccode, 2, g.L[2]);
             st.shifted = true;
         }
-        const float xt = tf32r(xr - ox), yt = tf32r(yr - oy), zt = DIM == 3 ? tf32r(zr - oz) : 0.0f;
-        const float ht = VARH ? tf32r(pj.w) : 0.0f;
-        float n = fmaf(zt, zt, fmaf(yt, yt, xt * xt)) - (VARH ? khsq * ht * ht : 0.0f) - nsub;
+        Feat f;
+        f.xt = tf32r(xr - ox); f.yt = tf32r(yr - oy); f.zt = DIM == 3 ? tf32r(zr - oz) : 0.0f;
+        f.ht = VARH ? tf32r(pj.w) : 0.0f;
+        float n = fmaf(f.zt, f.zt, fmaf(f.yt, f.yt, f.xt * f.xt)) - (VARH ? khsq * f.ht * f.ht : 0.0f) - nsub;
         n = valid ? n : 1.0e30f;                                // padding never passes
-        const float nh = tf32r(n), nl = tf32r(n - nh);
+        f.nh = tf32r(n); f.nl = tf32r(n - f.nh);
+        if (lane == 0) { ws.hdr[2 + st.M] = cb0; ws.bcode[st.M] = ccode; }   // (slot M is free: the last drain consumed it)
+        if (ing) st.tests += (unsigned)min(32u, ce - cb0);
+        return f;
+    };
+    auto filter = [&](const Feat& f) {
         __syncwarp();                                           // readers of the previous batch are done
         const int slot = 31 - lane;                              // candidate c -> column 31 - c -> bit 31 - c of the masks
-        ws.G[0][slot] = make_float2(xt, 1.0f); ws.G[1][slot] = make_float2(yt, 1.0f);
-        ws.G[2][slot] = make_float2(zt, nh);   ws.G[3][slot] = make_float2(ht, nl);
+        ws.G[0][slot] = make_float2(f.xt, 1.0f); ws.G[1][slot] = make_float2(f.yt, 1.0f);
+        ws.G[2][slot] = make_float2(f.zt, f.nh); ws.G[3][slot] = make_float2(f.ht, f.nl);
         __syncwarp();
         uint32_t pm0 = 0u, pm1 = 0u, pm2 = 0u, pm3 = 0u;        // sign bits of the quad's particles 0..3 (this thread's columns)
 #pragma unroll
@@ -336,15 +342,13 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
             }
         }
         // byte q of P: this thread's 8 columns against particle q of the quad; transpose the 4 x 4 bytes of the quad
+        // (byte k of lane t <- byte t of lane k) in two butterfly rounds: 2 x 2 bytes with lane ^ 1, halves with lane ^ 2
         const uint32_t P = __byte_perm(__byte_perm(pm0, pm1, 0x0040), __byte_perm(pm2, pm3, 0x0040), 0x5410);
-        const uint32_t s1 = __shfl_xor_sync(SPH_FULL_MASK, P, 1), s2 = __shfl_xor_sync(SPH_FULL_MASK, P, 2),
-                       s3 = __shfl_xor_sync(SPH_FULL_MASK, P, 3);
-        uint32_t mask = __byte_perm(__byte_perm(P, s1, selA), __byte_perm(s2, s3, selB), selC);
+        const uint32_t Rr = __byte_perm(P, __shfl_xor_sync(SPH_FULL_MASK, P, 1), sel1);
+        uint32_t mask = __byte_perm(Rr, __shfl_xor_sync(SPH_FULL_MASK, Rr, 2), sel2);
         if (!ing) mask = 0u;
         ws.mask[st.M][lane] = mask;
         if (mask) st.nz |= 0x80000000u >> st.M;
-        if (lane == 0) { ws.hdr[2 + st.M] = cb0; ws.bcode[st.M] = ccode; }
-        if (ing) st.tests += (unsigned)min(32u, ce - cb0);
         ++st.M;
     };
 
@@ -363,12 +367,11 @@ __device__ __forceinline__ void tile_walk(const GridDesc& g, const PairConsts& p
                 setup_group(); grp = true; b = -1; npass = 0; pass = 0;
                 continue;
             }
-            const uint32_t cb0 = nb0, ce = ne, ccode = ncode;
-            const float4 pj = pjn;
+            const Feat f = features(nb0, ne, ncode, pjn);
             if (nb0 + 32u < ne) { nb0 += 32u; pjn = load_batch(nb0, ne); }     // prefetch the next batch
             else if (pop_run()) pjn = load_batch(nb0, ne);
             else have = false;
-            process(cb0, ce, ccode, pj);
+            filter(f);
         }
     };
 
