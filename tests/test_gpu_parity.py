@@ -143,3 +143,44 @@ def test_momentum_conservation_on_gpu(O, WL):
         a = a.cpu().numpy().astype(np.float64)
         assert abs((m * a).sum()) < 2e-6 * (m * np.abs(a)).sum()
     ctx.close()
+
+
+@pytest.mark.parametrize("dim,varh", [(2, False), (3, False), (3, True)], ids=["2d", "3d", "3d_varh"])
+def test_coincident_particles_and_uniform_mass_wendland(O, WL, dim, varh):
+    """R18: grad W := 0 at r = 0.  Every tenth particle sits exactly on its predecessor (different velocity, density
+    and h), all masses are equal and no p is supplied, so the momentum pass runs its uniform-mass layouts (UM / VU: the
+    Wendland-C2 gradient from the polynomial f'(q)/q with the mass in its constant, p/rho^2 recomputed when h varies):
+    sets bit-exact, rho and a within 1e-5, the coincident pair adds m W(0) to rho and nothing to a."""
+    wl = WL.random_box(n=1500, dim=dim, periodic=True, seed=60 + dim, kernel="wendland_c2", variable_h=varh)
+    A = wl.arrays[0]
+    A.m[:] = A.m[0]
+    for k in "xyz":
+        c = getattr(A, k)
+        c[1::10] = c[0::10][:len(c[1::10])]
+    ctx, _ = make_ctx(wl)
+    off, idx = ctx.nnps_get_neighbors(0, 0)
+    ooff, oidx = O.neighbors(wl, fields_of(A), fields_of(A), pred32=True, method="cell")
+    assert np.array_equal(off, ooff) and np.array_equal(idx.astype(np.int64), oidx)
+    r = rows(off, idx)
+    assert all(i - 1 in r[i] for i in range(1, A.n, 10))          # the coincident partner is a neighbour
+    st = oracle_state_with_p(O, wl)
+    rho, _ = ctx.summation_density(0, 1)
+    orho, _, opairs = O.density(wl, st, 0, [0], pred32=True)
+    assert_close(rho.cpu().numpy(), orho, "rho")
+    assert ctx.get_stats().pairs_density == opairs
+    ctx.close()
+    ctx, _ = make_ctx(wl)                     # a fresh build: rho as given, p = EOS(rho) on both sides
+    ax, ay, az, ar = ctx.wcsph_accel(0, 1, want_arho=True)
+    o = O.accel(wl, st, 0, [0], pred32=True)
+    scale = max(np.abs(o["au"]).max(), np.abs(o["av"]).max(), np.abs(o["aw"]).max())
+    for name, g_, w_ in (("ax", ax, o["au"]), ("ay", ay, o["av"]), ("az", az, o["aw"])):
+        if g_ is None:
+            continue
+        g = g_.cpu().numpy().astype(np.float64)
+        assert np.isfinite(g).all(), f"{name}: non-finite"
+        err = np.abs(g - w_).max() / scale
+        assert err <= TOL, f"{name}: {err:.3e} of max|a|"
+    assert_close(ar.cpu().numpy(), o["arho"], "arho")
+    assert ctx.get_stats().pairs_accel == o["n_pairs"]
+    ctx.synchronize()
+    ctx.close()
