@@ -129,6 +129,37 @@ def test_two_particle_acceleration_by_hand(O, WL):
     assert o["au"][0] == pytest.approx(a0[0], rel=1e-13)
 
 
+def test_coincident_particle_adds_no_force(O, WL):
+    """R18: grad W := 0 at r = 0.  A third particle placed exactly on particle 0 (other velocity, density,
+    pressure and mass) is a neighbour of it but leaves a_0 and arho_0 at the values written out by hand for the pair
+    (0, 1) above plus ITS OWN pair term with particle 1 -- nothing comes from the coincident pair, and nothing is NaN."""
+    wl, st = _prepared(O, WL, n=3, dim=2, periodic=False, seed=1, kernel="cubic")
+    A = st.arrays[0]
+    A["x"][:] = [0.30, 0.42, 0.30]; A["y"][:] = [0.40, 0.45, 0.40]; A["h"][:] = 0.1; A["m"][:] = [2.0, 3.0, 5.0]
+    A["rho"][:] = [1.1, 0.9, 1.3]; A["p"][:] = [0.7, -0.2, 0.4]
+    A["u"][:] = [1.0, -1.0, 4.0]; A["v"][:] = [0.2, 0.0, -3.0]
+    o = O.accel(wl, st, 0, [0], pred32=False, method="brute")
+    assert o["n_pairs"] == 9 and all(np.isfinite(o[k]).all() for k in ("au", "av", "arho"))
+    d = np.array([-0.12, -0.05]); r = np.hypot(*d); h = 0.1; q = r / h
+    grad0 = 10 / (7 * np.pi) / h ** 3 * (-0.75 * (2 - q) ** 2) * d / r
+    v01 = np.array([2.0, 0.2]); vr = v01 @ d
+    Pi = -wl.alpha * wl.c0 * (h * vr / (r * r + wl.eps * h * h)) / 1.0
+    a0 = -3.0 * (0.7 / 1.1 ** 2 + (-0.2) / 0.9 ** 2 + Pi) * grad0
+    assert o["au"][0] == pytest.approx(a0[0], rel=1e-13) and o["av"][0] == pytest.approx(a0[1], rel=1e-13)
+    assert o["arho"][0] == pytest.approx(3.0 * (v01 @ grad0), rel=1e-13)
+    # particle 2 (same place): only its pair with particle 1 counts
+    v21 = np.array([5.0, -3.0]); vr2 = v21 @ d
+    assert vr2 < 0
+    Pi2 = -wl.alpha * wl.c0 * (h * vr2 / (r * r + wl.eps * h * h)) / (0.5 * (1.3 + 0.9))
+    a2 = -3.0 * (0.4 / 1.3 ** 2 + (-0.2) / 0.9 ** 2 + Pi2) * grad0
+    assert o["au"][2] == pytest.approx(a2[0], rel=1e-13) and o["av"][2] == pytest.approx(a2[1], rel=1e-13)
+    assert o["arho"][2] == pytest.approx(3.0 * (v21 @ grad0), rel=1e-13)
+    # ... while the density does see it: rho_0 = m_0 W(0) + m_2 W(0) + m_1 W(r)
+    rho, _, _ = O.density(wl, st, 0, [0], pred32=False, method="brute")
+    sig = 10.0 / (7.0 * np.pi)
+    assert rho[0] == pytest.approx((2.0 + 5.0) * sig / 0.01 + 3.0 * sig / 0.01 * 0.25 * (2 - q) ** 3, rel=1e-13)
+
+
 def test_gravity_is_the_initial_value(O, WL):
     """Listing 4: the accumulator starts at the body force; an isolated particle gets exactly g."""
     wl, st = _prepared(O, WL, n=2, dim=2, periodic=False, seed=1, g=(0.0, -9.81, 0.0))
