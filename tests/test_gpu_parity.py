@@ -27,11 +27,12 @@ def _small_cases(WL):
         WL.lattice((32, 32), 2, 1.0, "quintic"),          # r = 3 dx = k h exactly on the lattice: strict '<' (R4)
         WL.lattice((16, 16, 16), 3, 1.3, "cubic"),
         WL.taylor_green_2d(),                              # C1
+        WL.random_box(n=900, dim=2, periodic=True, seed=19, kernel="wendland_c2"),              # 2-D Wendland-C2 (sigma_2, h^-4)
     ]
 
 
 CASE_IDS = ["2d_per", "2d_open_varh", "3d_per_varh", "3d_open_two", "3cells", "2d_per_two_varh", "single",
-            "one_cell", "lattice2d_quintic", "lattice3d_cubic", "C1"]
+            "one_cell", "lattice2d_quintic", "lattice3d_cubic", "C1", "2d_per_wendland"]
 
 
 @pytest.fixture(scope="module", params=list(range(len(CASE_IDS))), ids=CASE_IDS)
